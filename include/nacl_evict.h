@@ -1,0 +1,146 @@
+/*
+ * nacl_evict.h -- C ABI of libnacl_evict.so: NACL one-shot encoding-phase KV-cache
+ * eviction (arXiv 2408.03675) as hand-written sm_100a CUDA kernels.
+ *
+ * The operation (PAPER.md = the paper's LaTeX source, cited by line; readings R1..R15
+ * in DESIGN.md section 2).  For every batch element b and kv head hk of one layer:
+ *   1. proxy logits     s[i,j] = Q[b,hq,i,:] . K[b,hk,j,:] / sqrt(d)  for the G = Hq/Hkv
+ *                       query heads hq = hk*G+g of the group and the P proxy rows
+ *                       (Alg.1);
+ *   2. importance       imp[j] = sum_{g,i} Softmax_j(s[i,:])[j]   -- F_score, a full-length
+ *                       softmax per proxy row, reduced column-wise;
+ *   3. protected set    Pi = [0,n_sink) U [L-n_recent,L);
+ *   4. Proxy-Tokens Eviction: T = the (budget_proxy - |Pi|) positions outside Pi with the
+ *                       largest imp, ties to the lower index;
+ *   5. Random Eviction: U = budget_random positions drawn without replacement from the
+ *                       rest with probability proportional to imp, as
+ *                       Gumbel-top-k: key_j = fl32(ln imp_j - ln(-ln u_j)), u_j from
+ *                       Philox4x32-10(counter=(j,hk,b,layer), key=seed), largest keys win,
+ *                       ties to the lower index;
+ *   6. out_idx[b,hk,:] = sorted(Pi U T U U), C = budget_proxy + budget_random entries
+ *                       (PAPER.md:163, 183);
+ *   7. out_K[b,hk,c,:] = K[b,hk,out_idx[c],:], out_V likewise.
+ *
+ * Layouts (contiguous, row-major):
+ *   K, V        [batch, Hkv, L, d]     Qproxy  [batch, Hq, P, d]  (queries of the last P
+ *               prompt positions, in order)
+ *   out_K/out_V [batch, Hkv, C, d]     out_idx [batch, Hkv, C] int32, strictly ascending
+ *   out_importance (optional) [batch, Hkv, L] fp32;  out_lse (optional) [batch, Hq, P] fp32
+ * Element type: bfloat16 (nacl_evict) or IEEE fp32 (nacl_evict_f32); nacl_evict_ex takes a tag.
+ * budget_* / n_* are token counts; budget_proxy INCLUDES the n_sink + n_recent protected
+ * tokens (R7).
+ *
+ * Ownership / behaviour: every pointer of nacl_evict, nacl_evict_f32 and nacl_evict_ex is a
+ * DEVICE pointer owned by the caller; inputs are read-only; outputs must not alias inputs;
+ * pointers must be 16-byte aligned and d*sizeof(element) a multiple of 16.  Work is enqueued
+ * on `stream` (a cudaStream_t passed as void*); the call never synchronises the host and
+ * results are valid once the stream reaches that point.  With a caller-supplied workspace
+ * (nacl_evict_ex) the call allocates nothing and is CUDA-graph capturable; without one a
+ * grow-only per-device workspace is created on first use (cudaMalloc: not capturable).
+ * Same inputs and seed give bit-identical outputs run to run (no floating-point atomics).
+ * nacl_evict_host is the same operation on HOST buffers (copies inside; synchronous).
+ *
+ * Errors: 0 = OK; negative = error; nothing is thrown and no output is written on a
+ * validation error.  Validation is host-side and never reads device memory.
+ *
+ * Supported: 1 <= P <= L <= 2^24; Hq % Hkv == 0; d a multiple of 16, d <= 256; any L (ragged
+ * last tile is masked).  The tensor-core path (tcgen05 + TMA) serves bf16, d == 128,
+ * G*P <= 256; every other shape runs the generic CUDA-core kernels of the same library.
+ */
+#ifndef NACL_EVICT_H
+#define NACL_EVICT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NACL_VERSION 100 /* major*10000 + minor*100 + patch */
+
+#define NACL_DTYPE_F32 0
+#define NACL_DTYPE_BF16 1
+
+#define NACL_OK 0
+#define NACL_ERR_NULL (-1)        /* a required pointer is NULL */
+#define NACL_ERR_SHAPE (-2)       /* sizes <= 0, Hq % Hkv != 0, P > L, unsupported d, L > 2^24 */
+#define NACL_ERR_BUDGET (-3)      /* negative counts, n_sink+n_recent > L, budget_proxy < protected, total > L */
+#define NACL_ERR_ALIGN (-4)       /* pointer not 16-byte aligned or d*elem not a multiple of 16 */
+#define NACL_ERR_WORKSPACE (-5)   /* supplied workspace too small or misaligned */
+#define NACL_ERR_CUDA (-6)        /* a CUDA runtime/driver call failed; see nacl_last_cuda_error() */
+#define NACL_ERR_UNSUPPORTED (-7) /* a flag or dtype this build does not implement */
+
+/* nacl_evict_ex flags */
+#define NACL_FLAG_CAUSAL 1u                  /* DESIGN.md R1; not implemented on the GPU yet -> NACL_ERR_UNSUPPORTED */
+#define NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE 2u /* sampling weight exp(imp_j) (R4) */
+#define NACL_FLAG_SAMPLE_UNIFORM 4u          /* uniform sampling weights (paper's ablation) */
+#define NACL_FLAG_SCORE_CUDA_CORES 0x100u    /* debugging: run the generic CUDA-core scoring kernels even where
+                                                the tensor-core path applies */
+
+typedef struct nacl_params {
+  uint32_t struct_size;            /* = sizeof(nacl_params_t) */
+  int32_t dtype;                   /* NACL_DTYPE_* of K, V, Qproxy, out_K, out_V */
+  const void* K;                   /* [batch,Hkv,L,d] */
+  const void* V;                   /* [batch,Hkv,L,d] */
+  const void* Qproxy;              /* [batch,Hq,P,d] */
+  int32_t batch, L, Hq, Hkv, d, P;
+  int32_t budget_proxy, budget_random, n_sink, n_recent;
+  uint64_t seed;
+  int32_t layer;
+  uint32_t flags;
+  void* out_K;                     /* [batch,Hkv,C,d] */
+  void* out_V;                     /* [batch,Hkv,C,d] */
+  int32_t* out_idx;                /* [batch,Hkv,C] */
+  float* out_importance;           /* optional [batch,Hkv,L] */
+  float* out_lse;                  /* optional [batch,Hq,P]: ln sum_j exp(s[i,j]) */
+  void* workspace;                 /* optional; >= nacl_workspace_bytes(...) bytes, 256-byte aligned */
+  size_t workspace_bytes;
+  void* stream;                    /* cudaStream_t */
+} nacl_params_t;
+
+/* bf16 K/V/Q.  Steps 1-7 above on `stream`. */
+int nacl_evict(const void* K, const void* V, const void* Qproxy,
+               int batch, int L, int Hq, int Hkv, int d, int P,
+               int budget_proxy, int budget_random, int n_sink, int n_recent,
+               uint64_t seed, int layer,
+               void* out_K, void* out_V, int32_t* out_idx, void* stream);
+
+/* fp32 K/V/Q, otherwise identical. */
+int nacl_evict_f32(const void* K, const void* V, const void* Qproxy,
+                   int batch, int L, int Hq, int Hkv, int d, int P,
+                   int budget_proxy, int budget_random, int n_sink, int n_recent,
+                   uint64_t seed, int layer,
+                   void* out_K, void* out_V, int32_t* out_idx, void* stream);
+
+/* Superset entry point: dtype tag, flags, optional importance / lse outputs, explicit workspace. */
+int nacl_evict_ex(const nacl_params_t* p);
+
+/* Same operation with every tensor in HOST memory (pinned memory makes the copies
+ * asynchronous).  Copies K, V, Qproxy to grow-only device staging buffers, runs steps 1-7
+ * and copies out_K, out_V, out_idx back; returns after the results are in host memory.
+ * device < 0 uses the current device. */
+int nacl_evict_host(const void* K, const void* V, const void* Qproxy, int dtype,
+                    int batch, int L, int Hq, int Hkv, int d, int P,
+                    int budget_proxy, int budget_random, int n_sink, int n_recent,
+                    uint64_t seed, int layer,
+                    void* out_K, void* out_V, int32_t* out_idx, int device);
+
+/* Bytes of scratch one call needs (a pure function of the shape; 0 on invalid shapes). */
+size_t nacl_workspace_bytes(int batch, int L, int Hq, int Hkv, int d, int P);
+
+/* Number of kernels one call with these arguments launches (for launch accounting). */
+int nacl_launch_count(int dtype, int batch, int L, int Hq, int Hkv, int d, int P, uint32_t flags);
+
+/* Frees the per-device internal workspaces / staging buffers (optional, e.g. before exit). */
+void nacl_release(void);
+
+const char* nacl_strerror(int code);
+/* cudaError_t of the most recent NACL_ERR_CUDA on this thread, as an int. */
+int nacl_last_cuda_error(void);
+int nacl_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

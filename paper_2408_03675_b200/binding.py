@@ -1,0 +1,205 @@
+"""ctypes binding of libnacl_evict.so -- argument marshalling only.
+
+Every step of the path (scoring, softmax statistics, column sum, selects, sampling keys,
+compaction, gather) runs in the library's CUDA kernels; PyTorch supplies device memory and the
+stream.  Function names mirror include/nacl_evict.h.  There is no CPU fallback: if the library is
+missing or cannot be loaded, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+NACL_DTYPE_F32, NACL_DTYPE_BF16 = 0, 1
+FLAG_CAUSAL, FLAG_SAMPLE_SOFTMAX_OF_SCORE, FLAG_SAMPLE_UNIFORM, FLAG_SCORE_CUDA_CORES = 1, 2, 4, 0x100
+
+EXPORTS = ("nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes",
+           "nacl_launch_count", "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version")
+
+
+class NaclParams(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("dtype", C.c_int32),
+        ("K", C.c_void_p), ("V", C.c_void_p), ("Qproxy", C.c_void_p),
+        ("batch", C.c_int32), ("L", C.c_int32), ("Hq", C.c_int32), ("Hkv", C.c_int32), ("d", C.c_int32), ("P", C.c_int32),
+        ("budget_proxy", C.c_int32), ("budget_random", C.c_int32), ("n_sink", C.c_int32), ("n_recent", C.c_int32),
+        ("seed", C.c_uint64), ("layer", C.c_int32), ("flags", C.c_uint32),
+        ("out_K", C.c_void_p), ("out_V", C.c_void_p), ("out_idx", C.c_void_p),
+        ("out_importance", C.c_void_p), ("out_lse", C.c_void_p),
+        ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("stream", C.c_void_p),
+    ]
+
+
+class NaclError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        msg = _lib.nacl_strerror(code).decode()
+        extra = f" (cudaError {_lib.nacl_last_cuda_error()})" if code == -6 else ""
+        super().__init__(f"{where}: {msg}{extra} [code {code}]")
+        self.code = code
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def _load() -> C.CDLL:
+    path = _build.LIB
+    if not os.path.exists(path) or _build.needs_build():
+        path = _build.build()  # raises if nvcc is missing or the build fails: no fallback
+    lib = C.CDLL(path)
+    vp, i32, u64, u32 = C.c_void_p, C.c_int, C.c_uint64, C.c_uint32
+    sig = [vp, vp, vp] + [i32] * 10 + [u64, i32, vp, vp, vp, vp]
+    lib.nacl_evict.argtypes = sig
+    lib.nacl_evict.restype = i32
+    lib.nacl_evict_f32.argtypes = sig
+    lib.nacl_evict_f32.restype = i32
+    lib.nacl_evict_ex.argtypes = [C.POINTER(NaclParams)]
+    lib.nacl_evict_ex.restype = i32
+    lib.nacl_evict_host.argtypes = [vp, vp, vp, i32] + [i32] * 10 + [u64, i32, vp, vp, vp, i32]
+    lib.nacl_evict_host.restype = i32
+    lib.nacl_workspace_bytes.argtypes = [i32] * 6
+    lib.nacl_workspace_bytes.restype = C.c_size_t
+    lib.nacl_launch_count.argtypes = [i32] * 7 + [u32]
+    lib.nacl_launch_count.restype = i32
+    lib.nacl_release.argtypes = []
+    lib.nacl_release.restype = None
+    lib.nacl_strerror.argtypes = [i32]
+    lib.nacl_strerror.restype = C.c_char_p
+    lib.nacl_last_cuda_error.argtypes = []
+    lib.nacl_last_cuda_error.restype = i32
+    lib.nacl_version.argtypes = []
+    lib.nacl_version.restype = i32
+    return lib
+
+
+_lib = _load()
+
+
+def _dtype_tag(t: torch.Tensor) -> int:
+    if t.dtype == torch.bfloat16:
+        return NACL_DTYPE_BF16
+    if t.dtype == torch.float32:
+        return NACL_DTYPE_F32
+    raise TypeError(f"nacl_evict takes bfloat16 or float32 tensors, got {t.dtype}")
+
+
+def _shapes(K, V, Q):
+    if K.dim() != 4 or Q.dim() != 4 or V.shape != K.shape:
+        raise ValueError("expected K,V [batch,Hkv,L,d] and Qproxy [batch,Hq,P,d]")
+    B, Hkv, L, d = K.shape
+    B2, Hq, P, d2 = Q.shape
+    if B2 != B or d2 != d or K.dtype != V.dtype or K.dtype != Q.dtype:
+        raise ValueError("K/V/Qproxy batch, head_dim or dtype mismatch")
+    for t in (K, V, Q):
+        if not t.is_contiguous():
+            raise ValueError("tensors must be contiguous")
+    return B, Hkv, L, d, Hq, P
+
+
+def nacl_version() -> int:
+    return int(_lib.nacl_version())
+
+
+def nacl_workspace_bytes(batch, L, Hq, Hkv, d, P) -> int:
+    return int(_lib.nacl_workspace_bytes(batch, L, Hq, Hkv, d, P))
+
+
+def nacl_launch_count(dtype, batch, L, Hq, Hkv, d, P, flags=0) -> int:
+    return int(_lib.nacl_launch_count(dtype, batch, L, Hq, Hkv, d, P, flags))
+
+
+def nacl_release() -> None:
+    _lib.nacl_release()
+
+
+def nacl_evict(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer,
+               out_K=None, out_V=None, out_idx=None, stream=None):
+    """include/nacl_evict.h `nacl_evict` / `nacl_evict_f32` on CUDA tensors.  Returns (out_K, out_V, out_idx)."""
+    B, Hkv, L, d, Hq, P = _shapes(K, V, Qproxy)
+    if not K.is_cuda:
+        raise ValueError("nacl_evict takes CUDA tensors (use nacl_evict_host for host buffers)")
+    Cn = budget_proxy + budget_random
+    if out_K is None:
+        out_K = torch.empty((B, Hkv, max(Cn, 0), d), dtype=K.dtype, device=K.device)
+    if out_V is None:
+        out_V = torch.empty_like(out_K)
+    if out_idx is None:
+        out_idx = torch.empty((B, Hkv, max(Cn, 0)), dtype=torch.int32, device=K.device)
+    st = (stream or torch.cuda.current_stream(K.device)).cuda_stream
+    fn = _lib.nacl_evict if K.dtype == torch.bfloat16 else _lib.nacl_evict_f32
+    _dtype_tag(K)
+    with torch.cuda.device(K.device):
+        rc = fn(K.data_ptr(), V.data_ptr(), Qproxy.data_ptr(), B, L, Hq, Hkv, d, P, budget_proxy, budget_random,
+                n_sink, n_recent, seed, layer, out_K.data_ptr(), out_V.data_ptr(), out_idx.data_ptr(), st)
+    if rc != 0:
+        raise NaclError(rc, "nacl_evict")
+    return out_K, out_V, out_idx
+
+
+def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer, flags=0,
+                  out_K=None, out_V=None, out_idx=None, want_importance=False, want_lse=False,
+                  workspace=None, stream=None):
+    """include/nacl_evict.h `nacl_evict_ex`.  Returns a dict with out_K, out_V, out_idx and, if asked,
+    importance [B,Hkv,L] fp32 and lse [B,Hq,P] fp32."""
+    B, Hkv, L, d, Hq, P = _shapes(K, V, Qproxy)
+    if not K.is_cuda:
+        raise ValueError("nacl_evict_ex takes CUDA tensors")
+    dev = K.device
+    Cn = budget_proxy + budget_random
+    if out_K is None:
+        out_K = torch.empty((B, Hkv, max(Cn, 0), d), dtype=K.dtype, device=dev)
+    if out_V is None:
+        out_V = torch.empty_like(out_K)
+    if out_idx is None:
+        out_idx = torch.empty((B, Hkv, max(Cn, 0)), dtype=torch.int32, device=dev)
+    imp = torch.empty((B, Hkv, L), dtype=torch.float32, device=dev) if want_importance else None
+    lse = torch.empty((B, Hq, P), dtype=torch.float32, device=dev) if want_lse else None
+    p = NaclParams()
+    p.struct_size = C.sizeof(NaclParams)
+    p.dtype = _dtype_tag(K)
+    p.K, p.V, p.Qproxy = K.data_ptr(), V.data_ptr(), Qproxy.data_ptr()
+    p.batch, p.L, p.Hq, p.Hkv, p.d, p.P = B, L, Hq, Hkv, d, P
+    p.budget_proxy, p.budget_random, p.n_sink, p.n_recent = budget_proxy, budget_random, n_sink, n_recent
+    p.seed, p.layer, p.flags = seed, layer, flags
+    p.out_K, p.out_V, p.out_idx = out_K.data_ptr(), out_V.data_ptr(), out_idx.data_ptr()
+    p.out_importance = imp.data_ptr() if imp is not None else None
+    p.out_lse = lse.data_ptr() if lse is not None else None
+    if workspace is not None:
+        p.workspace, p.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
+    p.stream = (stream or torch.cuda.current_stream(dev)).cuda_stream
+    with torch.cuda.device(dev):
+        rc = _lib.nacl_evict_ex(C.byref(p))
+    if rc != 0:
+        raise NaclError(rc, "nacl_evict_ex")
+    out = {"out_K": out_K, "out_V": out_V, "out_idx": out_idx}
+    if imp is not None:
+        out["importance"] = imp
+    if lse is not None:
+        out["lse"] = lse
+    return out
+
+
+def nacl_evict_host(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer,
+                    out_K=None, out_V=None, out_idx=None, device=-1):
+    """include/nacl_evict.h `nacl_evict_host`: HOST tensors in, HOST tensors out (copies inside, synchronous)."""
+    B, Hkv, L, d, Hq, P = _shapes(K, V, Qproxy)
+    if K.is_cuda:
+        raise ValueError("nacl_evict_host takes host tensors")
+    Cn = budget_proxy + budget_random
+    pin = K.is_pinned()
+    if out_K is None:
+        out_K = torch.empty((B, Hkv, max(Cn, 0), d), dtype=K.dtype, pin_memory=pin)
+    if out_V is None:
+        out_V = torch.empty_like(out_K, pin_memory=pin)
+    if out_idx is None:
+        out_idx = torch.empty((B, Hkv, max(Cn, 0)), dtype=torch.int32, pin_memory=pin)
+    rc = _lib.nacl_evict_host(K.data_ptr(), V.data_ptr(), Qproxy.data_ptr(), _dtype_tag(K), B, L, Hq, Hkv, d, P,
+                              budget_proxy, budget_random, n_sink, n_recent, seed, layer,
+                              out_K.data_ptr(), out_V.data_ptr(), out_idx.data_ptr(), device)
+    if rc != 0:
+        raise NaclError(rc, "nacl_evict_host")
+    return out_K, out_V, out_idx

@@ -1,0 +1,313 @@
+// api.cu -- the C ABI of libnacl_evict.so (include/nacl_evict.h): argument validation, workspace
+// carve-up and the launch sequence of one eviction call.
+// Host code only enqueues; it never reads device memory and never synchronises (except
+// nacl_evict_host, which is documented as synchronous).
+#include <mutex>
+#include <new>
+
+#include "nacl_internal.cuh"
+
+namespace nacl {
+
+static thread_local int g_last_cuda_error = 0;
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+SplitPlan make_split_plan(int batch, int L, int Hkv) {
+  // about 8 work items per SM so that a dynamically scheduled grid ends with a short tail
+  const long heads = (long)batch * Hkv;
+  const long items_target = 8L * kNumSMs;
+  long per_head = (items_target + heads - 1) / heads;
+  if (per_head < 1) per_head = 1;
+  long chunk = ((long)L + per_head - 1) / per_head;
+  chunk = (chunk + 127) / 128 * 128;
+  if (chunk < 512) chunk = 512;
+  SplitPlan sp;
+  sp.chunk = (int)chunk;
+  sp.n_chunks = (int)(((long)L + chunk - 1) / chunk);
+  return sp;
+}
+
+Workspace carve_workspace(void* base, int batch, int L, int Hq, int Hkv, int P) {
+  const SplitPlan sp = make_split_plan(batch, L, Hkv);
+  const size_t n_rows = (size_t)batch * Hq * P;
+  const size_t n_imp = (size_t)batch * Hkv * L;
+  size_t off = 0;
+  char* b = static_cast<char*>(base);
+  Workspace ws;
+  ws.part = reinterpret_cast<float2*>(b + off); off = align_up(off + n_rows * sp.n_chunks * sizeof(float2), 256);
+  ws.lse = reinterpret_cast<float*>(b + off);   off = align_up(off + n_rows * sizeof(float), 256);
+  ws.imp = reinterpret_cast<float*>(b + off);   off = align_up(off + n_imp * sizeof(float), 256);
+  ws.key = reinterpret_cast<uint32_t*>(b + off); off = align_up(off + n_imp * sizeof(uint32_t), 256);
+  ws.sync = reinterpret_cast<int*>(b + off);    off = align_up(off + kSyncInts * sizeof(int), 256);
+  ws.bytes = off;
+  return ws;
+}
+
+// ------------------------------------------------------------------ validation
+static int validate_shape(int dtype, int batch, int L, int Hq, int Hkv, int d, int P) {
+  if (dtype != NACL_DTYPE_F32 && dtype != NACL_DTYPE_BF16) return NACL_ERR_UNSUPPORTED;
+  if (batch < 1 || L < 1 || Hq < 1 || Hkv < 1 || d < 1 || P < 1) return NACL_ERR_SHAPE;
+  if (Hq % Hkv != 0 || P > L || L > (1 << 24)) return NACL_ERR_SHAPE;
+  if (d % 16 != 0 || d > 256) return NACL_ERR_SHAPE;
+  if ((long)batch * Hkv > 65535 || batch > 65535) return NACL_ERR_SHAPE;
+  if ((long)batch * Hq * P > (1L << 30)) return NACL_ERR_SHAPE;
+  return NACL_OK;
+}
+
+static int validate_budget(int L, int budget_proxy, int budget_random, int n_sink, int n_recent) {
+  if (budget_proxy < 0 || budget_random < 0 || n_sink < 0 || n_recent < 0) return NACL_ERR_BUDGET;
+  const long n_prot = (long)n_sink + n_recent;
+  if (n_prot > L) return NACL_ERR_BUDGET;
+  if (budget_proxy < n_prot) return NACL_ERR_BUDGET;  // protected tokens count inside budget_proxy (R7)
+  if ((long)budget_proxy + budget_random > L) return NACL_ERR_BUDGET;
+  return NACL_OK;
+}
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// ------------------------------------------------------------------ internal grow-only buffers
+struct DeviceCache {
+  void* ws = nullptr;
+  size_t ws_bytes = 0;
+  void* stage[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // K V Q oK oV idx
+  size_t stage_bytes[6] = {0, 0, 0, 0, 0, 0};
+  cudaStream_t stream = nullptr;
+};
+static std::mutex g_mu;       // guards g_cache
+static std::mutex g_host_mu;  // serialises nacl_evict_host (its staging buffers are shared per device)
+static DeviceCache g_cache[64];
+
+static cudaError_t grow(void** p, size_t* have, size_t want) {
+  if (*have >= want && *p) return cudaSuccess;
+  if (*p) {
+    cudaError_t e = cudaFree(*p);
+    *p = nullptr;
+    *have = 0;
+    if (e != cudaSuccess) return e;
+  }
+  size_t cap = want + want / 8 + 256;
+  cudaError_t e = cudaMalloc(p, cap);
+  if (e != cudaSuccess) { *p = nullptr; return e; }
+  *have = cap;
+  return cudaSuccess;
+}
+
+static int fail_cuda(cudaError_t e) {
+  g_last_cuda_error = (int)e;
+  cudaGetLastError();  // clear the sticky-free error state
+  return NACL_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------ the call
+static int evict_impl(const nacl_params_t& p) {
+  if (!p.K || !p.V || !p.Qproxy || !p.out_K || !p.out_V || !p.out_idx) return NACL_ERR_NULL;
+  int rc = validate_shape(p.dtype, p.batch, p.L, p.Hq, p.Hkv, p.d, p.P);
+  if (rc) return rc;
+  rc = validate_budget(p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent);
+  if (rc) return rc;
+  const uint32_t known = NACL_FLAG_CAUSAL | NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE | NACL_FLAG_SAMPLE_UNIFORM | NACL_FLAG_SCORE_CUDA_CORES;
+  if (p.flags & ~known) return NACL_ERR_UNSUPPORTED;
+  if (p.flags & NACL_FLAG_CAUSAL) return NACL_ERR_UNSUPPORTED;
+  if ((p.flags & NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE) && (p.flags & NACL_FLAG_SAMPLE_UNIFORM)) return NACL_ERR_UNSUPPORTED;
+
+  Shape s;
+  s.batch = p.batch; s.L = p.L; s.Hq = p.Hq; s.Hkv = p.Hkv; s.d = p.d; s.P = p.P;
+  s.G = p.Hq / p.Hkv; s.rows = s.G * p.P; s.dtype = p.dtype; s.esize = p.dtype == NACL_DTYPE_F32 ? 4 : 2;
+  const int row_bytes = s.d * s.esize;
+  if (row_bytes % 16 != 0) return NACL_ERR_ALIGN;
+  if (!aligned16(p.K) || !aligned16(p.V) || !aligned16(p.Qproxy) || !aligned16(p.out_K) || !aligned16(p.out_V) ||
+      (reinterpret_cast<uintptr_t>(p.out_idx) & 3u))
+    return NACL_ERR_ALIGN;
+
+  const size_t need = nacl_workspace_bytes(p.batch, p.L, p.Hq, p.Hkv, p.d, p.P);
+  void* wsp = p.workspace;
+  if (wsp) {
+    if (p.workspace_bytes < need || (reinterpret_cast<uintptr_t>(wsp) & 255u)) return NACL_ERR_WORKSPACE;
+  } else {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(e);
+    if (dev < 0 || dev >= 64) return NACL_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lk(g_mu);
+    e = grow(&g_cache[dev].ws, &g_cache[dev].ws_bytes, need);
+    if (e != cudaSuccess) return fail_cuda(e);
+    wsp = g_cache[dev].ws;
+  }
+  const Workspace ws = carve_workspace(wsp, p.batch, p.L, p.Hq, p.Hkv, p.P);
+  const SplitPlan sp = make_split_plan(p.batch, p.L, p.Hkv);
+  cudaStream_t st = static_cast<cudaStream_t>(p.stream);
+
+  cudaError_t e;
+  const bool tc = !(p.flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
+  if (tc) e = launch_score_tc(s, p.K, p.Qproxy, sp, ws, p.out_importance, p.out_lse, st);
+  else e = launch_score_generic(s, p.K, p.Qproxy, sp, ws, p.out_importance, p.out_lse, st);
+  if (e != cudaSuccess) return fail_cuda(e);
+
+  const int C = p.budget_proxy + p.budget_random;
+  if (p.budget_random > 0) {
+    e = launch_keys(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.seed, p.layer, p.flags, st);
+    if (e != cudaSuccess) return fail_cuda(e);
+  }
+  e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent,
+                    p.out_idx, st);
+  if (e != cudaSuccess) return fail_cuda(e);
+  e = launch_gather(p.K, p.V, p.out_idx, p.batch * p.Hkv, p.L, C, row_bytes, p.out_K, p.out_V, st);
+  if (e != cudaSuccess) return fail_cuda(e);
+  return NACL_OK;
+}
+
+static nacl_params_t make_params(int dtype, const void* K, const void* V, const void* Q, int batch, int L, int Hq, int Hkv,
+                                 int d, int P, int bp, int br, int n_sink, int n_recent, uint64_t seed, int layer,
+                                 void* oK, void* oV, int32_t* oidx, void* stream) {
+  nacl_params_t p{};
+  p.struct_size = sizeof(nacl_params_t);
+  p.dtype = dtype;
+  p.K = K; p.V = V; p.Qproxy = Q;
+  p.batch = batch; p.L = L; p.Hq = Hq; p.Hkv = Hkv; p.d = d; p.P = P;
+  p.budget_proxy = bp; p.budget_random = br; p.n_sink = n_sink; p.n_recent = n_recent;
+  p.seed = seed; p.layer = layer; p.flags = 0;
+  p.out_K = oK; p.out_V = oV; p.out_idx = oidx;
+  p.stream = stream;
+  return p;
+}
+
+}  // namespace nacl
+
+using namespace nacl;
+
+#pragma GCC visibility push(default)
+extern "C" {
+
+int nacl_evict(const void* K, const void* V, const void* Qproxy, int batch, int L, int Hq, int Hkv, int d, int P,
+               int budget_proxy, int budget_random, int n_sink, int n_recent, uint64_t seed, int layer, void* out_K,
+               void* out_V, int32_t* out_idx, void* stream) {
+  return evict_impl(make_params(NACL_DTYPE_BF16, K, V, Qproxy, batch, L, Hq, Hkv, d, P, budget_proxy, budget_random, n_sink,
+                                n_recent, seed, layer, out_K, out_V, out_idx, stream));
+}
+
+int nacl_evict_f32(const void* K, const void* V, const void* Qproxy, int batch, int L, int Hq, int Hkv, int d, int P,
+                   int budget_proxy, int budget_random, int n_sink, int n_recent, uint64_t seed, int layer, void* out_K,
+                   void* out_V, int32_t* out_idx, void* stream) {
+  return evict_impl(make_params(NACL_DTYPE_F32, K, V, Qproxy, batch, L, Hq, Hkv, d, P, budget_proxy, budget_random, n_sink,
+                                n_recent, seed, layer, out_K, out_V, out_idx, stream));
+}
+
+int nacl_evict_ex(const nacl_params_t* p) {
+  if (!p) return NACL_ERR_NULL;
+  if (p->struct_size != sizeof(nacl_params_t)) return NACL_ERR_UNSUPPORTED;
+  return evict_impl(*p);
+}
+
+int nacl_evict_host(const void* K, const void* V, const void* Qproxy, int dtype, int batch, int L, int Hq, int Hkv, int d,
+                    int P, int budget_proxy, int budget_random, int n_sink, int n_recent, uint64_t seed, int layer,
+                    void* out_K, void* out_V, int32_t* out_idx, int device) {
+  if (!K || !V || !Qproxy || !out_K || !out_V || !out_idx) return NACL_ERR_NULL;
+  int rc = validate_shape(dtype, batch, L, Hq, Hkv, d, P);
+  if (rc) return rc;
+  rc = validate_budget(L, budget_proxy, budget_random, n_sink, n_recent);
+  if (rc) return rc;
+  std::lock_guard<std::mutex> host_lk(g_host_mu);
+  cudaError_t e;
+  int prev = -1;
+  if ((e = cudaGetDevice(&prev)) != cudaSuccess) return fail_cuda(e);
+  if (device < 0) device = prev;
+  if (device >= 64) return NACL_ERR_UNSUPPORTED;
+  if (device != prev && (e = cudaSetDevice(device)) != cudaSuccess) return fail_cuda(e);
+
+  const size_t esz = dtype == NACL_DTYPE_F32 ? 4 : 2;
+  const int C = budget_proxy + budget_random;
+  const size_t kv_bytes = (size_t)batch * Hkv * L * d * esz;
+  const size_t q_bytes = (size_t)batch * Hq * P * d * esz;
+  const size_t okv_bytes = (size_t)batch * Hkv * C * d * esz;
+  const size_t idx_bytes = (size_t)batch * Hkv * C * sizeof(int32_t);
+  const size_t want[6] = {kv_bytes, kv_bytes, q_bytes, okv_bytes, okv_bytes, idx_bytes};
+
+  std::unique_lock<std::mutex> lk(g_mu);
+  DeviceCache& dc = g_cache[device];
+  rc = NACL_OK;
+  for (int i = 0; i < 6 && rc == NACL_OK; ++i)
+    if ((e = grow(&dc.stage[i], &dc.stage_bytes[i], want[i] ? want[i] : 16)) != cudaSuccess) rc = fail_cuda(e);
+  if (rc == NACL_OK && !dc.stream && (e = cudaStreamCreateWithFlags(&dc.stream, cudaStreamNonBlocking)) != cudaSuccess)
+    rc = fail_cuda(e);
+  void* sK = dc.stage[0]; void* sV = dc.stage[1]; void* sQ = dc.stage[2];
+  void* soK = dc.stage[3]; void* soV = dc.stage[4]; void* sidx = dc.stage[5];
+  cudaStream_t st = dc.stream;
+  lk.unlock();
+
+  if (rc == NACL_OK) {
+    // one cudaMemcpyAsync per tensor; pinned host memory makes them truly asynchronous
+    if ((e = cudaMemcpyAsync(sQ, Qproxy, q_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(sK, K, kv_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(sV, V, kv_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+      rc = fail_cuda(e);
+  }
+  if (rc == NACL_OK) {
+    nacl_params_t p = make_params(dtype, sK, sV, sQ, batch, L, Hq, Hkv, d, P, budget_proxy, budget_random, n_sink, n_recent,
+                                  seed, layer, soK, soV, static_cast<int32_t*>(sidx), st);
+    rc = evict_impl(p);
+  }
+  if (rc == NACL_OK && C > 0) {
+    if ((e = cudaMemcpyAsync(out_idx, sidx, idx_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(out_K, soK, okv_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(out_V, soV, okv_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+      rc = fail_cuda(e);
+  }
+  if (rc == NACL_OK && (e = cudaStreamSynchronize(st)) != cudaSuccess) rc = fail_cuda(e);
+  if (device != prev) cudaSetDevice(prev);
+  return rc;
+}
+
+size_t nacl_workspace_bytes(int batch, int L, int Hq, int Hkv, int d, int P) {
+  if (validate_shape(NACL_DTYPE_BF16, batch, L, Hq, Hkv, d, P) != NACL_OK) return 0;
+  return carve_workspace(nullptr, batch, L, Hq, Hkv, P).bytes;
+}
+
+int nacl_launch_count(int dtype, int batch, int L, int Hq, int Hkv, int d, int P, uint32_t flags) {
+  if (validate_shape(dtype, batch, L, Hq, Hkv, d, P) != NACL_OK) return 0;
+  Shape s;
+  s.batch = batch; s.L = L; s.Hq = Hq; s.Hkv = Hkv; s.d = d; s.P = P;
+  s.G = Hq / Hkv; s.rows = s.G * P; s.dtype = dtype; s.esize = dtype == NACL_DTYPE_F32 ? 4 : 2;
+  const bool tc = !(flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
+  // scoring + keys + select + gather (budget_random > 0 and C > 0 assumed)
+  return (tc ? score_tc_launch_count(s) : 3) + 3;
+}
+
+void nacl_release(void) {
+  std::lock_guard<std::mutex> lk(g_mu);
+  int prev = -1;
+  if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return; }
+  for (int dev = 0; dev < 64; ++dev) {
+    DeviceCache& dc = g_cache[dev];
+    bool any = dc.ws || dc.stream;
+    for (int i = 0; i < 6; ++i) any = any || dc.stage[i];
+    if (!any) continue;
+    if (cudaSetDevice(dev) != cudaSuccess) { cudaGetLastError(); continue; }
+    if (dc.ws) cudaFree(dc.ws);
+    for (int i = 0; i < 6; ++i) if (dc.stage[i]) cudaFree(dc.stage[i]);
+    if (dc.stream) cudaStreamDestroy(dc.stream);
+    dc = DeviceCache();
+  }
+  cudaSetDevice(prev);
+  cudaGetLastError();
+}
+
+const char* nacl_strerror(int code) {
+  switch (code) {
+    case NACL_OK: return "ok";
+    case NACL_ERR_NULL: return "a required pointer is NULL";
+    case NACL_ERR_SHAPE: return "unsupported shape (sizes, Hq % Hkv, P > L, d, L > 2^24)";
+    case NACL_ERR_BUDGET: return "budget error (negative count, protected > L, budget_proxy < protected, total > L)";
+    case NACL_ERR_ALIGN: return "pointer not 16-byte aligned or row size not a multiple of 16 bytes";
+    case NACL_ERR_WORKSPACE: return "workspace too small or not 256-byte aligned";
+    case NACL_ERR_CUDA: return "a CUDA call failed (see nacl_last_cuda_error)";
+    case NACL_ERR_UNSUPPORTED: return "flag, dtype or struct version not supported by this build";
+    default: return "unknown error code";
+  }
+}
+
+int nacl_last_cuda_error(void) { return g_last_cuda_error; }
+int nacl_version(void) { return NACL_VERSION; }
+
+}  // extern "C"
+#pragma GCC visibility pop

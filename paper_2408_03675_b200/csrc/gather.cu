@@ -1,0 +1,71 @@
+// gather.cu -- step a7 of SURVEY.md section 8: cache compaction K,V <- K_S,V_S.
+// Pure data movement, bit-exact rows.  Every thread moves 16-byte vectors (LDG.128 / STG.128):
+// consecutive threads take consecutive vectors of the OUTPUT, so writes are fully coalesced and
+// reads are whole contiguous rows (row_bytes >= 128 B in every supported shape) at ascending
+// addresses.  Inputs are streamed past L1 (read once); outputs are streaming stores.
+#include "nacl_internal.cuh"
+
+namespace nacl {
+namespace {
+
+__device__ __forceinline__ int4 ld_stream(const int4* p) {
+  int4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_stream(int4* p, const int4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.s32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+constexpr int GT = 256;  // threads per block
+constexpr int GU = 4;    // vectors of K and of V in flight per thread
+
+// vpr = 16-byte vectors per row; n_vec = n_prob * C * vpr output vectors per tensor
+__global__ void __launch_bounds__(GT) gather_kernel(const int4* __restrict__ K, const int4* __restrict__ V,
+                                                     const int32_t* __restrict__ idx, int L, int C, int vpr,
+                                                     size_t n_vec, int4* __restrict__ oK, int4* __restrict__ oV) {
+  const size_t stride = (size_t)gridDim.x * GT;
+  for (size_t v0 = (size_t)blockIdx.x * GT + threadIdx.x; v0 < n_vec; v0 += stride * GU) {
+    size_t src[GU];
+    bool ok[GU];
+#pragma unroll
+    for (int u = 0; u < GU; ++u) {
+      const size_t v = v0 + (size_t)u * stride;
+      ok[u] = v < n_vec;
+      if (ok[u]) {
+        const size_t row = v / (size_t)vpr;          // p * C + c
+        const int off = (int)(v - row * (size_t)vpr);
+        const size_t p = row / (size_t)C;
+        const int j = idx[row];
+        src[u] = (p * (size_t)L + (size_t)j) * (size_t)vpr + off;
+      }
+    }
+    int4 a[GU], b[GU];
+#pragma unroll
+    for (int u = 0; u < GU; ++u)
+      if (ok[u]) { a[u] = ld_stream(K + src[u]); b[u] = ld_stream(V + src[u]); }
+#pragma unroll
+    for (int u = 0; u < GU; ++u)
+      if (ok[u]) {
+        const size_t v = v0 + (size_t)u * stride;
+        st_stream(oK + v, a[u]);
+        st_stream(oV + v, b[u]);
+      }
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_gather(const void* K, const void* V, const int32_t* idx, int n_prob, int L, int C, int row_bytes,
+                          void* out_K, void* out_V, cudaStream_t st) {
+  const int vpr = row_bytes / 16;
+  const size_t n_vec = (size_t)n_prob * C * vpr;
+  if (n_vec == 0) return cudaSuccess;
+  size_t want = (n_vec + (size_t)GT * GU - 1) / ((size_t)GT * GU);
+  const size_t cap = (size_t)kNumSMs * 8 * 4;  // a few waves of 8 resident CTAs per SM
+  int blocks = (int)(want < cap ? want : cap);
+  gather_kernel<<<blocks, GT, 0, st>>>((const int4*)K, (const int4*)V, idx, L, C, vpr, n_vec, (int4*)out_K, (int4*)out_V);
+  return cudaGetLastError();
+}
+
+}  // namespace nacl

@@ -1,0 +1,90 @@
+// nacl_internal.cuh -- declarations shared by the translation units of libnacl_evict.so.
+// Product code (CUDA path).  Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "nacl_evict.h"
+
+namespace nacl {
+
+constexpr int kNumSMs = 148;  // B200; grid sizing and the workspace formula assume it
+
+// ------------------------------------------------------------------ shape / plan
+struct Shape {
+  int batch, L, Hq, Hkv, d, P;
+  int G;        // Hq / Hkv
+  int rows;     // G * P proxy rows per kv head
+  int dtype;    // NACL_DTYPE_*
+  int esize;    // bytes per element
+};
+
+// How L is split for the split-L softmax statistics (a pure function of the shape).
+struct SplitPlan {
+  int chunk;     // keys per chunk (multiple of 128)
+  int n_chunks;  // ceil(L / chunk)
+};
+SplitPlan make_split_plan(int batch, int L, int Hkv);
+
+// Workspace carve-up (all offsets 256-byte aligned).
+struct Workspace {
+  float2* part;        // [batch*Hq*P, n_chunks]  (m, Z) partial softmax statistics per row and chunk
+  float* lse;          // [batch*Hq*P]            natural-log LSE of every proxy row
+  float* imp;          // [batch*Hkv, L]          importance F_score
+  uint32_t* key;       // [batch*Hkv, L]          order-mapped fp32 Gumbel-top-k keys
+  int* sync;           // [kSyncInts]             counters of the persistent tensor-core kernel (zeroed per call)
+  size_t bytes;
+};
+constexpr int kSyncInts = 4096;
+Workspace carve_workspace(void* base, int batch, int L, int Hq, int Hkv, int P);
+
+// ------------------------------------------------------------------ kernels (launchers)
+// Each launcher enqueues on `st` and returns the cudaError_t of the launch.
+
+// generic CUDA-core scoring (any dtype / d / G*P): 3 launches
+cudaError_t launch_score_generic(const Shape& s, const void* K, const void* Q, const SplitPlan& sp,
+                                 const Workspace& ws, float* imp_out, float* lse_out, cudaStream_t st);
+
+// tensor-core scoring (bf16, d == 128, G*P % 16 == 0, G*P <= 256): tcgen05 + TMA
+bool score_tc_supported(const Shape& s);
+int score_tc_launch_count(const Shape& s);
+cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const SplitPlan& sp,
+                            const Workspace& ws, float* imp_out, float* lse_out, cudaStream_t st);
+
+// Gumbel-top-k keys: key[p,j] = ordermap(fl32(ln w(imp) - ln(-ln u)))
+cudaError_t launch_keys(const float* imp, uint32_t* key, int batch, int Hkv, int L,
+                        uint64_t seed, int layer, uint32_t flags, cudaStream_t st);
+
+// protected + top-k + Gumbel-top-k + ascending compaction -> out_idx
+cudaError_t launch_select(const float* imp, const uint32_t* key, int batch, int Hkv, int L,
+                          int budget_proxy, int budget_random, int n_sink, int n_recent,
+                          int32_t* out_idx, cudaStream_t st);
+
+// K,V <- K_S,V_S
+cudaError_t launch_gather(const void* K, const void* V, const int32_t* idx, int n_prob, int L, int C,
+                          int row_bytes, void* out_K, void* out_V, cudaStream_t st);
+
+// ------------------------------------------------------------------ small device helpers
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// merge two (max, sum-exp) softmax partials; (m = -inf, z = 0) is the identity
+__device__ __forceinline__ void merge_mz(float& m, float& z, float m2, float z2) {
+  float mn = fmaxf(m, m2);
+  if (mn == -INFINITY) { m = mn; z = 0.f; return; }
+  z = z * expf(m - mn) + z2 * expf(m2 - mn);
+  m = mn;
+}
+
+}  // namespace nacl

@@ -1,0 +1,131 @@
+"""GPU <-> oracle parity protocol (test infrastructure).
+
+1. scores     : |imp_gpu - imp_ref| <= 2e-3*|imp_ref| + 1e-30 for every (b, hk, j)      (north star)
+2. staged     : the oracle's steps 4-7 run on the GPU's own fp32 importance must give exactly the
+                GPU's index list (sharp test of select / sampling keys / compaction)
+3. end-to-end : index sets identical to the oracle's except (a) top-k swaps at positions whose oracle
+                score lies within 2e-3 (relative) of the top-k cutoff, (b) random-stage differences
+                that are such swaps (changed candidate pool) or whose oracle key lies within
+                delta = 2*ln(1+2e-3)+1e-5 of the oracle keys at ranks Br +- n_swap
+4. gather     : out_K/out_V bytewise equal to the rows the GPU's own out_idx names
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+import torch
+
+import oracle
+
+REL_TOL = 2e-3
+KEY_DELTA = 2 * math.log1p(REL_TOL) + 1e-5
+
+
+def host_bits(t: torch.Tensor) -> np.ndarray:
+    return oracle.as_host_array(t)
+
+
+def check_scores(imp_gpu: np.ndarray, imp_ref: np.ndarray, G: int, P: int):
+    err = np.abs(imp_gpu.astype(np.float64) - imp_ref)
+    bound = REL_TOL * np.abs(imp_ref) + 1e-30
+    bad = err > bound
+    assert not bad.any(), f"{bad.sum()} scores outside rel {REL_TOL}: max rel err {np.max(err / (np.abs(imp_ref) + 1e-300)):.3e}"
+    mass = imp_gpu.astype(np.float64).sum(-1)
+    np.testing.assert_allclose(mass, G * P, rtol=1e-4)
+    return float(np.max(err / (np.abs(imp_ref) + 1e-300)))
+
+
+def check_staged(idx_gpu: np.ndarray, imp_gpu: np.ndarray, Bp, Br, n_sink, n_recent, seed, layer, flags=0):
+    idx_st, part_st = oracle.select(imp_gpu, Bp, Br, n_sink, n_recent, seed, layer, flags, return_parts=True)
+    np.testing.assert_array_equal(idx_gpu, idx_st)
+    return part_st
+
+
+def check_structure(idx: np.ndarray, L, C, n_sink, n_recent):
+    assert idx.shape[-1] == C
+    if C == 0:
+        return
+    assert idx.min() >= 0 and idx.max() < L
+    if C > 1:
+        assert np.all(np.diff(idx.astype(np.int64), axis=-1) > 0), "indices not strictly ascending"
+    prot = np.concatenate([np.arange(n_sink), np.arange(L - n_recent, L)])
+    flat = idx.reshape(-1, C)
+    for row in flat:
+        assert np.isin(prot, row).all(), "protected position missing"
+
+
+def check_e2e_sets(idx_gpu, part_gpu, imp_ref, Bp, Br, n_sink, n_recent, seed, layer, flags=0):
+    """Returns (n_topk_swaps, n_random_diffs) summed over heads; asserts every difference is admissible."""
+    idx_ref, part_ref, key_ref = oracle.select(imp_ref, Bp, Br, n_sink, n_recent, seed, layer, flags,
+                                               return_parts=True, return_keys=True)
+    B, Hkv, L = imp_ref.shape
+    k1 = Bp - n_sink - n_recent
+    tot_swaps = tot_rand = 0
+    for b in range(B):
+        for h in range(Hkv):
+            ig, pg, ir, pr = idx_gpu[b, h], part_gpu[b, h], idx_ref[b, h], part_ref[b, h]
+            Tg, Tr = set(ig[pg == 1].tolist()), set(ir[pr == 1].tolist())
+            Ug, Ur = set(ig[pg == 2].tolist()), set(ir[pr == 2].tolist())
+            swaps = Tg ^ Tr
+            if swaps:
+                s = imp_ref[b, h]
+                free = np.sort(s[n_sink:L - n_recent])[::-1]
+                tau = free[k1 - 1] if k1 > 0 else np.inf
+                for j in swaps:
+                    assert abs(s[j] - tau) <= REL_TOL * tau + 1e-30, f"top-k mismatch at ({b},{h},{j}) outside the band"
+            n_swap = len(swaps) // 2 + len(swaps) % 2
+            rdiff = Ug ^ Ur
+            if rdiff:
+                keys = key_ref[b, h]
+                cand = np.sort(keys[~np.isnan(keys)])[::-1]
+                hi_rank = max(Br - n_swap, 1)
+                lo_rank = min(Br + n_swap + 1, len(cand))
+                k_hi, k_lo = cand[hi_rank - 1] + KEY_DELTA, cand[lo_rank - 1] - KEY_DELTA
+                for j in rdiff:
+                    if j in swaps:
+                        continue
+                    kj = keys[j]
+                    assert not np.isnan(kj) and k_lo <= kj <= k_hi, f"random-stage mismatch at ({b},{h},{j}) outside the band"
+            tot_swaps += len(swaps)
+            tot_rand += len(rdiff)
+    return tot_swaps, tot_rand
+
+
+def check_gather(K, V, out_K, out_V, idx_gpu):
+    Kb, Vb = host_bits(K), host_bits(V)
+    oK, oV = host_bits(out_K), host_bits(out_V)
+    B, Hkv = idx_gpu.shape[:2]
+    for b in range(B):
+        for h in range(Hkv):
+            np.testing.assert_array_equal(oK[b, h], Kb[b, h, idx_gpu[b, h]])
+            np.testing.assert_array_equal(oV[b, h], Vb[b, h, idx_gpu[b, h]])
+
+
+def full_parity(K, V, Q, Bp, Br, n_sink, n_recent, seed, layer, flags=0, oracle_flags=None, imp_ref=None):
+    """Runs the CUDA path through the C ABI on cuda:0 and every check above.  K,V,Q are HOST tensors."""
+    from paper_2408_03675_b200 import binding
+
+    dev = torch.device("cuda:0")
+    Kd, Vd, Qd = K.to(dev), V.to(dev), Q.to(dev)
+    res = binding.nacl_evict_ex(Kd, Vd, Qd, Bp, Br, n_sink, n_recent, seed, layer, flags=flags, want_importance=True)
+    torch.cuda.synchronize()
+    idx_gpu = res["out_idx"].cpu().numpy()
+    imp_gpu = res["importance"].cpu().numpy()
+    B, Hkv, L, d = K.shape
+    Hq, P = Q.shape[1], Q.shape[2]
+    G = Hq // Hkv
+    oflags = (flags & 0x7) if oracle_flags is None else oracle_flags
+    if imp_ref is None:
+        imp_ref = oracle.importance(K, Q, flags=oflags & oracle.CAUSAL)
+    max_rel = check_scores(imp_gpu, imp_ref, G, P)
+    check_structure(idx_gpu, L, Bp + Br, n_sink, n_recent)
+    part_gpu = check_staged(idx_gpu, imp_gpu, Bp, Br, n_sink, n_recent, seed, layer, oflags)
+    swaps, rdiff = check_e2e_sets(idx_gpu, part_gpu, imp_ref, Bp, Br, n_sink, n_recent, seed, layer, oflags)
+    check_gather(K, V, res["out_K"].cpu(), res["out_V"].cpu(), idx_gpu)
+    # determinism: a second run is bit-identical
+    res2 = binding.nacl_evict_ex(Kd, Vd, Qd, Bp, Br, n_sink, n_recent, seed, layer, flags=flags, want_importance=True)
+    torch.cuda.synchronize()
+    assert torch.equal(res2["out_idx"], res["out_idx"]) and torch.equal(res2["importance"], res["importance"])
+    assert torch.equal(res2["out_K"].view(torch.uint8), res["out_K"].view(torch.uint8))
+    return {"max_rel_err": max_rel, "topk_swaps": swaps, "random_diffs": rdiff, "imp_gpu": imp_gpu, "idx_gpu": idx_gpu}

@@ -1,0 +1,108 @@
+"""CPU-side checks of the C ABI: the library loads, exports every symbol include/nacl_evict.h declares,
+and its host-side validation (which never touches device memory) returns the documented codes."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2408_03675_b200 import build as nacl_build
+from paper_2408_03675_b200 import CONFIGS
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    path = nacl_build.build()
+    L = C.CDLL(path)
+    L.nacl_strerror.restype = C.c_char_p
+    L.nacl_workspace_bytes.restype = C.c_size_t
+    return L
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "nacl_evict.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(nacl_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = declared_symbols()
+    assert {"nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in include/nacl_evict.h but not exported"
+
+
+def test_version_and_strerror(lib):
+    assert lib.nacl_version() == 100
+    for code in range(0, -8, -1):
+        assert lib.nacl_strerror(code)
+    assert b"unknown" in lib.nacl_strerror(-99)
+
+
+def test_workspace_bytes_is_a_pure_function_of_shape(lib):
+    for cfg in CONFIGS.values():
+        w = lib.nacl_workspace_bytes(cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P)
+        assert w == lib.nacl_workspace_bytes(cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P)
+        # at least the importance and the key vectors
+        assert w >= 2 * 4 * cfg.batch * cfg.Hkv * cfg.L
+        assert w < 64 << 20
+    assert lib.nacl_workspace_bytes(1, 0, 4, 4, 64, 1) == 0
+    assert lib.nacl_workspace_bytes(1, 128, 5, 4, 64, 1) == 0  # Hq % Hkv
+
+
+def _call(lib, fn, K=0x1000, V=0x2000, Q=0x3000, batch=1, L=512, Hq=4, Hkv=4, d=64, P=16, bp=76, br=26, ns=4, nr=16,
+          oK=0x4000, oV=0x5000, oidx=0x6000):
+    f = getattr(lib, fn)
+    f.argtypes = [C.c_void_p] * 3 + [C.c_int] * 10 + [C.c_uint64, C.c_int] + [C.c_void_p] * 4
+    f.restype = C.c_int
+    return f(K, V, Q, batch, L, Hq, Hkv, d, P, bp, br, ns, nr, 0, 0, oK, oV, oidx, None)
+
+
+@pytest.mark.parametrize("fn", ["nacl_evict", "nacl_evict_f32"])
+def test_validation_codes_without_touching_the_device(lib, fn):
+    # fake (never dereferenced) pointers: every case below must be rejected on the host
+    assert _call(lib, fn, K=None) == -1
+    assert _call(lib, fn, oidx=None) == -1
+    assert _call(lib, fn, Hq=6) == -2            # Hq % Hkv
+    assert _call(lib, fn, P=600) == -2           # P > L
+    assert _call(lib, fn, d=72) == -2            # d % 16
+    assert _call(lib, fn, L=(1 << 24) + 1) == -2
+    assert _call(lib, fn, bp=10) == -3           # budget_proxy < n_sink + n_recent
+    assert _call(lib, fn, bp=500, br=13) == -3   # total > L
+    assert _call(lib, fn, br=-1) == -3
+    assert _call(lib, fn, ns=400, nr=200) == -3  # protected > L
+    assert _call(lib, fn, K=0x1008) == -4        # misaligned
+
+
+def test_ex_rejects_wrong_struct_and_unknown_flags(lib):
+    from paper_2408_03675_b200.binding import NaclParams
+
+    p = NaclParams()
+    p.struct_size = 8
+    lib.nacl_evict_ex.argtypes = [C.POINTER(NaclParams)]
+    assert lib.nacl_evict_ex(C.byref(p)) == -7
+    assert lib.nacl_evict_ex(None) == -1
+    p.struct_size = C.sizeof(NaclParams)
+    p.dtype = 1
+    p.K, p.V, p.Qproxy, p.out_K, p.out_V, p.out_idx = 0x1000, 0x2000, 0x3000, 0x4000, 0x5000, 0x6000
+    p.batch, p.L, p.Hq, p.Hkv, p.d, p.P = 1, 512, 4, 4, 64, 16
+    p.budget_proxy, p.budget_random, p.n_sink, p.n_recent = 76, 26, 4, 16
+    p.flags = 1  # CAUSAL: oracle-only for now
+    assert lib.nacl_evict_ex(C.byref(p)) == -7
+    p.flags = 0x8000
+    assert lib.nacl_evict_ex(C.byref(p)) == -7
+    p.flags = 0
+    p.workspace, p.workspace_bytes = 0x10000, 16
+    assert lib.nacl_evict_ex(C.byref(p)) == -5
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2408_03675_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert "nacl_oracle" not in txt, f

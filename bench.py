@@ -1,0 +1,379 @@
+#!/usr/bin/env python
+"""bench.py -- NACL encoding-phase eviction throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+
+One *step* = one pass of the whole hot path over one batch
+of synthetic prompts: every layer of the workload is evicted once through the C ABI
+(`nacl_evict`, include/nacl_evict.h).  Default workload: BASELINE.json configs[3] -- the L=32k
+configuration the metric is quoted on (Mistral-7B-shaped GQA, batch 4, 32 layers).  Each layer has
+its own K/V/Q and output buffers (16 GiB of K/V in total), so every timed call reads inputs that
+are cold in the 126 MB L2.
+
+Prints ONE JSON line (rank 0).  `value` = KV GB/s = algorithmic bytes / device time, with
+algorithmic bytes per layer = B*Hkv*d*e*(L + 4C): K read once for scoring + C rows of K and of V
+read and written (BASELINE.json north star).
+
+Multi-GPU (torchrun): the path shards over independent batch elements with no data-path
+collective; every rank evicts its own batch of prompts ("weak" scaling),
+`value` = bytes of all ranks / max-over-ranks device time.
+
+`--impl reference`: there is no reference implementation to install (the reference is a paper);
+per the task's tier framing this arm times the fp64 CPU oracle (oracle/) on the host cores,
+each step a bounded sample (one layer) of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import torch  # noqa: E402
+
+from paper_2408_03675_b200 import CONFIGS  # noqa: E402
+from paper_2408_03675_b200 import dist as nacl_dist  # noqa: E402
+from paper_2408_03675_b200.inputs import make_layer_inputs  # noqa: E402
+
+METRIC = "eviction throughput per layer at L=32k (KV GB/s)"
+UNIT = "GB/s"
+
+
+def load_peaks() -> dict:
+    """Measured roofline denominators (driver-written); the profiling guide's fallback otherwise."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        p["source"] = "measured (MEASURED_PEAKS.json)"
+        return p
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0,
+            "source": "fallback (B200_PROFILING.md)"}
+
+
+class ClockSampler:
+    """Samples SM clock / throttle reasons with nvidia-smi while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines: list[str] = []
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._pump, daemon=True)
+        self.thread.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        if self.thread is not None:
+            self.thread.join(timeout=2)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.lines:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+                pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------ workload
+def workload_desc(cfg, layers, world) -> dict:
+    Bp, Br = cfg.budgets()
+    return {
+        "workload": cfg.name, "layers": layers, "batch_per_gpu": cfg.batch, "global_batch": cfg.batch * world,
+        "L": cfg.L, "Hq": cfg.Hq, "Hkv": cfg.Hkv, "head_dim": cfg.d, "P": cfg.P, "budget_proxy": Bp, "budget_random": Br,
+        "n_sink": cfg.n_sink, "n_recent": cfg.n_recent, "heavy_hitter_rate": cfg.hh_rate, "alpha": cfg.hh_alpha,
+        "parallelism": f"batch-sharded x{world}, no collective", "l2": "inputs_exceed_l2 (distinct K/V per layer)",
+        "alg_bytes_per_layer": cfg.alg_bytes_per_layer(),
+    }
+
+
+def stage_alg_bytes(cfg) -> dict:
+    """Algorithmic HBM bytes one launch of each kernel has to move."""
+    kv_head = cfg.batch * cfg.Hkv
+    k_bytes = kv_head * cfg.L * cfg.d * cfg.elem_bytes
+    imp_bytes = kv_head * cfg.L * 4
+    return {
+        "score_stats": k_bytes,                      # K streamed once
+        "score_combine": 0,
+        "score_colsum": k_bytes + imp_bytes,         # K streamed again (L2 hits show up as traffic < this) + imp written
+        "score_fused": k_bytes + imp_bytes,          # both sweeps in one launch: K once
+        "gumbel_keys": 2 * imp_bytes,
+        "select": 2 * imp_bytes + kv_head * cfg.C * 4,
+        "gather": 4 * kv_head * cfg.C * cfg.d * cfg.elem_bytes + kv_head * cfg.C * 4,
+    }
+
+
+def load_traffic(cfg_name: str, kernel: str):
+    """dram bytes per launch of `kernel` from the committed ncu --set full summary, if one exists."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(path) as f:
+            t = json.load(f)
+        return t.get(cfg_name, {}).get(kernel)
+    except (OSError, ValueError):
+        return None
+
+
+def run_ours(args) -> dict:
+    from paper_2408_03675_b200 import binding  # raises when libnacl_evict.so cannot be built/loaded: no fallback
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device for --impl ours (there is no CPU fallback)")
+    rank, local_rank, world = nacl_dist.init()
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    cfg = CONFIGS[args.config]
+    layers = args.layers or cfg.layers
+    Bp, Br = cfg.budgets()
+    C = Bp + Br
+    tdt = torch.float32 if cfg.dtype == "f32" else torch.bfloat16
+    rank_cfg = cfg.scaled(config_id=cfg.config_id + 10 * rank)  # every rank evicts its own batch of prompts
+
+    data = []
+    for l in range(layers):
+        K, V, Q, _ = make_layer_inputs(rank_cfg, layer=l, device=dev)
+        oK = torch.empty((cfg.batch, cfg.Hkv, C, cfg.d), dtype=tdt, device=dev)
+        oV = torch.empty_like(oK)
+        oi = torch.empty((cfg.batch, cfg.Hkv, C), dtype=torch.int32, device=dev)
+        data.append((K, V, Q, oK, oV, oi))
+    ws = torch.empty(binding.nacl_workspace_bytes(cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P) + 256,
+                     dtype=torch.uint8, device=dev)
+    off = (-ws.data_ptr()) % 256
+    ws = ws[off:]
+    stream = torch.cuda.current_stream(dev)
+
+    def step():
+        for l, (K, V, Q, oK, oV, oi) in enumerate(data):
+            binding.nacl_evict_ex(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l,
+                                  out_K=oK, out_V=oV, out_idx=oi, workspace=ws, stream=stream)
+
+    def timed(n_steps: int) -> float:
+        nacl_dist.barrier(dev)
+        torch.cuda.synchronize(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(n_steps):
+            step()
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        nacl_dist.barrier(dev)
+        return nacl_dist.max_over_ranks(e0.elapsed_time(e1), dev)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ms_total = timed(args.steps)
+    # the same region again with per-kernel events (include/nacl_evict.h nacl_profile_*), for the roofline
+    binding.nacl_profile_enable(True)
+    binding.nacl_profile_read(reset=True)
+    ms_total_prof = timed(args.steps)
+    stages = binding.nacl_profile_read(reset=True)
+    binding.nacl_profile_enable(False)
+    clocks = sampler.stop() if rank == 0 else None
+
+    ms_per_step = ms_total / args.steps
+    alg_bytes_step = cfg.alg_bytes_per_layer() * layers * world
+    value = alg_bytes_step / (ms_per_step * 1e-3) / 1e9
+    peaks = load_peaks()
+
+    # ---- roofline of the dominant kernel
+    sab = stage_alg_bytes(cfg)
+    stage_rows = {}
+    for name, (ms, n) in stages.items():
+        if n == 0:
+            continue
+        avg_us = ms / n * 1e3
+        stage_rows[name] = {"launches": n, "avg_us": round(avg_us, 2), "share": None,
+                            "alg_GBps": round(sab.get(name, 0) / (avg_us * 1e-6) / 1e9, 1)}
+    tot = sum(r["avg_us"] * r["launches"] for r in stage_rows.values()) or 1.0
+    for r in stage_rows.values():
+        r["share"] = round(r["avg_us"] * r["launches"] / tot, 4)
+    dom = max(stage_rows, key=lambda k: stage_rows[k]["avg_us"] * stage_rows[k]["launches"]) if stage_rows else None
+    roofline = None
+    if dom:
+        ach = stage_rows[dom]["alg_GBps"]
+        roofline = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": round(ach / peaks["hbm_gbs"], 4), "traffic": load_traffic(cfg.name, dom),
+                    "peak_source": peaks["source"], "alg_bytes_per_launch": sab.get(dom, 0)}
+
+    # ---- end to end through the host entry point: pinned host buffers, H2D + D2H inside the timed region
+    e2e = run_e2e(binding, cfg, layers, data, Bp, Br, dev, args, world)
+
+    out = {
+        "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic (seeded N(0,1) Q/K/V + planted heavy hitters, DESIGN.md section 4)",
+        "config": workload_desc(cfg, layers, world),
+        "us_per_layer": round(ms_per_step * 1e3 / layers, 2),
+        "prompt_tokens_per_s": round(cfg.batch * cfg.L * layers * world / (ms_per_step * 1e-3), 1),
+        "evicted_token_slots_per_s": round(cfg.batch * cfg.Hkv * (cfg.L - C) * layers * world / (ms_per_step * 1e-3), 1),
+        "hbm_frac_of_measured": round(value / world / peaks["hbm_gbs"], 4),
+        "hbm_frac_of_nominal_8TBps": round(value / world / 8000.0, 4),
+        "clocks": clocks, "e2e": e2e,
+        "gpu_launches": args.steps * layers * binding.nacl_launch_count(
+            1 if cfg.dtype == "bf16" else 0, cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P),
+        "roofline": roofline, "kernels": stage_rows,
+        "ms_per_step_with_kernel_events": round(ms_total_prof / args.steps, 4),
+        "library": os.path.relpath(binding.library_path(), ROOT),
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = run_cpu_sample(cfg, max_seconds=12.0, max_layers=4)
+    else:
+        out["cpu_baseline"] = None
+    nacl_dist.finalize()
+    return out if rank == 0 else {}
+
+
+def run_e2e(binding, cfg, layers, data, Bp, Br, dev, args, world) -> dict:
+    """The same metric through `nacl_evict_host` (HOST buffers in, HOST buffers out): every layer's
+    K/V/Q is copied from pinned host memory and its compacted K/V + index list is copied back, all
+    inside the timed region.  Host copies of the first `n_sets` layers are rotated over the layers."""
+    C = Bp + Br
+    n_sets = min(layers, 4)
+    host = []
+    for l in range(n_sets):
+        K, V, Q = data[l][0], data[l][1], data[l][2]
+        hK, hV, hQ = K.cpu().pin_memory(), V.cpu().pin_memory(), Q.cpu().pin_memory()
+        hoK = torch.empty((cfg.batch, cfg.Hkv, C, cfg.d), dtype=K.dtype, pin_memory=True)
+        hoV = torch.empty_like(hoK, pin_memory=True)
+        hoi = torch.empty((cfg.batch, cfg.Hkv, C), dtype=torch.int32, pin_memory=True)
+        host.append((hK, hV, hQ, hoK, hoV, hoi))
+    h2d = sum(t.numel() * t.element_size() for t in host[0][:3])
+    d2h = sum(t.numel() * t.element_size() for t in host[0][3:])
+
+    def step():
+        for l in range(layers):
+            hK, hV, hQ, hoK, hoV, hoi = host[l % n_sets]
+            binding.nacl_evict_host(hK, hV, hQ, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l,
+                                    out_K=hoK, out_V=hoV, out_idx=hoi, device=dev.index)
+
+    step()  # warm-up: staging buffers are allocated on first use
+    n_steps = max(1, min(args.steps, 2))
+    nacl_dist.barrier(dev)
+    torch.cuda.synchronize(dev)
+    t0 = time.perf_counter()
+    for _ in range(n_steps):
+        step()
+    torch.cuda.synchronize(dev)
+    dt = time.perf_counter() - t0
+    nacl_dist.barrier(dev)
+    dt = nacl_dist.max_over_ranks(dt, dev)
+    val = cfg.alg_bytes_per_layer() * layers * world * n_steps / dt / 1e9
+    return {"value": round(val, 3), "unit": UNIT, "h2d_bytes_per_step": h2d * layers, "d2h_bytes_per_step": d2h * layers,
+            "steps": n_steps, "ms_per_step": round(dt / n_steps * 1e3, 3), "api": "nacl_evict_host (pinned host buffers)",
+            "host_sets_rotated": n_sets, "timer": "host wall clock around synchronous calls, max over ranks"}
+
+
+def run_cpu_sample(cfg, max_seconds: float, max_layers: int, layer0: int = 0) -> dict:
+    """Times the fp64 oracle as it stands on the host cores over whole layers of the workload until
+    `max_seconds` of CPU work or `max_layers` layers."""
+    import oracle
+
+    Bp, Br = cfg.budgets()
+    n, spent = 0, 0.0
+    while n < max_layers and spent < max_seconds:
+        K, V, Q, _ = make_layer_inputs(cfg, layer=layer0 + n, device="cpu")
+        t0 = time.perf_counter()
+        oracle.evict(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(layer0 + n), layer0 + n)
+        spent += time.perf_counter() - t0
+        n += 1
+    val = cfg.alg_bytes_per_layer() * n / spent / 1e9
+    return {"value": round(val, 5), "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
+            "sample": f"{n} whole layer(s) of {cfg.name} (layers {layer0}..{layer0 + n - 1}), {spent:.1f} s of oracle time",
+            "s_per_layer": round(spent / n, 3)}
+
+
+def run_reference(args) -> dict:
+    """`--impl reference`: the oracle on the host cores; one step = one whole layer of the workload."""
+    rank, _, world = nacl_dist.env_world()
+    if rank != 0:
+        return {}
+    import oracle
+
+    cfg = CONFIGS[args.config]
+    Bp, Br = cfg.budgets()
+    steps, warmup = max(1, min(args.steps, 4)), max(0, min(args.warmup, 1))
+    inputs = [make_layer_inputs(cfg, layer=l, device="cpu") for l in range(max(steps, 1))]
+    for w in range(warmup):
+        K, V, Q, _ = inputs[0]
+        oracle.evict(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(0), 0)
+    t0 = time.perf_counter()
+    for l in range(steps):
+        K, V, Q, _ = inputs[l]
+        oracle.evict(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l)
+    dt = time.perf_counter() - t0
+    val = cfg.alg_bytes_per_layer() * steps / dt / 1e9
+    desc = workload_desc(cfg, cfg.layers, 1)
+    sample = f"each step = one whole layer of {cfg.name}; {steps} step(s), {dt:.1f} s"
+    return {
+        "impl": "reference", "metric": METRIC, "value": round(val, 5), "unit": UNIT, "n_gpus": world, "steps": steps,
+        "warmup": warmup, "ms_per_step": round(dt / steps * 1e3, 2), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic (same seeded generator as the CUDA arm)", "config": desc,
+        "cpu_baseline": {"value": round(val, 5), "unit": UNIT, "cores": oracle.threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": round(val, 5), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0, "note": "fp64 CPU oracle (oracle/), rank 0 only; the reference is a paper with no code",
+    }
+
+
+def main() -> int:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", type=int, default=4, choices=sorted(CONFIGS))
+    ap.add_argument("--layers", type=int, default=0, help="override the number of layers per step (0 = the workload's)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    out = run_reference(args) if args.impl == "reference" else run_ours(args)
+    if out:
+        print(json.dumps(out), flush=True)
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

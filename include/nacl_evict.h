@@ -40,6 +40,8 @@
  * Same inputs and seed give bit-identical outputs run to run (no floating-point atomics).
  * nacl_evict_host is the same operation on HOST buffers (copies inside; synchronous).
  *
+ * With budget_proxy + budget_random == 0 the outputs are empty and their pointers may be NULL.
+ *
  * Errors: 0 = OK; negative = error; nothing is thrown and no output is written on a
  * validation error.  Validation is host-side and never reads device memory.
  *
@@ -131,6 +133,17 @@ size_t nacl_workspace_bytes(int batch, int L, int Hq, int Hkv, int d, int P);
 
 /* Number of kernels one call with these arguments launches (for launch accounting). */
 int nacl_launch_count(int dtype, int batch, int L, int Hq, int Hkv, int d, int P, uint32_t flags);
+
+/* Per-stage device timing, for benchmarks.  While enabled, every call brackets each of its kernel
+ * launches with a pair of CUDA events on the call's stream (so calls are NOT graph-capturable while
+ * enabled).  nacl_profile_read waits for the recorded events, adds their elapsed times to per-stage
+ * totals and returns the totals accumulated since the last reset: ms[s] = device milliseconds and
+ * launches[s] = kernel launches of stage s, s < NACL_N_STAGES (stage names: nacl_stage_name).
+ * Either output may be NULL.  Returns 0 or NACL_ERR_CUDA. */
+#define NACL_N_STAGES 6
+int nacl_profile_enable(int on);
+int nacl_profile_read(double* ms, int64_t* launches, int reset);
+const char* nacl_stage_name(int stage);
 
 /* Frees the per-device internal workspaces / staging buffers (optional, e.g. before exit). */
 void nacl_release(void);

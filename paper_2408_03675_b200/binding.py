@@ -18,7 +18,9 @@ NACL_DTYPE_F32, NACL_DTYPE_BF16 = 0, 1
 FLAG_CAUSAL, FLAG_SAMPLE_SOFTMAX_OF_SCORE, FLAG_SAMPLE_UNIFORM, FLAG_SCORE_CUDA_CORES = 1, 2, 4, 0x100
 
 EXPORTS = ("nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes",
-           "nacl_launch_count", "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version")
+           "nacl_launch_count", "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version",
+           "nacl_profile_enable", "nacl_profile_read", "nacl_stage_name")
+N_STAGES = 6
 
 
 class NaclParams(C.Structure):
@@ -73,6 +75,12 @@ def _load() -> C.CDLL:
     lib.nacl_last_cuda_error.restype = i32
     lib.nacl_version.argtypes = []
     lib.nacl_version.restype = i32
+    lib.nacl_profile_enable.argtypes = [i32]
+    lib.nacl_profile_enable.restype = i32
+    lib.nacl_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int64), i32]
+    lib.nacl_profile_read.restype = i32
+    lib.nacl_stage_name.argtypes = [i32]
+    lib.nacl_stage_name.restype = C.c_char_p
     return lib
 
 
@@ -114,6 +122,20 @@ def nacl_launch_count(dtype, batch, L, Hq, Hkv, d, P, flags=0) -> int:
 
 def nacl_release() -> None:
     _lib.nacl_release()
+
+
+def nacl_profile_enable(on: bool) -> None:
+    _lib.nacl_profile_enable(1 if on else 0)
+
+
+def nacl_profile_read(reset: bool = True) -> dict:
+    """{stage name: (device ms, launches)} accumulated since the last reset (include/nacl_evict.h)."""
+    ms = (C.c_double * N_STAGES)()
+    n = (C.c_int64 * N_STAGES)()
+    rc = _lib.nacl_profile_read(ms, n, 1 if reset else 0)
+    if rc != 0:
+        raise NaclError(rc, "nacl_profile_read")
+    return {_lib.nacl_stage_name(s).decode(): (float(ms[s]), int(n[s])) for s in range(N_STAGES)}
 
 
 def nacl_evict(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer,

@@ -4,6 +4,7 @@
 // nacl_evict_host, which is documented as synchronous).
 #include <mutex>
 #include <new>
+#include <vector>
 
 #include "nacl_internal.cuh"
 
@@ -12,6 +13,37 @@ namespace nacl {
 static thread_local int g_last_cuda_error = 0;
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ------------------------------------------------------------------ per-stage timing
+struct ProfRecord { int stage; cudaEvent_t a, b; };
+static std::mutex g_prof_mu;
+static bool g_prof_on = false;
+static std::vector<ProfRecord> g_prof_pending;
+static std::vector<cudaEvent_t> g_prof_free;
+static double g_prof_ms[ST_COUNT] = {0, 0, 0, 0, 0, 0};
+static int64_t g_prof_n[ST_COUNT] = {0, 0, 0, 0, 0, 0};
+
+static cudaEvent_t prof_event() {
+  if (!g_prof_free.empty()) { cudaEvent_t e = g_prof_free.back(); g_prof_free.pop_back(); return e; }
+  cudaEvent_t e = nullptr;
+  if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  return e;
+}
+
+StageScope::StageScope(int stage, cudaStream_t st) : stage_(stage), st_(st), slot_(-1) {
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  if (!g_prof_on) return;
+  ProfRecord r{stage, prof_event(), prof_event()};
+  if (!r.a || !r.b) return;
+  cudaEventRecord(r.a, st);
+  g_prof_pending.push_back(r);
+  slot_ = (int)g_prof_pending.size() - 1;
+}
+StageScope::~StageScope() {
+  if (slot_ < 0) return;
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  if (slot_ < (int)g_prof_pending.size()) cudaEventRecord(g_prof_pending[slot_].b, st_);
+}
 
 SplitPlan make_split_plan(int batch, int L, int Hkv) {
   // about 8 work items per SM so that a dynamically scheduled grid ends with a short tail
@@ -101,7 +133,10 @@ static int fail_cuda(cudaError_t e) {
 
 // ------------------------------------------------------------------ the call
 static int evict_impl(const nacl_params_t& p) {
-  if (!p.K || !p.V || !p.Qproxy || !p.out_K || !p.out_V || !p.out_idx) return NACL_ERR_NULL;
+  if (!p.K || !p.V || !p.Qproxy) return NACL_ERR_NULL;
+  // an empty budget (C == 0) has empty outputs: their pointers may be NULL
+  const bool empty_out = p.budget_proxy == 0 && p.budget_random == 0;
+  if (!empty_out && (!p.out_K || !p.out_V || !p.out_idx)) return NACL_ERR_NULL;
   int rc = validate_shape(p.dtype, p.batch, p.L, p.Hq, p.Hkv, p.d, p.P);
   if (rc) return rc;
   rc = validate_budget(p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent);
@@ -146,13 +181,20 @@ static int evict_impl(const nacl_params_t& p) {
 
   const int C = p.budget_proxy + p.budget_random;
   if (p.budget_random > 0) {
+    StageScope sc(ST_KEYS, st);
     e = launch_keys(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.seed, p.layer, p.flags, st);
     if (e != cudaSuccess) return fail_cuda(e);
   }
-  e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent,
-                    p.out_idx, st);
+  {
+    StageScope sc(ST_SELECT, st);
+    e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent,
+                      p.out_idx, st);
+  }
   if (e != cudaSuccess) return fail_cuda(e);
-  e = launch_gather(p.K, p.V, p.out_idx, p.batch * p.Hkv, p.L, C, row_bytes, p.out_K, p.out_V, st);
+  {
+    StageScope sc(ST_GATHER, st);
+    e = launch_gather(p.K, p.V, p.out_idx, p.batch * p.Hkv, p.L, C, row_bytes, p.out_K, p.out_V, st);
+  }
   if (e != cudaSuccess) return fail_cuda(e);
   return NACL_OK;
 }
@@ -271,6 +313,45 @@ int nacl_launch_count(int dtype, int batch, int L, int Hq, int Hkv, int d, int P
   const bool tc = !(flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
   // scoring + keys + select + gather (budget_random > 0 and C > 0 assumed)
   return (tc ? score_tc_launch_count(s) : 3) + 3;
+}
+
+int nacl_profile_enable(int on) {
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  g_prof_on = on != 0;
+  return NACL_OK;
+}
+
+int nacl_profile_read(double* ms, int64_t* launches, int reset) {
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  int rc = NACL_OK;
+  for (const ProfRecord& r : g_prof_pending) {
+    float t = 0.f;
+    cudaError_t e = cudaEventSynchronize(r.b);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&t, r.a, r.b);
+    if (e != cudaSuccess) { rc = fail_cuda(e); }
+    else { g_prof_ms[r.stage] += (double)t; g_prof_n[r.stage] += 1; }
+    g_prof_free.push_back(r.a);
+    g_prof_free.push_back(r.b);
+  }
+  g_prof_pending.clear();
+  for (int s = 0; s < ST_COUNT; ++s) {
+    if (ms) ms[s] = g_prof_ms[s];
+    if (launches) launches[s] = g_prof_n[s];
+    if (reset) { g_prof_ms[s] = 0; g_prof_n[s] = 0; }
+  }
+  return rc;
+}
+
+const char* nacl_stage_name(int stage) {
+  switch (stage) {
+    case ST_STATS: return "score_stats";
+    case ST_COMBINE: return "score_combine";
+    case ST_COLSUM: return "score_colsum";
+    case ST_KEYS: return "gumbel_keys";
+    case ST_SELECT: return "select";
+    case ST_GATHER: return "gather";
+    default: return "?";
+  }
 }
 
 void nacl_release(void) {

@@ -41,6 +41,17 @@ struct Workspace {
 constexpr int kSyncInts = 4096;
 Workspace carve_workspace(void* base, int batch, int L, int Hq, int Hkv, int P);
 
+// ------------------------------------------------------------------ per-stage device timing (nacl_profile_*)
+enum Stage { ST_STATS = 0, ST_COMBINE, ST_COLSUM, ST_KEYS, ST_SELECT, ST_GATHER, ST_COUNT };
+// Brackets one kernel launch with two CUDA events on `st` while profiling is enabled; free otherwise.
+struct StageScope {
+  StageScope(int stage, cudaStream_t st);
+  ~StageScope();
+  int stage_;
+  cudaStream_t st_;
+  int slot_;  // -1 when profiling is off
+};
+
 // ------------------------------------------------------------------ kernels (launchers)
 // Each launcher enqueues on `st` and returns the cudaError_t of the launch.
 

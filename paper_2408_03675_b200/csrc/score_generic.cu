@@ -167,15 +167,24 @@ cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const Spl
   if ((e = cudaFuncSetAttribute(colsum_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
   const float inv_sqrt_d = 1.0f / sqrtf((float)s.d);
   dim3 g1(sp.n_chunks, s.Hkv, s.batch);
-  stats_kernel<T><<<g1, NT, smem, st>>>((const T*)K, (const T*)Q, ws.part, s.L, s.Hq, s.Hkv, s.d, s.P, s.G, sp.chunk,
-                                        sp.n_chunks, inv_sqrt_d);
+  {
+    StageScope sc(ST_STATS, st);
+    stats_kernel<T><<<g1, NT, smem, st>>>((const T*)K, (const T*)Q, ws.part, s.L, s.Hq, s.Hkv, s.d, s.P, s.G, sp.chunk,
+                                          sp.n_chunks, inv_sqrt_d);
+  }
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   const int n_rows = s.batch * s.Hq * s.P;
-  combine_kernel<<<(n_rows + 127) / 128, 128, 0, st>>>(ws.part, ws.lse, lse_out, n_rows, sp.n_chunks);
+  {
+    StageScope sc(ST_COMBINE, st);
+    combine_kernel<<<(n_rows + 127) / 128, 128, 0, st>>>(ws.part, ws.lse, lse_out, n_rows, sp.n_chunks);
+  }
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   dim3 g2((s.L + TK - 1) / TK, s.Hkv, s.batch);
-  colsum_kernel<T><<<g2, NT, smem, st>>>((const T*)K, (const T*)Q, ws.lse, ws.imp, imp_out, s.L, s.Hq, s.Hkv, s.d, s.P,
-                                         s.G, inv_sqrt_d);
+  {
+    StageScope sc(ST_COLSUM, st);
+    colsum_kernel<T><<<g2, NT, smem, st>>>((const T*)K, (const T*)Q, ws.lse, ws.imp, imp_out, s.L, s.Hq, s.Hkv, s.d, s.P,
+                                           s.G, inv_sqrt_d);
+  }
   return cudaGetLastError();
 }
 

@@ -5,8 +5,12 @@
                 GPU's index list (sharp test of select / sampling keys / compaction)
 3. end-to-end : index sets identical to the oracle's except (a) top-k swaps at positions whose oracle
                 score lies within 2e-3 (relative) of the top-k cutoff, (b) random-stage differences
-                that are such swaps (changed candidate pool) or whose oracle key lies within
-                delta = 2*ln(1+2e-3)+1e-5 of the oracle keys at ranks Br +- n_swap
+                that are such swaps (changed candidate pool), or whose oracle key lies within
+                delta = 2*ln(1+2e-3)+1e-5 of the oracle keys at ranks Br +- n_swap, or whose oracle
+                importance is below the absolute score tolerance 1e-30 (fp32 flushes such scores to
+                zero where fp64 does not, R13: within the stated score tolerance they are
+                indistinguishable from zero, so which of them fills the tail of the sample is not
+                determined; the staged check still pins the kernel's choice exactly)
 4. gather     : out_K/out_V bytewise equal to the rows the GPU's own out_idx names
 """
 from __future__ import annotations
@@ -19,6 +23,7 @@ import torch
 import oracle
 
 REL_TOL = 2e-3
+ABS_TOL = 1e-30
 KEY_DELTA = 2 * math.log1p(REL_TOL) + 1e-5
 
 
@@ -28,7 +33,7 @@ def host_bits(t: torch.Tensor) -> np.ndarray:
 
 def check_scores(imp_gpu: np.ndarray, imp_ref: np.ndarray, G: int, P: int):
     err = np.abs(imp_gpu.astype(np.float64) - imp_ref)
-    bound = REL_TOL * np.abs(imp_ref) + 1e-30
+    bound = REL_TOL * np.abs(imp_ref) + ABS_TOL
     bad = err > bound
     assert not bad.any(), f"{bad.sum()} scores outside rel {REL_TOL}: max rel err {np.max(err / (np.abs(imp_ref) + 1e-300)):.3e}"
     mass = imp_gpu.astype(np.float64).sum(-1)
@@ -73,7 +78,7 @@ def check_e2e_sets(idx_gpu, part_gpu, imp_ref, Bp, Br, n_sink, n_recent, seed, l
                 free = np.sort(s[n_sink:L - n_recent])[::-1]
                 tau = free[k1 - 1] if k1 > 0 else np.inf
                 for j in swaps:
-                    assert abs(s[j] - tau) <= REL_TOL * tau + 1e-30, f"top-k mismatch at ({b},{h},{j}) outside the band"
+                    assert abs(s[j] - tau) <= REL_TOL * tau + ABS_TOL, f"top-k mismatch at ({b},{h},{j}) outside the band"
             n_swap = len(swaps) // 2 + len(swaps) % 2
             rdiff = Ug ^ Ur
             if rdiff:
@@ -83,7 +88,7 @@ def check_e2e_sets(idx_gpu, part_gpu, imp_ref, Bp, Br, n_sink, n_recent, seed, l
                 lo_rank = min(Br + n_swap + 1, len(cand))
                 k_hi, k_lo = cand[hi_rank - 1] + KEY_DELTA, cand[lo_rank - 1] - KEY_DELTA
                 for j in rdiff:
-                    if j in swaps:
+                    if j in swaps or imp_ref[b, h, j] <= ABS_TOL:
                         continue
                     kj = keys[j]
                     assert not np.isnan(kj) and k_lo <= kj <= k_hi, f"random-stage mismatch at ({b},{h},{j}) outside the band"

@@ -140,7 +140,7 @@ int nacl_launch_count(int dtype, int batch, int L, int Hq, int Hkv, int d, int P
  * totals and returns the totals accumulated since the last reset: ms[s] = device milliseconds and
  * launches[s] = kernel launches of stage s, s < NACL_N_STAGES (stage names: nacl_stage_name).
  * Either output may be NULL.  Returns 0 or NACL_ERR_CUDA. */
-#define NACL_N_STAGES 6
+#define NACL_N_STAGES 7
 int nacl_profile_enable(int on);
 int nacl_profile_read(double* ms, int64_t* launches, int reset);
 const char* nacl_stage_name(int stage);

@@ -20,8 +20,8 @@ static std::mutex g_prof_mu;
 static bool g_prof_on = false;
 static std::vector<ProfRecord> g_prof_pending;
 static std::vector<cudaEvent_t> g_prof_free;
-static double g_prof_ms[ST_COUNT] = {0, 0, 0, 0, 0, 0};
-static int64_t g_prof_n[ST_COUNT] = {0, 0, 0, 0, 0, 0};
+static double g_prof_ms[ST_COUNT] = {};
+static int64_t g_prof_n[ST_COUNT] = {};
 
 static cudaEvent_t prof_event() {
   if (!g_prof_free.empty()) { cudaEvent_t e = g_prof_free.back(); g_prof_free.pop_back(); return e; }
@@ -71,7 +71,7 @@ Workspace carve_workspace(void* base, int batch, int L, int Hq, int Hkv, int P) 
   ws.lse = reinterpret_cast<float*>(b + off);   off = align_up(off + n_rows * sizeof(float), 256);
   ws.imp = reinterpret_cast<float*>(b + off);   off = align_up(off + n_imp * sizeof(float), 256);
   ws.key = reinterpret_cast<uint32_t*>(b + off); off = align_up(off + n_imp * sizeof(uint32_t), 256);
-  ws.sync = reinterpret_cast<int*>(b + off);    off = align_up(off + kSyncInts * sizeof(int), 256);
+  ws.sync = reinterpret_cast<int*>(b + off);    off = align_up(off + sync_ints((size_t)batch * Hkv) * sizeof(int), 256);
   ws.bytes = off;
   return ws;
 }
@@ -350,6 +350,7 @@ const char* nacl_stage_name(int stage) {
     case ST_KEYS: return "gumbel_keys";
     case ST_SELECT: return "select";
     case ST_GATHER: return "gather";
+    case ST_FUSED: return "score_fused";
     default: return "?";
   }
 }

@@ -35,14 +35,14 @@ struct Workspace {
   float* lse;          // [batch*Hq*P]            natural-log LSE of every proxy row
   float* imp;          // [batch*Hkv, L]          importance F_score
   uint32_t* key;       // [batch*Hkv, L]          order-mapped fp32 Gumbel-top-k keys
-  int* sync;           // [kSyncInts]             counters of the persistent tensor-core kernel (zeroed per call)
+  int* sync;           // [sync_ints(heads)]      ticket + per-head counters / flags of the persistent tensor-core kernel (zeroed per call)
   size_t bytes;
 };
-constexpr int kSyncInts = 4096;
+inline size_t sync_ints(size_t heads) { return 16 + 2 * heads; }
 Workspace carve_workspace(void* base, int batch, int L, int Hq, int Hkv, int P);
 
 // ------------------------------------------------------------------ per-stage device timing (nacl_profile_*)
-enum Stage { ST_STATS = 0, ST_COMBINE, ST_COLSUM, ST_KEYS, ST_SELECT, ST_GATHER, ST_COUNT };
+enum Stage { ST_STATS = 0, ST_COMBINE, ST_COLSUM, ST_KEYS, ST_SELECT, ST_GATHER, ST_FUSED, ST_COUNT };
 // Brackets one kernel launch with two CUDA events on `st` while profiling is enabled; free otherwise.
 struct StageScope {
   StageScope(int stage, cudaStream_t st);

@@ -46,9 +46,9 @@ StageScope::~StageScope() {
 }
 
 SplitPlan make_split_plan(int batch, int L, int Hkv) {
-  // about 8 work items per SM so that a dynamically scheduled grid ends with a short tail
+  // about 6 work items per SM (and per sweep) so that a dynamically scheduled grid ends with a short tail
   const long heads = (long)batch * Hkv;
-  const long items_target = 8L * kNumSMs;
+  const long items_target = 6L * kNumSMs;
   long per_head = (items_target + heads - 1) / heads;
   if (per_head < 1) per_head = 1;
   long chunk = ((long)L + per_head - 1) / per_head;
@@ -67,7 +67,7 @@ Workspace carve_workspace(void* base, int batch, int L, int Hq, int Hkv, int P) 
   size_t off = 0;
   char* b = static_cast<char*>(base);
   Workspace ws;
-  ws.part = reinterpret_cast<float2*>(b + off); off = align_up(off + n_rows * sp.n_chunks * sizeof(float2), 256);
+  ws.part = reinterpret_cast<float2*>(b + off); off = align_up(off + n_rows * sp.n_chunks * 2 * sizeof(float2), 256);  // x2: one partial per epilogue warpgroup (score_tc.cu)
   ws.lse = reinterpret_cast<float*>(b + off);   off = align_up(off + n_rows * sizeof(float), 256);
   ws.imp = reinterpret_cast<float*>(b + off);   off = align_up(off + n_imp * sizeof(float), 256);
   ws.key = reinterpret_cast<uint32_t*>(b + off); off = align_up(off + n_imp * sizeof(uint32_t), 256);

@@ -21,7 +21,7 @@ constexpr int GT = 256;  // threads per block
 constexpr int GU = 4;    // vectors of K and of V in flight per thread
 
 // vpr = 16-byte vectors per row; n_vec = n_prob * C * vpr output vectors per tensor
-__global__ void __launch_bounds__(GT) gather_kernel(const int4* __restrict__ K, const int4* __restrict__ V,
+__global__ void __launch_bounds__(GT) nacl_gather_kernel(const int4* __restrict__ K, const int4* __restrict__ V,
                                                      const int32_t* __restrict__ idx, int L, int C, int vpr,
                                                      size_t n_vec, int4* __restrict__ oK, int4* __restrict__ oV) {
   const size_t stride = (size_t)gridDim.x * GT;
@@ -64,7 +64,7 @@ cudaError_t launch_gather(const void* K, const void* V, const int32_t* idx, int 
   size_t want = (n_vec + (size_t)GT * GU - 1) / ((size_t)GT * GU);
   const size_t cap = (size_t)kNumSMs * 8 * 4;  // a few waves of 8 resident CTAs per SM
   int blocks = (int)(want < cap ? want : cap);
-  gather_kernel<<<blocks, GT, 0, st>>>((const int4*)K, (const int4*)V, idx, L, C, vpr, n_vec, (int4*)out_K, (int4*)out_V);
+  nacl_gather_kernel<<<blocks, GT, 0, st>>>((const int4*)K, (const int4*)V, idx, L, C, vpr, n_vec, (int4*)out_K, (int4*)out_V);
   return cudaGetLastError();
 }
 

@@ -51,7 +51,7 @@ __device__ __forceinline__ size_t row_id(int b, int hk, int gr, int G, int P, in
 }
 
 template <typename T>
-__global__ void __launch_bounds__(NT) stats_kernel(const T* __restrict__ K, const T* __restrict__ Q, float2* __restrict__ part,
+__global__ void __launch_bounds__(NT) nacl_stats_kernel(const T* __restrict__ K, const T* __restrict__ Q, float2* __restrict__ part,
                                                     int L, int Hq, int Hkv, int d, int P, int G, int chunk, int n_chunks,
                                                     float inv_sqrt_d) {
   extern __shared__ float smem[];
@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(NT) stats_kernel(const T* __restrict__ K, cons
   }
 }
 
-__global__ void combine_kernel(const float2* __restrict__ part, float* __restrict__ lse, float* __restrict__ lse_out,
+__global__ void nacl_combine_kernel(const float2* __restrict__ part, float* __restrict__ lse, float* __restrict__ lse_out,
                                int n_rows, int n_chunks) {
   int row = blockIdx.x * blockDim.x + threadIdx.x;
   if (row >= n_rows) return;
@@ -113,7 +113,7 @@ __global__ void combine_kernel(const float2* __restrict__ part, float* __restric
 }
 
 template <typename T>
-__global__ void __launch_bounds__(NT) colsum_kernel(const T* __restrict__ K, const T* __restrict__ Q, const float* __restrict__ lse,
+__global__ void __launch_bounds__(NT) nacl_colsum_kernel(const T* __restrict__ K, const T* __restrict__ Q, const float* __restrict__ lse,
                                                      float* __restrict__ imp, float* __restrict__ imp_out,
                                                      int L, int Hq, int Hkv, int d, int P, int G, float inv_sqrt_d) {
   extern __shared__ float smem[];
@@ -163,26 +163,26 @@ cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const Spl
                          float* imp_out, float* lse_out, cudaStream_t st) {
   const size_t smem = (size_t)2 * 64 * (s.d + 1) * sizeof(float);
   cudaError_t e;
-  if ((e = cudaFuncSetAttribute(stats_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(colsum_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(nacl_stats_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(nacl_colsum_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
   const float inv_sqrt_d = 1.0f / sqrtf((float)s.d);
   dim3 g1(sp.n_chunks, s.Hkv, s.batch);
   {
     StageScope sc(ST_STATS, st);
-    stats_kernel<T><<<g1, NT, smem, st>>>((const T*)K, (const T*)Q, ws.part, s.L, s.Hq, s.Hkv, s.d, s.P, s.G, sp.chunk,
+    nacl_stats_kernel<T><<<g1, NT, smem, st>>>((const T*)K, (const T*)Q, ws.part, s.L, s.Hq, s.Hkv, s.d, s.P, s.G, sp.chunk,
                                           sp.n_chunks, inv_sqrt_d);
   }
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   const int n_rows = s.batch * s.Hq * s.P;
   {
     StageScope sc(ST_COMBINE, st);
-    combine_kernel<<<(n_rows + 127) / 128, 128, 0, st>>>(ws.part, ws.lse, lse_out, n_rows, sp.n_chunks);
+    nacl_combine_kernel<<<(n_rows + 127) / 128, 128, 0, st>>>(ws.part, ws.lse, lse_out, n_rows, sp.n_chunks);
   }
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   dim3 g2((s.L + TK - 1) / TK, s.Hkv, s.batch);
   {
     StageScope sc(ST_COLSUM, st);
-    colsum_kernel<T><<<g2, NT, smem, st>>>((const T*)K, (const T*)Q, ws.lse, ws.imp, imp_out, s.L, s.Hq, s.Hkv, s.d, s.P,
+    nacl_colsum_kernel<T><<<g2, NT, smem, st>>>((const T*)K, (const T*)Q, ws.lse, ws.imp, imp_out, s.L, s.Hq, s.Hkv, s.d, s.P,
                                            s.G, inv_sqrt_d);
   }
   return cudaGetLastError();

@@ -1,9 +1,9 @@
 // select.cu -- steps a4-a6 of SURVEY.md section 8: protected set, Proxy-Tokens top-k, Random
 // Eviction as Gumbel-top-k, and the ascending kept-position list.
 //
-//   keys_kernel  : key[j] = ordermap(fl32(ln w_j - ln(-ln u_j))),  u_j from Philox4x32-10 keyed by
+//   nacl_keys_kernel  : key[j] = ordermap(fl32(ln w_j - ln(-ln u_j))),  u_j from Philox4x32-10 keyed by
 //                  (seed; layer, batch, kv head, position)                PAPER.md:148-161, 37; R4/R5/R10/R15
-//   select_kernel: one CTA per (batch, kv head).  MSB radix select (12+10+10 bits) of the
+//   nacl_select_kernel: one CTA per (batch, kv head).  MSB radix select (12+10+10 bits) of the
 //                  (budget_proxy - |Pi|) largest importances outside Pi, a second
 //                  radix select of the budget_random largest keys among the rest, ties to the lower
 //                  index in both (R9), then an order-preserving compaction that emits the
@@ -38,7 +38,7 @@ __device__ __forceinline__ uint32_t ordermap(uint32_t bits) {
   return (bits & 0x80000000u) ? ~bits : (bits | 0x80000000u);
 }
 
-__global__ void __launch_bounds__(256) keys_kernel(const float* __restrict__ imp, uint32_t* __restrict__ key,
+__global__ void __launch_bounds__(256) nacl_keys_kernel(const float* __restrict__ imp, uint32_t* __restrict__ key,
                                                     int Hkv, int L, uint32_t k0, uint32_t k1, uint32_t layer, uint32_t flags) {
   const int p = blockIdx.y;  // b * Hkv + hk
   const int b = p / Hkv, hk = p - b * Hkv;
@@ -167,7 +167,7 @@ __device__ void block_radix_select(F getval, int lo, int hi, int K, SelShared& s
   cut = result;
 }
 
-__global__ void __launch_bounds__(ST) select_kernel(const float* __restrict__ imp, const uint32_t* __restrict__ key, int L,
+__global__ void __launch_bounds__(ST) nacl_select_kernel(const float* __restrict__ imp, const uint32_t* __restrict__ key, int L,
                                                      int k1, int Br, int n_sink, int n_recent, int C,
                                                      int32_t* __restrict__ out_idx) {
   __shared__ SelShared sh;
@@ -218,7 +218,7 @@ __global__ void __launch_bounds__(ST) select_kernel(const float* __restrict__ im
 cudaError_t launch_keys(const float* imp, uint32_t* key, int batch, int Hkv, int L, uint64_t seed, int layer,
                         uint32_t flags, cudaStream_t st) {
   dim3 grid((L + 255) / 256, batch * Hkv);
-  keys_kernel<<<grid, 256, 0, st>>>(imp, key, Hkv, L, (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32),
+  nacl_keys_kernel<<<grid, 256, 0, st>>>(imp, key, Hkv, L, (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32),
                                     (uint32_t)layer, flags);
   return cudaGetLastError();
 }
@@ -228,7 +228,7 @@ cudaError_t launch_select(const float* imp, const uint32_t* key, int batch, int 
   const int C = budget_proxy + budget_random;
   if (C == 0) return cudaSuccess;
   const int k1 = budget_proxy - n_sink - n_recent;
-  select_kernel<<<batch * Hkv, ST, 0, st>>>(imp, key, L, k1, budget_random, n_sink, n_recent, C, out_idx);
+  nacl_select_kernel<<<batch * Hkv, ST, 0, st>>>(imp, key, L, k1, budget_random, n_sink, n_recent, C, out_idx);
   return cudaGetLastError();
 }
 

@@ -822,10 +822,11 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
 }
 
 
+}  // namespace nacl
+
 #ifdef NACL_TC_TRACE
-int debug_trace_read(long long* host, size_t bytes) {
-  return (int)cudaMemcpyFromSymbol(host, g_trace, bytes < sizeof(g_trace) ? bytes : sizeof(g_trace));
+// diagnostics build only: per-warp wait/compute cycle counters of the last launch
+extern "C" __attribute__((visibility("default"))) int nacl_debug_trace_read(long long* host, size_t bytes) {
+  return (int)cudaMemcpyFromSymbol(host, nacl::g_trace, bytes < sizeof(nacl::g_trace) ? bytes : sizeof(nacl::g_trace));
 }
 #endif
-
-}  // namespace nacl

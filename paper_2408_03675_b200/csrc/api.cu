@@ -67,7 +67,10 @@ Workspace carve_workspace(void* base, int batch, int L, int Hq, int Hkv, int P) 
   size_t off = 0;
   char* b = static_cast<char*>(base);
   Workspace ws;
-  ws.part = reinterpret_cast<float2*>(b + off); off = align_up(off + n_rows * sp.n_chunks * 2 * sizeof(float2), 256);  // x2: one partial per epilogue warpgroup (score_tc.cu)
+  size_t n_part = n_rows * sp.n_chunks;  // generic path; the tensor-core path keeps one partial per (CTA + head, warpgroup, row)
+  const size_t n_part_tc = score_tc_part_elems(batch * Hkv, (Hq / Hkv) * P);
+  if (n_part_tc > n_part) n_part = n_part_tc;
+  ws.part = reinterpret_cast<float2*>(b + off); off = align_up(off + n_part * sizeof(float2), 256);
   ws.lse = reinterpret_cast<float*>(b + off);   off = align_up(off + n_rows * sizeof(float), 256);
   ws.imp = reinterpret_cast<float*>(b + off);   off = align_up(off + n_imp * sizeof(float), 256);
   ws.key = reinterpret_cast<uint32_t*>(b + off); off = align_up(off + n_imp * sizeof(uint32_t), 256);

@@ -31,11 +31,12 @@ SplitPlan make_split_plan(int batch, int L, int Hkv);
 
 // Workspace carve-up (all offsets 256-byte aligned).
 struct Workspace {
-  float2* part;        // [batch*Hq*P, n_chunks]  (m, Z) partial softmax statistics per row and chunk
+  float2* part;        // partial softmax statistics (m, Z): generic path [batch*Hq*P, n_chunks]; tensor-core path
+                       // [148 + heads, n_slots, G*P] (score_tc.cu)
   float* lse;          // [batch*Hq*P]            natural-log LSE of every proxy row
   float* imp;          // [batch*Hkv, L]          importance F_score
   uint32_t* key;       // [batch*Hkv, L]          order-mapped fp32 Gumbel-top-k keys
-  int* sync;           // [sync_ints(heads)]      ticket + per-head counters / flags of the persistent tensor-core kernel (zeroed per call)
+  int* sync;           // [sync_ints(heads)]      reserved (counters / flags for future fused variants)
   size_t bytes;
 };
 inline size_t sync_ints(size_t heads) { return 16 + 2 * heads; }
@@ -62,6 +63,7 @@ cudaError_t launch_score_generic(const Shape& s, const void* K, const void* Q, c
 // tensor-core scoring (bf16, d == 128, G*P % 16 == 0, G*P <= 256): tcgen05 + TMA
 bool score_tc_supported(const Shape& s);
 int score_tc_launch_count(const Shape& s);
+size_t score_tc_part_elems(int heads, int rows);  // float2 elements of Workspace::part the tensor-core path needs
 cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const SplitPlan& sp,
                             const Workspace& ws, float* imp_out, float* lse_out, cudaStream_t st);
 

@@ -22,18 +22,22 @@
 // No floating-point atomics with more than two addends anywhere: all sums have a fixed order.
 //
 // Two MMA orientations share the same shared-memory operands (both K-major, 128B swizzle):
-//   S tiles:  D[row, key] = Q_half (M=128 proxy rows) x K_tile^T (N=128 keys)   -> a thread owns a
-//             proxy row, its running (max, sum-exp) live in two registers;
-//   C tiles:  D[key, row] = K_tile (M=128 keys) x Q^T (N = G*P proxy rows)       -> a thread owns a
-//             key, its column sum is a private register, no cross-thread reduction.
+//   S tiles:  D[row, key] = Q_half (M=128 proxy rows) x K_tile^T (N=128 keys), one MMA group per
+//             128-row half -> a thread owns a proxy row and a range of key columns; its running
+//             (max, sum-exp) live in two registers;
+//   C tiles:  D[key, row] = K_tile (M=128 keys) x Q^T (N = G*P proxy rows) -> a thread owns a key
+//             and a quarter of the proxy rows; the four quarter sums of a key meet in shared memory
+//             and a combiner warp adds them in a fixed order (deterministic) and stores imp.
 //
-// Epilogue arithmetic.  At G*P = 256 the path is bound by the 16/clk/SM MUFU.EX2 unit, not by HBM
-// (profiles/): half of the exponentials are therefore evaluated on the FMA pipe (Cody-Waite range
-// reduction + degree-3 minimax polynomial, relative error <= 7.5e-5, against the 2e-3 score
-// tolerance of the north star) and all multiply-adds are the packed fma/add.f32x2 forms.
+// Epilogue arithmetic.  At G*P = 256 the path is bound by the 16/clk/SM MUFU.EX2 unit and the FMA
+// pipe, not by HBM (profiles/): half of the exponentials are therefore evaluated on the FMA pipe
+// (Cody-Waite range reduction + degree-3 minimax polynomial, relative error <= 7.5e-5, against the
+// 2e-3 score tolerance of the north star) and all multiply-adds are the packed fma/add.f32x2 forms.
 //
-// Warp roles (352 threads, 1 CTA per SM): warps 0-7 = two epilogue warpgroups (warp%4 = TMEM lane
-// quarter), warp 8 = TMA producer, warps 9-10 = tcgen05.mma issuers (one per epilogue warpgroup).
+// Warp roles (608 threads, 1 CTA per SM): warps 0-15 = epilogue (warp%4 = TMEM lane quarter = SM
+// sub-partition, warp/4 = column quarter of the tile), warp 16 = TMA producer, warp 17 = TMEM
+// allocator + tcgen05.mma issuer, warp 18 = column-sum combiner.  All 16 epilogue warps work on
+// the same tile; two 256-column TMEM buffers let the MMA of tile t+1 run under the epilogue of t.
 #include <cuda.h>
 
 #include "nacl_internal.cuh"
@@ -45,20 +49,38 @@ constexpr int TILE = 128;                      // keys per tile
 constexpr int HD = 128;                        // head dim served by this path
 constexpr int BOX_BYTES = 128 * 128;           // one TMA box: 128 rows x 64 bf16 (128 B, swizzled)
 constexpr int KSTAGE_BYTES = 2 * BOX_BYTES;    // a K tile = two boxes (d 0..63, d 64..127)
-constexpr int N_EPI_WARPS = 8;
+constexpr int N_EPI_WARPS = 16;
 constexpr int EPI_THREADS = N_EPI_WARPS * 32;
-constexpr int W_TMA = 8, W_MMA = 9;            // warp roles after the 8 epilogue warps: TMA, MMA issuers 9 and 10
+constexpr int W_TMA = 16, W_MMA = 17, W_CMB = 18;  // warp roles after the epilogue warps
 constexpr int NTHREADS = EPI_THREADS + 3 * 32;
 constexpr int TMEM_COLS = 512;
-constexpr int N_BUFS = 4;                      // TMEM accumulator buffers, two per epilogue warpgroup
-constexpr int BUF_COLS = 128;                  // TMEM columns per accumulator buffer
+constexpr int N_BUFS = 2;                      // TMEM accumulator buffers (one tile each)
+constexpr int BUF_COLS = 256;                  // TMEM columns per accumulator buffer
+constexpr int N_CS = 4;                        // shared-memory buffers for the quarter column sums of a C tile
 constexpr int MAX_GRID = kNumSMs;              // the partial-statistics workspace is sized for this many CTAs
 constexpr uint32_t SPIN_LIMIT = 1u << 26;      // watchdog: a wait that long is a bug -> trap (loud failure)
-constexpr uint32_t POLY_MASK = 0xAAu;          // which of every 8 element pairs take the FMA-pipe exp2 (bit e&7)
+#ifndef NACL_POLY_MASK
+#define NACL_POLY_MASK 0x2Au
+#endif
+constexpr uint32_t POLY_MASK = NACL_POLY_MASK;  // which of every 8 element pairs take the FMA-pipe exp2 (bit e&7)
+
+// Optional wait/compute cycle accounting per warp role (diagnostics build only: -DNACL_TC_TRACE).
+#ifdef NACL_TC_TRACE
+#define TR_N 8
+__device__ long long g_trace[2][160][19][TR_N];
+__device__ __forceinline__ long long gtimer_ns() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define TR_DECL long long tr_[TR_N]; for (int i_ = 0; i_ < TR_N; ++i_) tr_[i_] = 0; const long long tr_start_ = clock64(); const long long tr_ns_ = gtimer_ns();
+#define TRW(cat, ...) { const long long t_ = clock64(); __VA_ARGS__; tr_[cat] += clock64() - t_; }
+#define TR_FLUSH() { tr_[TR_N - 1] = clock64() - tr_start_; tr_[TR_N - 2] = gtimer_ns() - tr_ns_; if (lane == 0 && blockIdx.x < 160) for (int i_ = 0; i_ < TR_N; ++i_) g_trace[p.phase][blockIdx.x][warp][i_] = tr_[i_]; }
+#else
+#define TR_DECL
+#define TRW(cat, ...) { __VA_ARGS__; }
+#define TR_FLUSH()
+#endif
 
 struct TcParams {
   int L, rows, T;          // keys per head, proxy rows per kv head (G*P), key tiles per head
-  int heads, n_slots;      // n_slots: partials per (row, piece): 2 when both warpgroups see every proxy row (rows <= 128), else 1
+  int heads, n_slots;      // n_slots: epilogue warps that share a proxy row in sweep S = partials per (row, piece): 2 if rows > 128, else 4
   int phase;               // 0 = sweep S (statistics), 1 = sweep C (column sums)
   long long N;             // heads * T
   float scale_log2;        // log2(e) / sqrt(d)
@@ -108,6 +130,14 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm,
                : "memory");
 }
 
+// one lane of the (converged) warp; the role loops run warp-wide so that addresses and descriptors stay in
+// uniform registers, and only the TMA / MMA / commit instructions themselves are issued by the elected lane
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
@@ -115,6 +145,9 @@ __device__ __forceinline__ void tc_commit(uint32_t bar) {
 }
 // D[tmem] (+)= A[smem] * B[smem]^T, bf16 inputs, fp32 accumulate; issued by ONE thread
 __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+#ifdef NACL_DIAG_NO_MMA
+  return;
+#endif
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
       "setp.ne.b32 p, %4, 0;\n\t"
@@ -154,6 +187,19 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[32]) {
         "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
       : "r"(taddr)
       : "memory");
+}
+
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+               : "r"(taddr)
+               : "memory");
+}
+__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3])
+               : "r"(taddr)
+               : "memory");
 }
 
 __device__ __forceinline__ float fast_exp2(float x) {
@@ -269,8 +315,9 @@ struct Smem {
   static constexpr int OFF_Q = 0;
   static constexpr int OFF_K = OFF_Q + NQ * Q_BYTES;
   static constexpr int OFF_LSE = OFF_K + STAGES * KSTAGE_BYTES;   // float[LSE_SLOTS][256]: -lse (log2 domain) of the segment's head
-  static constexpr int OFF_BARS = OFF_LSE + LSE_SLOTS * 256 * 4;
-  static constexpr int N_BARS = 2 * STAGES + 2 * NQ + 2 * N_BUFS;
+  static constexpr int OFF_CS = OFF_LSE + LSE_SLOTS * 256 * 4;    // float[N_CS][4][128]: quarter column sums of a C tile
+  static constexpr int OFF_BARS = OFF_CS + N_CS * 4 * TILE * 4;
+  static constexpr int N_BARS = 2 * STAGES + 2 * NQ + 2 * N_BUFS + 2 * N_CS;
   static constexpr int OFF_TMEM = OFF_BARS + N_BARS * 8;
   static constexpr int TOTAL = OFF_TMEM + 8;
 };
@@ -278,6 +325,13 @@ struct Smem {
 // ------------------------------------------------------------------ epilogue helpers
 // one 32-column segment of an S tile: online (max, sum-exp) update of the row this thread owns
 __device__ __forceinline__ void s_update(const uint32_t (&v)[32], float sc, float& m, float& z) {
+#ifdef NACL_EPI_TRIVIAL  // diagnostics: pipeline ceiling without the exponentials (results are wrong)
+  float t0 = 0.f;
+#pragma unroll
+  for (int e = 0; e < 32; ++e) t0 += __uint_as_float(v[e]);
+  z += t0 * sc; m = 0.f;
+  return;
+#endif
   float g0 = __uint_as_float(v[0]), g1 = __uint_as_float(v[1]);
 #pragma unroll
   for (int e = 2; e < 30; e += 4) {
@@ -300,29 +354,26 @@ __device__ __forceinline__ void s_update(const uint32_t (&v)[32], float sc, floa
   m = m_new;
 }
 
-// S tile (128 proxy rows x 128 keys): the TMEM loads of segment s+1 are in flight while segment s is reduced
-__device__ __forceinline__ void s_tile(uint32_t tbuf, float sc, float& m, float& z) {
+// S tile, this warp's share: NC (32 or 64) key columns of the 32 proxy rows (TMEM lanes) it owns
+template <int NC>
+__device__ __forceinline__ void s_cols(uint32_t taddr, float sc, float& m, float& z) {
   uint32_t va[32], vb[32];
-  tmem_ld32(tbuf, va);
+  tmem_ld32(taddr, va);
+  if (NC == 64) tmem_ld32(taddr + 32, vb);
   tc_wait_ld(va);
-  tmem_ld32(tbuf + 32, vb);
   s_update(va, sc, m, z);
-  tc_wait_ld(vb);
-  tmem_ld32(tbuf + 64, va);
-  s_update(vb, sc, m, z);
-  tc_wait_ld(va);
-  tmem_ld32(tbuf + 96, vb);
-  s_update(va, sc, m, z);
-  tc_wait_ld(vb);
-  s_update(vb, sc, m, z);
+  if (NC == 64) {
+    tc_wait_ld(vb);
+    s_update(vb, sc, m, z);
+  }
 }
 
-// last tile of a head: columns >= valid are keys past L and must not exist (-inf)
-__device__ __forceinline__ void s_tile_masked(uint32_t tbuf, float sc, int valid, float& m, float& z) {
+// last tile of a head: columns >= valid (relative to taddr) are keys past L and must not exist (-inf)
+__device__ __forceinline__ void s_cols_masked(uint32_t taddr, int nc, float sc, int valid, float& m, float& z) {
   uint32_t v[32];
 #pragma unroll 1
-  for (int c = 0; c < valid; c += 32) {
-    tmem_ld32(tbuf + c, v);
+  for (int c = 0; c < nc && c < valid; c += 32) {
+    tmem_ld32(taddr + c, v);
     tc_wait_ld(v);
 #pragma unroll
     for (int e = 0; e < 32; ++e)
@@ -336,6 +387,14 @@ template <int N4>
 __device__ __forceinline__ void c_update(const uint32_t (&v)[32], float sc, const float* nl, u64& a0, u64& a1) {
   const ulonglong2* l2 = reinterpret_cast<const ulonglong2*>(nl);
   const u64 sc2 = pack2(sc, sc);
+#ifdef NACL_EPI_TRIVIAL
+#pragma unroll
+  for (int e = 0; e < N4; ++e) {
+    a0 = add2(a0, pack2u(v[4 * e + 0], v[4 * e + 1]));
+    a1 = add2(a1, pack2u(v[4 * e + 2], v[4 * e + 3]));
+  }
+  return;
+#endif
 #pragma unroll
   for (int e = 0; e < N4; ++e) {
     const ulonglong2 l = l2[e];
@@ -346,27 +405,24 @@ __device__ __forceinline__ void c_update(const uint32_t (&v)[32], float sc, cons
   }
 }
 
-// C tile: this thread owns one key; sum over the proxy rows (TMEM columns) of exp2(s*sc - lse2[row])
-__device__ __forceinline__ float c_tile(uint32_t tbuf, int rows, float sc, const float* nl) {
+// C tile, this warp's share: the key this thread owns, summed over nc proxy rows (TMEM columns from taddr on;
+// nc a multiple of 4, <= 64) of exp2(s*sc - lse2[row]); nl = -lse2 of those rows
+__device__ __forceinline__ float c_cols(uint32_t taddr, int nc, float sc, const float* nl) {
   u64 a0 = 0ull, a1 = 0ull;
-  const int nseg = rows >> 5;
   uint32_t va[32], vb[32];
-  if (nseg > 0) tmem_ld32(tbuf, va);
-#pragma unroll 1
-  for (int s = 0; s < nseg; s += 2) {
+  if (nc == 64) {
+    tmem_ld32(taddr, va);
+    tmem_ld32(taddr + 32, vb);
     tc_wait_ld(va);
-    if (s + 1 < nseg) tmem_ld32(tbuf + (s + 1) * 32, vb);
-    c_update<8>(va, sc, nl + s * 32, a0, a1);
-    if (s + 1 < nseg) {
-      tc_wait_ld(vb);
-      if (s + 2 < nseg) tmem_ld32(tbuf + (s + 2) * 32, va);
-      c_update<8>(vb, sc, nl + (s + 1) * 32, a0, a1);
-    }
-  }
-  if (rows & 16) {
-    tmem_ld16(tbuf + nseg * 32, va);
-    tc_wait_ld(va);
-    c_update<4>(va, sc, nl + nseg * 32, a0, a1);
+    c_update<8>(va, sc, nl, a0, a1);
+    tc_wait_ld(vb);
+    c_update<8>(vb, sc, nl + 32, a0, a1);
+  } else {
+    int c = 0;
+    if (nc & 32) { tmem_ld32(taddr, va); tc_wait_ld(va); c_update<8>(va, sc, nl, a0, a1); c = 32; }
+    if (nc & 16) { tmem_ld16(taddr + c, va); tc_wait_ld(va); c_update<4>(va, sc, nl + c, a0, a1); c += 16; }
+    if (nc & 8) { tmem_ld8(taddr + c, va); tc_wait_ld(va); c_update<2>(va, sc, nl + c, a0, a1); c += 8; }
+    if (nc & 4) { tmem_ld4(taddr + c, va); tc_wait_ld(va); c_update<1>(va, sc, nl + c, a0, a1); }
   }
   float s0, s1;
   unpack2(add2(a0, a1), s0, s1);
@@ -383,24 +439,30 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
   if ((sbase & 1023u) != 0) __trap();  // the 128B-swizzled operand tiles need 1024-byte alignment
 
   const uint32_t bars = sbase + SM::OFF_BARS;
-  constexpr int B_KE = STAGES, B_QF = 2 * STAGES, B_QE = B_QF + NQ, B_TF = B_QE + NQ, B_TE = B_TF + N_BUFS;
-  static_assert(B_TE + N_BUFS == SM::N_BARS, "barrier count");
+  constexpr int B_KE = STAGES, B_QF = 2 * STAGES, B_QE = B_QF + NQ, B_TF = B_QE + NQ, B_TE = B_TF + N_BUFS, B_CF = B_TE + N_BUFS,
+                B_CE = B_CF + N_CS;
+  static_assert(B_CE + N_CS == SM::N_BARS, "barrier count");
   auto k_full = [&](int s) { return bars + 8u * s; };
   auto k_empty = [&](int s) { return bars + 8u * (B_KE + s); };
   auto q_full = [&](int s) { return bars + 8u * (B_QF + s); };
   auto q_empty = [&](int s) { return bars + 8u * (B_QE + s); };
   auto tm_full = [&](int b) { return bars + 8u * (B_TF + b); };
   auto tm_empty = [&](int b) { return bars + 8u * (B_TE + b); };
+  auto cs_full = [&](int b) { return bars + 8u * (B_CF + b); };
+  auto cs_empty = [&](int b) { return bars + 8u * (B_CE + b); };
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + SM::OFF_TMEM);
   float* nlse_s = reinterpret_cast<float*>(smem + SM::OFF_LSE);
+  float* cs_s = reinterpret_cast<float*>(smem + SM::OFF_CS);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const bool modeB = p.rows > 128;
+  const int n_half = p.rows > 128 ? 2 : 1;  // 128-row MMA groups of an S tile
+  TR_DECL
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < STAGES; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), modeB ? 2 : 1); }  // issuers that read a stage
-    for (int s = 0; s < NQ; ++s) { mbar_init(q_full(s), 1); mbar_init(q_empty(s), 2); }
-    for (int b = 0; b < N_BUFS; ++b) { mbar_init(tm_full(b), 1); mbar_init(tm_empty(b), 4); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
+    for (int s = 0; s < NQ; ++s) { mbar_init(q_full(s), 1); mbar_init(q_empty(s), 1); }
+    for (int b = 0; b < N_BUFS; ++b) { mbar_init(tm_full(b), 1); mbar_init(tm_empty(b), N_EPI_WARPS); }
+    for (int b = 0; b < N_CS; ++b) { mbar_init(cs_full(b), N_EPI_WARPS); mbar_init(cs_empty(b), 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == W_MMA) {
@@ -414,124 +476,158 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
 
   if (warp == W_TMA) {
     // ================================================================ TMA producer
-    if (lane == 0) {
-      int stage = 0, qrun = 0;
-      uint32_t kphase = 0;
-      Walk walk(p);
-      Seg sg;
-      while (walk.next(sg)) {
-        const int qb = qrun % NQ;
-        mbar_wait(q_empty(qb), ((qrun / NQ) & 1) ^ 1);
+    int stage = 0, qrun = 0;
+    uint32_t kphase = 0;
+    Walk walk(p);
+    Seg sg;
+    while (walk.next(sg)) {
+      const int qb = qrun % NQ;
+      TRW(1, mbar_wait(q_empty(qb), ((qrun / NQ) & 1) ^ 1));
+      const uint32_t qdst = sbase + SM::OFF_Q + qb * SM::Q_BYTES;
+      if (elect_one()) {
         mbar_expect_tx(q_full(qb), SM::Q_BYTES);
-        const uint32_t qdst = sbase + SM::OFF_Q + qb * SM::Q_BYTES;
         tma_load_2d(qdst, &tmQ, 0, sg.head * p.rows, q_full(qb));
         tma_load_2d(qdst + QROWS * 128, &tmQ, 64, sg.head * p.rows, q_full(qb));
-        ++qrun;
-        for (int i = 0; i < sg.n; ++i) {
-          mbar_wait(k_empty(stage), kphase ^ 1);
+      }
+      ++qrun;
+      for (int i = 0; i < sg.n; ++i) {
+        TRW(0, mbar_wait(k_empty(stage), kphase ^ 1));
+        const uint32_t kdst = sbase + SM::OFF_K + stage * KSTAGE_BYTES;
+        const int j0 = (sg.tile + walk.step * i) * TILE;
+        if (elect_one()) {
           mbar_expect_tx(k_full(stage), KSTAGE_BYTES);
-          const uint32_t kdst = sbase + SM::OFF_K + stage * KSTAGE_BYTES;
-          const int j0 = (sg.tile + walk.step * i) * TILE;
           tma_load_3d(kdst, &tmK, 0, j0, sg.head, k_full(stage));
           tma_load_3d(kdst + BOX_BYTES, &tmK, 64, j0, sg.head, k_full(stage));
-          if (++stage == STAGES) { stage = 0; kphase ^= 1; }
         }
+        if (++stage == STAGES) { stage = 0; kphase ^= 1; }
       }
     }
     __syncwarp();
-  } else if (warp == W_MMA || warp == W_MMA + 1) {
-    // ================================================================ tcgen05.mma issuer of epilogue warpgroup w
-    if (lane == 0) {
-      const int w = warp - W_MMA;
-      int stage = 0, qrun = 0;
-      uint32_t kphase = 0, tcount = 0;
-      const uint32_t idesc = p.phase == 0 ? umma_idesc(128, TILE) : umma_idesc(128, modeB ? min(128, p.rows - 128 * w) : p.rows);
+  } else if (warp == W_MMA) {
+    // ================================================================ tcgen05.mma issuer
+    int stage = 0, qrun = 0;
+    uint32_t kphase = 0, tcount = 0;
+    const uint32_t idesc = p.phase == 0 ? umma_idesc(128, TILE) : umma_idesc(128, p.rows);
+    Walk walk(p);
+    Seg sg;
+    while (walk.next(sg)) {
+      const int qb = qrun % NQ;
+      TRW(2, mbar_wait(q_full(qb), (qrun / NQ) & 1));
+      const uint32_t qsrc = sbase + SM::OFF_Q + qb * SM::Q_BYTES;
+      ++qrun;
+      for (int i = 0; i < sg.n; ++i) {
+        const uint32_t buf = tcount & 1, par = (tcount >> 1) & 1;
+        TRW(0, mbar_wait(k_full(stage), kphase));
+        TRW(1, mbar_wait(tm_empty(buf), par ^ 1));
+        tc_fence_after();
+        const uint32_t ksrc = sbase + SM::OFF_K + stage * KSTAGE_BYTES;
+        const uint32_t dcol = tmem_base + buf * BUF_COLS;
+        if (elect_one()) {
+          if (p.phase == 0) {
+            for (int h = 0; h < n_half; ++h) {  // proxy rows [128h, 128h+128): 128 rows x 128 B further down in each Q box
+#pragma unroll
+              for (int k = 0; k < 8; ++k) {
+                const uint32_t ko = (k >> 2) * BOX_BYTES + (k & 3) * 32;
+                const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32 + h * BOX_BYTES;
+                tc_mma(dcol + h * 128, umma_desc(qsrc + qo), umma_desc(ksrc + ko), idesc, k > 0);
+              }
+            }
+          } else {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+              const uint32_t ko = (k >> 2) * BOX_BYTES + (k & 3) * 32;
+              const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32;
+              tc_mma(dcol, umma_desc(ksrc + ko), umma_desc(qsrc + qo), idesc, k > 0);
+            }
+          }
+          tc_commit(tm_full(buf));    // the accumulator buffer is complete
+          tc_commit(k_empty(stage));  // the reads of the stage are done once these MMAs complete
+          if (i == sg.n - 1) tc_commit(q_empty(qb));  // every MMA that read the segment's Q has completed
+        }
+        __syncwarp();
+        ++tcount;
+        if (++stage == STAGES) { stage = 0; kphase ^= 1; }
+      }
+    }
+    __syncwarp();
+  } else if (warp == W_CMB) {
+    // ================================================================ column-sum combiner (sweep C only)
+    if (p.phase != 0) {
+      uint32_t ccount = 0;
       Walk walk(p);
       Seg sg;
       while (walk.next(sg)) {
-        const int qb = qrun % NQ;
-        mbar_wait(q_full(qb), (qrun / NQ) & 1);
-        const uint32_t qsrc = sbase + SM::OFF_Q + qb * SM::Q_BYTES;
-        ++qrun;
-        for (int i = 0; i < sg.n; ++i) {
-          // rows <= 128: the tile goes to warpgroup (tcount & 1), all proxy rows.
-          // rows  > 128: the tile goes to both warpgroups, warpgroup w takes proxy rows [128w, 128w+128).
-          if (modeB || (int)(tcount & 1) == w) {
-            const uint32_t buf = 2 * w + (modeB ? (tcount & 1) : ((tcount >> 1) & 1));
-            const uint32_t par = (modeB ? (tcount >> 1) : (tcount >> 2)) & 1;
-            mbar_wait(k_full(stage), kphase);
-            mbar_wait(tm_empty(buf), par ^ 1);
-            tc_fence_after();
-            const uint32_t ksrc = sbase + SM::OFF_K + stage * KSTAGE_BYTES;
-            const uint32_t dcol = tmem_base + buf * BUF_COLS;
-            const uint32_t qrow = modeB ? w * BOX_BYTES : 0;  // 128 rows x 128 B further down in each Q box
-            if (p.phase == 0) {
+        for (int i = 0; i < sg.n; ++i, ++ccount) {
+          const int cb = ccount % N_CS;
+          TRW(0, mbar_wait(cs_full(cb), (ccount / N_CS) & 1));
+          const float* c = cs_s + cb * 4 * TILE;
+          float r[4];
 #pragma unroll
-              for (int k = 0; k < 8; ++k) {
-                const uint32_t ko = (k >> 2) * BOX_BYTES + (k & 3) * 32;
-                const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32 + qrow;
-                tc_mma(dcol, umma_desc(qsrc + qo), umma_desc(ksrc + ko), idesc, k > 0);
-              }
-            } else {
-#pragma unroll
-              for (int k = 0; k < 8; ++k) {
-                const uint32_t ko = (k >> 2) * BOX_BYTES + (k & 3) * 32;
-                const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32 + qrow;
-                tc_mma(dcol, umma_desc(ksrc + ko), umma_desc(qsrc + qo), idesc, k > 0);
-              }
-            }
-            tc_commit(tm_full(buf));    // the accumulator buffer is complete
-            tc_commit(k_empty(stage));  // this issuer's reads of the stage are done once these MMAs complete
+          for (int u = 0; u < 4; ++u) {
+            const int key = lane + 32 * u;
+            r[u] = (c[key] + c[TILE + key]) + (c[2 * TILE + key] + c[3 * TILE + key]);
           }
-          ++tcount;
-          if (++stage == STAGES) { stage = 0; kphase ^= 1; }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(cs_empty(cb));
+          const int j0 = (sg.tile - i) * TILE;
+          const size_t o = (size_t)sg.head * p.L + j0;
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int key = lane + 32 * u;
+            if (j0 + key < p.L) {
+              p.imp[o + key] = r[u];
+              if (p.imp_out) p.imp_out[o + key] = r[u];
+            }
+          }
         }
-        tc_commit(q_empty(qb));  // every MMA of this issuer that read the segment's Q has completed
       }
     }
-    __syncwarp();
   } else {
-    // ================================================================ epilogue warpgroups (independent of each other)
-    const int wg = warp >> 2, quarter = warp & 3;
-    const int lrow = quarter * 32 + lane;             // TMEM lane owned by this thread
+    // ================================================================ epilogue warps
+    const int quarter = warp & 3, cq = warp >> 2;       // TMEM lane quarter, column quarter of the tile
     const uint32_t tbase = tmem_base + ((uint32_t)(quarter * 32) << 16);
-    const int row0 = modeB ? 128 * wg : 0;            // first proxy row this warpgroup is responsible for
-    const int nrows_w = min(128, p.rows - row0);      // ... and how many
     const float sc = p.scale_log2;
-    const bool live = nrows_w > quarter * 32;         // S tiles: does this warp own a live proxy row?
     const long long G = gridDim.x;
-    uint32_t ecount = 0;  // tiles seen so far, same sequence as the MMA warps' tcount
+    // sweep S: this warp's proxy rows and key columns
+    const int s_half = n_half == 2 ? (cq >> 1) : 0;
+    const int s_slot = n_half == 2 ? (cq & 1) : cq;
+    const int s_nc = n_half == 2 ? 64 : 32;
+    const int s_col0 = s_slot * s_nc;
+    const int s_row = s_half * 128 + quarter * 32 + lane;
+    const bool live = s_half * 128 + quarter * 32 < p.rows;  // does this warp own a live proxy row?
+    // sweep C: this warp's proxy rows (columns)
+    const int c_nc = p.rows >> 2, c_col0 = cq * c_nc;
+    uint32_t ecount = 0;  // tiles seen so far, same sequence as the MMA warp's tcount
     int nseg = 0;
     Walk walk(p);
     Seg sg;
     while (walk.next(sg)) {
       if (p.phase == 0) {
-        // ---------------- S segment: running (max, sum-exp) of row lrow over this warpgroup's tiles
+        // ---------------- S segment: running (max, sum-exp) of row s_row over this warp's key columns
         float m0 = -INFINITY, z0 = 0.f;
         for (int i = 0; i < sg.n; ++i) {
-          const uint32_t g = ecount + i;
-          if (!modeB && (int)(g & 1) != wg) continue;
-          const uint32_t buf = 2 * wg + (modeB ? (g & 1) : ((g >> 1) & 1));
-          mbar_wait(tm_full(buf), (modeB ? (g >> 1) : (g >> 2)) & 1);
+          const uint32_t g = ecount + i, buf = g & 1;
+          TRW(0, mbar_wait(tm_full(buf), (g >> 1) & 1));
           tc_fence_after();
-          const int valid = p.L - (sg.tile + i) * TILE;
-          if (live) {
-            if (valid >= TILE) s_tile(tbase + buf * BUF_COLS, sc, m0, z0);
-            else s_tile_masked(tbase + buf * BUF_COLS, sc, valid, m0, z0);
-          }
+          const int valid = p.L - (sg.tile + i) * TILE - s_col0;
+          TRW(1, if (live) {
+            const uint32_t ta = tbase + buf * BUF_COLS + s_half * 128 + s_col0;
+            if (valid >= s_nc) { if (n_half == 2) s_cols<64>(ta, sc, m0, z0); else s_cols<32>(ta, sc, m0, z0); }
+            else s_cols_masked(ta, s_nc, sc, valid, m0, z0);
+          })
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(tm_empty(buf));
         }
-        // this warpgroup's partial of the piece; (-inf, 0) when it saw no tile
-        if (lrow < nrows_w)
-          __stcg(&p.part[(((size_t)blockIdx.x + sg.head) * p.n_slots + (modeB ? 0 : wg)) * p.rows + row0 + lrow], make_float2(m0, z0));
+        // this warp's partial of the piece; (-inf, 0) when it saw no valid key
+        if (s_row < p.rows)
+          __stcg(&p.part[(((size_t)blockIdx.x + sg.head) * p.n_slots + s_slot) * p.rows + s_row], make_float2(m0, z0));
       } else {
         // ---------------- C segment: merge the head's partials (ascending piece order) into -lse, then column sums
         const int ls = nseg % LSE_SLOTS;
         float* nl = nlse_s + ls * 256;
-        {
-          const int r = warp * 32 + lane;
+        TRW(2, {
+          const int r = threadIdx.x;
           if (r < p.rows) {
             const int c_first = cta_of_tile((long long)sg.head * p.T, p.N, G);
             const int c_last = cta_of_tile((long long)(sg.head + 1) * p.T - 1, p.N, G);
@@ -541,30 +637,22 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
             // the CTA that owns the head's first tile publishes lse
             if (p.lse_out && sg.tile - (sg.n - 1) == 0) p.lse_out[(size_t)sg.head * p.rows + r] = l2 * 0.69314718055994530942f;
           }
-        }
-        asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory");
+        })
+        TRW(3, asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory"));
         for (int i = 0; i < sg.n; ++i) {
-          const uint32_t g = ecount + i;
-          if (!modeB && (int)(g & 1) != wg) continue;
-          const uint32_t buf = 2 * wg + (modeB ? (g & 1) : ((g >> 1) & 1));
-          mbar_wait(tm_full(buf), (modeB ? (g >> 1) : (g >> 2)) & 1);
+          const uint32_t g = ecount + i, buf = g & 1;
+          const int cb = g % N_CS;
+          TRW(0, mbar_wait(tm_full(buf), (g >> 1) & 1));
           tc_fence_after();
-          const float r = c_tile(tbase + buf * BUF_COLS, nrows_w, sc, nl + row0);
+          float r;
+          TRW(1, r = c_cols(tbase + buf * BUF_COLS + c_col0, c_nc, sc, nl + c_col0));
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(tm_empty(buf));
-          const int j = (sg.tile - i) * TILE + lrow;
-          if (j < p.L) {
-            const size_t o = (size_t)sg.head * p.L + j;
-            if (modeB) {
-              // two addends per element onto a zeroed word: a + b == b + a bit for bit, whichever arrives first
-              atomicAdd(&p.imp[o], r);
-              if (p.imp_out) atomicAdd(&p.imp_out[o], r);
-            } else {
-              p.imp[o] = r;
-              if (p.imp_out) p.imp_out[o] = r;
-            }
-          }
+          TRW(4, mbar_wait(cs_empty(cb), ((g / N_CS) & 1) ^ 1));
+          cs_s[(cb * 4 + cq) * TILE + quarter * 32 + lane] = r;
+          __syncwarp();
+          if (lane == 0) mbar_arrive(cs_full(cb));
         }
       }
       ecount += sg.n;
@@ -572,6 +660,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
     }
   }
 
+  TR_FLUSH()
   tc_fence_before();
   __syncthreads();
   if (warp == W_MMA) {
@@ -639,7 +728,7 @@ bool score_tc_supported(const Shape& s) {
 
 int score_tc_launch_count(const Shape&) { return 2; }
 
-size_t score_tc_part_elems(int heads, int rows) { return (size_t)(MAX_GRID + heads) * 2 * rows; }
+size_t score_tc_part_elems(int heads, int rows) { return (size_t)(MAX_GRID + heads) * 4 * rows; }
 
 cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const SplitPlan&, const Workspace& ws,
                             float* imp_out, float* lse_out, cudaStream_t st) {
@@ -671,19 +760,21 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
   TcParams p;
   p.L = s.L; p.rows = s.rows; p.T = (s.L + TILE - 1) / TILE;
   p.heads = heads;
-  p.n_slots = s.rows <= 128 ? 2 : 1;
+  p.n_slots = s.rows <= 128 ? 4 : 2;
   p.phase = 0;
   p.N = (long long)heads * p.T;
   p.scale_log2 = 1.4426950408889634f / sqrtf((float)s.d);
   p.part = ws.part; p.lse_out = lse_out; p.imp = ws.imp; p.imp_out = imp_out;
 
-  cudaError_t e;
-  if (s.rows > 128) {  // each importance is the sum of two warpgroup partials added onto zero (see the C tiles)
-    if ((e = cudaMemsetAsync(ws.imp, 0, (size_t)heads * s.L * sizeof(float), st)) != cudaSuccess) return e;
-    if (imp_out && (e = cudaMemsetAsync(imp_out, 0, (size_t)heads * s.L * sizeof(float), st)) != cudaSuccess) return e;
-  }
-  if (qrows == 128) return launch_cfg<128, 2, 5>(tmK, tmQ, p, st);
-  return launch_cfg<256, 1, 3>(tmK, tmQ, p, st);
+  if (qrows == 128) return launch_cfg<128, 2, 4>(tmK, tmQ, p, st);
+  return launch_cfg<256, 1, 4>(tmK, tmQ, p, st);
 }
 
 }  // namespace nacl
+
+#ifdef NACL_TC_TRACE
+// diagnostics build only: per-warp wait/compute cycle counters of the last launches
+extern "C" __attribute__((visibility("default"))) int nacl_debug_trace_read(long long* host, size_t bytes) {
+  return (int)cudaMemcpyFromSymbol(host, nacl::g_trace, bytes < sizeof(nacl::g_trace) ? bytes : sizeof(nacl::g_trace));
+}
+#endif

@@ -73,7 +73,7 @@ Workspace carve_workspace(void* base, int batch, int L, int Hq, int Hkv, int P) 
   ws.part = reinterpret_cast<float2*>(b + off); off = align_up(off + n_part * sizeof(float2), 256);
   ws.lse = reinterpret_cast<float*>(b + off);   off = align_up(off + n_rows * sizeof(float), 256);
   ws.imp = reinterpret_cast<float*>(b + off);   off = align_up(off + n_imp * sizeof(float), 256);
-  ws.key = reinterpret_cast<uint32_t*>(b + off); off = align_up(off + n_imp * sizeof(uint32_t), 256);
+  ws.key = reinterpret_cast<uint32_t*>(b + off); off = align_up(off + select_scratch_words(batch, Hkv, L) * sizeof(uint32_t), 256);
   ws.sync = reinterpret_cast<int*>(b + off);    off = align_up(off + sync_ints((size_t)batch * Hkv) * sizeof(int), 256);
   ws.bytes = off;
   return ws;
@@ -183,16 +183,8 @@ static int evict_impl(const nacl_params_t& p) {
   if (e != cudaSuccess) return fail_cuda(e);
 
   const int C = p.budget_proxy + p.budget_random;
-  if (p.budget_random > 0) {
-    StageScope sc(ST_KEYS, st);
-    e = launch_keys(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.seed, p.layer, p.flags, st);
-    if (e != cudaSuccess) return fail_cuda(e);
-  }
-  {
-    StageScope sc(ST_SELECT, st);
-    e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent,
-                      p.out_idx, st);
-  }
+  e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
+                    p.flags, p.out_idx, st);
   if (e != cudaSuccess) return fail_cuda(e);
   {
     StageScope sc(ST_GATHER, st);
@@ -314,8 +306,8 @@ int nacl_launch_count(int dtype, int batch, int L, int Hq, int Hkv, int d, int P
   s.batch = batch; s.L = L; s.Hq = Hq; s.Hkv = Hkv; s.d = d; s.P = P;
   s.G = Hq / Hkv; s.rows = s.G * P; s.dtype = dtype; s.esize = dtype == NACL_DTYPE_F32 ? 4 : 2;
   const bool tc = !(flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
-  // scoring + keys + select + gather (budget_random > 0 and C > 0 assumed)
-  return (tc ? score_tc_launch_count(s) : 3) + 3;
+  // scoring + select (+ a separate keys kernel for very long rows) + gather (budget_random > 0 and C > 0 assumed)
+  return (tc ? score_tc_launch_count(s) : 3) + (select_uses_cluster(L) ? 1 : 2) + 1;
 }
 
 int nacl_profile_enable(int on) {

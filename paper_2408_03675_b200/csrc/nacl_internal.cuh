@@ -35,7 +35,7 @@ struct Workspace {
                        // [148 + heads, n_slots, G*P] (score_tc.cu)
   float* lse;          // [batch*Hq*P]            natural-log LSE of every proxy row
   float* imp;          // [batch*Hkv, L]          importance F_score
-  uint32_t* key;       // [batch*Hkv, L]          order-mapped fp32 Gumbel-top-k keys
+  uint32_t* key;       // select scratch (select_scratch_words): global radix histograms, or [batch*Hkv, L] keys for very long rows
   int* sync;           // [sync_ints(heads)]      reserved (counters / flags for future fused variants)
   size_t bytes;
 };
@@ -71,10 +71,13 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
 cudaError_t launch_keys(const float* imp, uint32_t* key, int batch, int Hkv, int L,
                         uint64_t seed, int layer, uint32_t flags, cudaStream_t st);
 
-// protected + top-k + Gumbel-top-k + ascending compaction -> out_idx
-cudaError_t launch_select(const float* imp, const uint32_t* key, int batch, int Hkv, int L,
-                          int budget_proxy, int budget_random, int n_sink, int n_recent,
-                          int32_t* out_idx, cudaStream_t st);
+// protected + top-k + Gumbel-top-k (keys fused when the row fits a cluster's shared memory) + ascending
+// compaction -> out_idx.  Records its own StageScopes.  `key` is scratch for the long-row fallback.
+bool select_uses_cluster(int L);
+size_t select_scratch_words(int batch, int Hkv, int L);  // 4-byte words of Workspace::key
+cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, int L, int budget_proxy, int budget_random,
+                          int n_sink, int n_recent, uint64_t seed, int layer, uint32_t flags, int32_t* out_idx,
+                          cudaStream_t st);
 
 // K,V <- K_S,V_S
 cudaError_t launch_gather(const void* K, const void* V, const int32_t* idx, int n_prob, int L, int C,

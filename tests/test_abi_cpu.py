@@ -45,8 +45,8 @@ def test_workspace_bytes_is_a_pure_function_of_shape(lib):
     for cfg in CONFIGS.values():
         w = lib.nacl_workspace_bytes(cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P)
         assert w == lib.nacl_workspace_bytes(cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P)
-        # at least the importance and the key vectors
-        assert w >= 2 * 4 * cfg.batch * cfg.Hkv * cfg.L
+        # at least the importance vector (the sampling keys stay in shared memory for rows a cluster can hold)
+        assert w >= 4 * cfg.batch * cfg.Hkv * cfg.L
         assert w < 64 << 20
     assert lib.nacl_workspace_bytes(1, 0, 4, 4, 64, 1) == 0
     assert lib.nacl_workspace_bytes(1, 128, 5, 4, 64, 1) == 0  # Hq % Hkv

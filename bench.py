@@ -74,7 +74,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.proc = None
@@ -146,14 +146,18 @@ def stage_alg_bytes(cfg) -> dict:
 
 
 def load_traffic(cfg_name: str, kernel: str):
-    """dram bytes per launch of `kernel` from the committed ncu --set full summary, if one exists."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram bytes (read + write) per launch of `kernel` from the committed ncu --set full summary
+    (profiles/traffic.csv: workload,kernel,dram_bytes_per_launch,source), if one exists."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         with open(path) as f:
-            t = json.load(f)
-        return t.get(cfg_name, {}).get(kernel)
+            for line in f:
+                c = [x.strip() for x in line.split(",")]
+                if len(c) >= 3 and c[0] == cfg_name and c[1] == kernel:
+                    return int(float(c[2]))
     except (OSError, ValueError):
-        return None
+        pass
+    return None
 
 
 def run_ours(args) -> dict:
@@ -362,7 +366,7 @@ def run_reference(args) -> dict:
 def main() -> int:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=4, choices=sorted(CONFIGS))

@@ -56,6 +56,10 @@ constexpr int NTHREADS = EPI_THREADS + 3 * 32;
 constexpr int TMEM_COLS = 512;
 constexpr int N_BUFS = 2;                      // TMEM accumulator buffers (one tile each)
 constexpr int BUF_COLS = 256;                  // TMEM columns per accumulator buffer
+#ifndef NACL_S_HALF_BARRIERS
+#define NACL_S_HALF_BARRIERS 0
+#endif
+constexpr bool kHalfBarriers = NACL_S_HALF_BARRIERS != 0;  // sweep S: full/empty barriers per 128-row half instead of per tile
 constexpr int N_CS = 4;                        // shared-memory buffers for the quarter column sums of a C tile
 constexpr int MAX_GRID = kNumSMs;              // the partial-statistics workspace is sized for this many CTAs
 constexpr uint32_t SPIN_LIMIT = 1u << 26;      // watchdog: a wait that long is a bug -> trap (loud failure)
@@ -317,7 +321,7 @@ struct Smem {
   static constexpr int OFF_LSE = OFF_K + STAGES * KSTAGE_BYTES;   // float[LSE_SLOTS][256]: -lse (log2 domain) of the segment's head
   static constexpr int OFF_CS = OFF_LSE + LSE_SLOTS * 256 * 4;    // float[N_CS][4][128]: quarter column sums of a C tile
   static constexpr int OFF_BARS = OFF_CS + N_CS * 4 * TILE * 4;
-  static constexpr int N_BARS = 2 * STAGES + 2 * NQ + 2 * N_BUFS + 2 * N_CS;
+  static constexpr int N_BARS = 2 * STAGES + 2 * NQ + 4 * N_BUFS + 2 * N_CS;
   static constexpr int OFF_TMEM = OFF_BARS + N_BARS * 8;
   static constexpr int TOTAL = OFF_TMEM + 8;
 };
@@ -439,15 +443,17 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
   if ((sbase & 1023u) != 0) __trap();  // the 128B-swizzled operand tiles need 1024-byte alignment
 
   const uint32_t bars = sbase + SM::OFF_BARS;
-  constexpr int B_KE = STAGES, B_QF = 2 * STAGES, B_QE = B_QF + NQ, B_TF = B_QE + NQ, B_TE = B_TF + N_BUFS, B_CF = B_TE + N_BUFS,
+  constexpr int B_KE = STAGES, B_QF = 2 * STAGES, B_QE = B_QF + NQ, B_TF = B_QE + NQ, B_TE = B_TF + 2 * N_BUFS, B_CF = B_TE + 2 * N_BUFS,
                 B_CE = B_CF + N_CS;
   static_assert(B_CE + N_CS == SM::N_BARS, "barrier count");
   auto k_full = [&](int s) { return bars + 8u * s; };
   auto k_empty = [&](int s) { return bars + 8u * (B_KE + s); };
   auto q_full = [&](int s) { return bars + 8u * (B_QF + s); };
   auto q_empty = [&](int s) { return bars + 8u * (B_QE + s); };
-  auto tm_full = [&](int b) { return bars + 8u * (B_TF + b); };
-  auto tm_empty = [&](int b) { return bars + 8u * (B_TE + b); };
+  // accumulator barriers per (buffer, 128-row half): sweep S fills and drains the two halves of a tile independently,
+  // sweep C (one N = G*P MMA group per tile) uses half 0 only
+  auto tm_full = [&](int b, int h) { return bars + 8u * (B_TF + 2 * b + h); };
+  auto tm_empty = [&](int b, int h) { return bars + 8u * (B_TE + 2 * b + h); };
   auto cs_full = [&](int b) { return bars + 8u * (B_CF + b); };
   auto cs_empty = [&](int b) { return bars + 8u * (B_CE + b); };
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + SM::OFF_TMEM);
@@ -461,7 +467,11 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
     for (int s = 0; s < NQ; ++s) { mbar_init(q_full(s), 1); mbar_init(q_empty(s), 1); }
-    for (int b = 0; b < N_BUFS; ++b) { mbar_init(tm_full(b), 1); mbar_init(tm_empty(b), N_EPI_WARPS); }
+    for (int b = 0; b < N_BUFS; ++b)
+      for (int h = 0; h < 2; ++h) {
+        mbar_init(tm_full(b, h), 1);
+        mbar_init(tm_empty(b, h), (p.phase == 0 && kHalfBarriers) ? N_EPI_WARPS / n_half : N_EPI_WARPS);  // epilogue warps that drain it
+      }
     for (int b = 0; b < N_CS; ++b) { mbar_init(cs_full(b), N_EPI_WARPS); mbar_init(cs_empty(b), 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -476,6 +486,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
 
   if (warp == W_TMA) {
     // ================================================================ TMA producer
+    const bool leader = elect_one();
     int stage = 0, qrun = 0;
     uint32_t kphase = 0;
     Walk walk(p);
@@ -484,7 +495,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
       const int qb = qrun % NQ;
       TRW(1, mbar_wait(q_empty(qb), ((qrun / NQ) & 1) ^ 1));
       const uint32_t qdst = sbase + SM::OFF_Q + qb * SM::Q_BYTES;
-      if (elect_one()) {
+      if (leader) {
         mbar_expect_tx(q_full(qb), SM::Q_BYTES);
         tma_load_2d(qdst, &tmQ, 0, sg.head * p.rows, q_full(qb));
         tma_load_2d(qdst + QROWS * 128, &tmQ, 64, sg.head * p.rows, q_full(qb));
@@ -494,7 +505,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
         TRW(0, mbar_wait(k_empty(stage), kphase ^ 1));
         const uint32_t kdst = sbase + SM::OFF_K + stage * KSTAGE_BYTES;
         const int j0 = (sg.tile + walk.step * i) * TILE;
-        if (elect_one()) {
+        if (leader) {
           mbar_expect_tx(k_full(stage), KSTAGE_BYTES);
           tma_load_3d(kdst, &tmK, 0, j0, sg.head, k_full(stage));
           tma_load_3d(kdst + BOX_BYTES, &tmK, 64, j0, sg.head, k_full(stage));
@@ -505,6 +516,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
     __syncwarp();
   } else if (warp == W_MMA) {
     // ================================================================ tcgen05.mma issuer
+    const bool leader = elect_one();  // ONE lane issues every MMA and every commit (a commit covers its own thread's MMAs)
     int stage = 0, qrun = 0;
     uint32_t kphase = 0, tcount = 0;
     const uint32_t idesc = p.phase == 0 ? umma_idesc(128, TILE) : umma_idesc(128, p.rows);
@@ -518,29 +530,42 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
       for (int i = 0; i < sg.n; ++i) {
         const uint32_t buf = tcount & 1, par = (tcount >> 1) & 1;
         TRW(0, mbar_wait(k_full(stage), kphase));
-        TRW(1, mbar_wait(tm_empty(buf), par ^ 1));
-        tc_fence_after();
         const uint32_t ksrc = sbase + SM::OFF_K + stage * KSTAGE_BYTES;
         const uint32_t dcol = tmem_base + buf * BUF_COLS;
-        if (elect_one()) {
-          if (p.phase == 0) {
-            for (int h = 0; h < n_half; ++h) {  // proxy rows [128h, 128h+128): 128 rows x 128 B further down in each Q box
+        if (p.phase == 0) {
+          // the two 128-row halves accumulate into different TMEM columns: their k-steps are interleaved so that
+          // consecutive MMAs never depend on each other (a dependent N=128 MMA chain runs at ~55 % of the pipe rate)
+          for (int h = 0; h < (kHalfBarriers ? n_half : 1); ++h) TRW(1, mbar_wait(tm_empty(buf, h), par ^ 1));
+          tc_fence_after();
+          if (leader) {
 #pragma unroll
-              for (int k = 0; k < 8; ++k) {
-                const uint32_t ko = (k >> 2) * BOX_BYTES + (k & 3) * 32;
-                const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32 + h * BOX_BYTES;
-                tc_mma(dcol + h * 128, umma_desc(qsrc + qo), umma_desc(ksrc + ko), idesc, k > 0);
-              }
+            for (int k = 0; k < 8; ++k) {
+              const uint32_t ko = (k >> 2) * BOX_BYTES + (k & 3) * 32;
+              const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32;
+              // proxy rows [128h, 128h+128) sit 128 rows x 128 B further down in each Q box
+              tc_mma(dcol, umma_desc(qsrc + qo), umma_desc(ksrc + ko), idesc, k > 0);
+              if (k == 7 && kHalfBarriers) tc_commit(tm_full(buf, 0));
+              if (n_half == 2) tc_mma(dcol + 128, umma_desc(qsrc + qo + BOX_BYTES), umma_desc(ksrc + ko), idesc, k > 0);
             }
-          } else {
+            if (kHalfBarriers) { if (n_half == 2) tc_commit(tm_full(buf, 1)); }
+            else tc_commit(tm_full(buf, 0));
+          }
+          __syncwarp();
+        } else {
+          TRW(1, mbar_wait(tm_empty(buf, 0), par ^ 1));
+          tc_fence_after();
+          if (leader) {
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
               const uint32_t ko = (k >> 2) * BOX_BYTES + (k & 3) * 32;
               const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32;
               tc_mma(dcol, umma_desc(ksrc + ko), umma_desc(qsrc + qo), idesc, k > 0);
             }
+            tc_commit(tm_full(buf, 0));  // the accumulator buffer is complete
           }
-          tc_commit(tm_full(buf));    // the accumulator buffer is complete
+          __syncwarp();
+        }
+        if (leader) {
           tc_commit(k_empty(stage));  // the reads of the stage are done once these MMAs complete
           if (i == sg.n - 1) tc_commit(q_empty(qb));  // every MMA that read the segment's Q has completed
         }
@@ -607,7 +632,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
         float m0 = -INFINITY, z0 = 0.f;
         for (int i = 0; i < sg.n; ++i) {
           const uint32_t g = ecount + i, buf = g & 1;
-          TRW(0, mbar_wait(tm_full(buf), (g >> 1) & 1));
+          TRW(0, mbar_wait(tm_full(buf, kHalfBarriers ? s_half : 0), (g >> 1) & 1));
           tc_fence_after();
           const int valid = p.L - (sg.tile + i) * TILE - s_col0;
           TRW(1, if (live) {
@@ -617,7 +642,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
           })
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(tm_empty(buf));
+          if (lane == 0) mbar_arrive(tm_empty(buf, kHalfBarriers ? s_half : 0));
         }
         // this warp's partial of the piece; (-inf, 0) when it saw no valid key
         if (s_row < p.rows)
@@ -642,13 +667,13 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
         for (int i = 0; i < sg.n; ++i) {
           const uint32_t g = ecount + i, buf = g & 1;
           const int cb = g % N_CS;
-          TRW(0, mbar_wait(tm_full(buf), (g >> 1) & 1));
+          TRW(0, mbar_wait(tm_full(buf, 0), (g >> 1) & 1));
           tc_fence_after();
           float r;
           TRW(1, r = c_cols(tbase + buf * BUF_COLS + c_col0, c_nc, sc, nl + c_col0));
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(tm_empty(buf));
+          if (lane == 0) mbar_arrive(tm_empty(buf, 0));
           TRW(4, mbar_wait(cs_empty(cb), ((g / N_CS) & 1) ^ 1));
           cs_s[(cb * 4 + cq) * TILE + quarter * 32 + lane] = r;
           __syncwarp();

@@ -33,6 +33,21 @@ def test_baseline_configs_small(binding, cid):
     print(f"cfg{cid}: max rel err {r['max_rel_err']:.2e}, top-k swaps {r['topk_swaps']}, random diffs {r['random_diffs']}")
 
 
+@pytest.mark.parametrize("cid,layer", [(3, 0), (4, 0), (4, 17), (5, 31)])
+def test_baseline_configs_full_size(binding, cid, layer):
+    """One whole layer of the 32-layer workloads at BASELINE.json's full sizes, in the launch configuration
+    bench.py times (same entry point, same shapes); the oracle finishes a layer in seconds, so every output is
+    compared, not a sample."""
+    cfg = CONFIGS[cid]
+    K, V, Q, planted = make_layer_inputs(cfg, layer=layer)
+    Bp, Br = cfg.budgets()
+    r = full_parity(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(layer), layer)
+    for b in range(cfg.batch):
+        for hk in range(cfg.Hkv):
+            assert set(planted[b, hk].tolist()) <= set(r["idx_gpu"][b, hk].tolist())
+    print(f"cfg{cid} layer {layer}: max rel err {r['max_rel_err']:.2e}, top-k swaps {r['topk_swaps']}, random diffs {r['random_diffs']}")
+
+
 # (B, L, Hq, Hkv, d, P, dtype, Bp, Br, n_sink, n_recent): several tiles + ragged tails, GQA, both dtypes
 RAGGED = [
     (2, 333, 4, 2, 64, 5, "f32", 40, 13, 3, 7),

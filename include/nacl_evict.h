@@ -128,6 +128,14 @@ int nacl_evict_host(const void* K, const void* V, const void* Qproxy, int dtype,
                     uint64_t seed, int layer,
                     void* out_K, void* out_V, int32_t* out_idx, int device);
 
+/* Step 5 on its own (R4/R5/R10/R15): the Random-Eviction sampling key of EVERY position,
+ *   out_keys[b,hk,j] = fl32( ln w_j - ln(-ln u_j) ),  u_j = Philox4x32-10(counter = (j, hk, b, layer), key = seed),
+ * w_j = importance[b,hk,j] (or exp / 1 under the NACL_FLAG_SAMPLE_* flags); -inf where w_j = 0.  The budget_random
+ * positions with the largest keys among the candidates are the sample.  importance, out_keys: DEVICE pointers,
+ * [batch,Hkv,L] fp32, 4-byte aligned; enqueued on `stream`.  nacl_evict computes the same keys internally. */
+int nacl_gumbel_keys(const float* importance, float* out_keys, int batch, int Hkv, int L,
+                     uint64_t seed, int layer, uint32_t flags, void* stream);
+
 /* Bytes of scratch one call needs (a pure function of the shape; 0 on invalid shapes). */
 size_t nacl_workspace_bytes(int batch, int L, int Hq, int Hkv, int d, int P);
 

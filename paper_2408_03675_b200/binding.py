@@ -19,7 +19,7 @@ FLAG_CAUSAL, FLAG_SAMPLE_SOFTMAX_OF_SCORE, FLAG_SAMPLE_UNIFORM, FLAG_SCORE_CUDA_
 
 EXPORTS = ("nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes",
            "nacl_launch_count", "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version",
-           "nacl_profile_enable", "nacl_profile_read", "nacl_stage_name")
+           "nacl_profile_enable", "nacl_profile_read", "nacl_stage_name", "nacl_gumbel_keys")
 N_STAGES = 7
 
 
@@ -75,6 +75,8 @@ def _load() -> C.CDLL:
     lib.nacl_last_cuda_error.restype = i32
     lib.nacl_version.argtypes = []
     lib.nacl_version.restype = i32
+    lib.nacl_gumbel_keys.argtypes = [vp, vp, i32, i32, i32, u64, i32, u32, vp]
+    lib.nacl_gumbel_keys.restype = i32
     lib.nacl_profile_enable.argtypes = [i32]
     lib.nacl_profile_enable.restype = i32
     lib.nacl_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int64), i32]
@@ -136,6 +138,21 @@ def nacl_profile_read(reset: bool = True) -> dict:
     if rc != 0:
         raise NaclError(rc, "nacl_profile_read")
     return {_lib.nacl_stage_name(s).decode(): (float(ms[s]), int(n[s])) for s in range(N_STAGES)}
+
+
+def nacl_gumbel_keys(importance: torch.Tensor, seed: int, layer: int, flags: int = 0, out: torch.Tensor | None = None,
+                     stream=None) -> torch.Tensor:
+    """Sampling keys of every position (include/nacl_evict.h nacl_gumbel_keys): importance [B,Hkv,L] fp32 on the GPU."""
+    assert importance.is_cuda and importance.dtype == torch.float32 and importance.dim() == 3 and importance.is_contiguous()
+    B, Hkv, L = importance.shape
+    if out is None:
+        out = torch.empty_like(importance)
+    st = (stream or torch.cuda.current_stream(importance.device)).cuda_stream
+    with torch.cuda.device(importance.device):
+        rc = _lib.nacl_gumbel_keys(importance.data_ptr(), out.data_ptr(), B, Hkv, L, seed & 0xFFFFFFFFFFFFFFFF, layer, flags, st)
+    if rc != 0:
+        raise NaclError(rc, "nacl_gumbel_keys")
+    return out
 
 
 def nacl_evict(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer,

@@ -295,6 +295,18 @@ int nacl_evict_host(const void* K, const void* V, const void* Qproxy, int dtype,
   return rc;
 }
 
+int nacl_gumbel_keys(const float* importance, float* out_keys, int batch, int Hkv, int L, uint64_t seed, int layer,
+                     uint32_t flags, void* stream) {
+  if (!importance || !out_keys) return NACL_ERR_NULL;
+  if (batch < 1 || Hkv < 1 || L < 1 || L > (1 << 24) || (long)batch * Hkv > 65535) return NACL_ERR_SHAPE;
+  if ((reinterpret_cast<uintptr_t>(importance) | reinterpret_cast<uintptr_t>(out_keys)) & 3u) return NACL_ERR_ALIGN;
+  const uint32_t known = NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE | NACL_FLAG_SAMPLE_UNIFORM;
+  if ((flags & ~known) || flags == known) return NACL_ERR_UNSUPPORTED;
+  cudaError_t e = launch_keys(importance, reinterpret_cast<uint32_t*>(out_keys), batch, Hkv, L, seed, layer, flags, false,
+                              static_cast<cudaStream_t>(stream));
+  return e == cudaSuccess ? NACL_OK : fail_cuda(e);
+}
+
 size_t nacl_workspace_bytes(int batch, int L, int Hq, int Hkv, int d, int P) {
   if (validate_shape(NACL_DTYPE_BF16, batch, L, Hq, Hkv, d, P) != NACL_OK) return 0;
   return carve_workspace(nullptr, batch, L, Hq, Hkv, P).bytes;

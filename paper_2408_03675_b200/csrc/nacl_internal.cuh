@@ -67,9 +67,9 @@ size_t score_tc_part_elems(int heads, int rows);  // float2 elements of Workspac
 cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const SplitPlan& sp,
                             const Workspace& ws, float* imp_out, float* lse_out, cudaStream_t st);
 
-// Gumbel-top-k keys: key[p,j] = ordermap(fl32(ln w(imp) - ln(-ln u)))
-cudaError_t launch_keys(const float* imp, uint32_t* key, int batch, int Hkv, int L,
-                        uint64_t seed, int layer, uint32_t flags, cudaStream_t st);
+// Gumbel-top-k keys: key[p,j] = fl32(ln w(imp) - ln(-ln u)), order-mapped to uint32 (ordermapped) or as float bits
+cudaError_t launch_keys(const float* imp, uint32_t* key, int batch, int Hkv, int L, uint64_t seed, int layer, uint32_t flags,
+                        bool ordermapped, cudaStream_t st);
 
 // protected + top-k + Gumbel-top-k (keys fused when the row fits a cluster's shared memory) + ascending
 // compaction -> out_idx.  Records its own StageScopes.  `key` is scratch for the long-row fallback.

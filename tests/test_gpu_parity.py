@@ -168,3 +168,32 @@ def test_caller_workspace_and_graph_capture(binding):
         g.replay()
         s.synchronize()
     assert torch.equal(oi, want[2]) and torch.equal(oK, want[0]) and torch.equal(oV, want[1])
+
+
+@pytest.mark.parametrize("flag_name", ["default", "FLAG_SAMPLE_SOFTMAX_OF_SCORE", "FLAG_SAMPLE_UNIFORM"])
+def test_gumbel_keys_bitwise_against_the_oracle(binding, flag_name):
+    """The sampling keys (Philox uniforms, two fp64 logarithms by the library's table-driven routine, one rounding to
+    fp32: DESIGN.md R15) against the oracle's libm keys for 2^20 positions whose importances span 40 decades, including
+    0 and fp32 subnormals.  Both logs are accurate to ~1 ulp of fp64, so a key can differ only where the fp64 sum falls
+    within ~1e-16 (relative) of an fp32 rounding boundary: at most a few positions in 10^6, and never by more than 1 ulp."""
+    flags = 0 if flag_name == "default" else getattr(binding, flag_name)
+    B, Hkv, L = 2, 4, 131072
+    rng = np.random.default_rng(7)
+    imp = np.exp(rng.uniform(-92.0, 5.5, size=(B, Hkv, L))).astype(np.float32)
+    imp[0, 0, :64] = 0.0
+    imp[0, 1, :64] = np.float32(1e-42)          # subnormal
+    imp[1, 2, :1024] = np.float32(1.0) + np.arange(1024, dtype=np.float32) * np.float32(2.0 ** -23)  # around ln = 0
+    if flags == binding.FLAG_SAMPLE_SOFTMAX_OF_SCORE:
+        imp = np.minimum(imp, np.float32(64.0))
+    seed, layer = 0x1234_5678_9ABC_DEF0, 5
+    keys_gpu = binding.nacl_gumbel_keys(torch.from_numpy(imp).cuda(), seed, layer, flags).cpu().numpy()
+    # all non-protected positions are candidates when nothing is kept by the top-k: Bp = |Pi| = 0, Br = 1
+    _, keys_ref = oracle.select(imp, 0, 1, 0, 0, seed, layer, flags & 0x7, return_keys=True)
+    assert not np.isnan(keys_ref).any()
+    a, b = keys_gpu.view(np.int32).astype(np.int64), keys_ref.view(np.int32).astype(np.int64)
+    diff = a != b
+    n_diff = int(diff.sum())
+    assert n_diff <= 8, f"{n_diff} of {a.size} keys differ"
+    if n_diff:
+        assert np.abs(a[diff] - b[diff]).max() <= 1  # neighbouring floats (same sign: no key sits at +-0 here)
+    print(f"{flag_name}: {n_diff} of {a.size} keys differ by 1 ulp")

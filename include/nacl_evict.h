@@ -40,6 +40,8 @@
  * Same inputs and seed give bit-identical outputs run to run (no floating-point atomics).
  * nacl_evict_host is the same operation on HOST buffers (copies inside; synchronous).
  *
+ * nacl_evict_ex with lse_in (the row log-sum-exps, e.g. from the prefill attention) runs a single sweep over K.
+ *
  * With budget_proxy + budget_random == 0 the outputs are empty and their pointers may be NULL.
  *
  * Errors: 0 = OK; negative = error; nothing is thrown and no output is written on a
@@ -59,7 +61,7 @@
 extern "C" {
 #endif
 
-#define NACL_VERSION 100 /* major*10000 + minor*100 + patch */
+#define NACL_VERSION 101 /* major*10000 + minor*100 + patch */
 
 #define NACL_DTYPE_F32 0
 #define NACL_DTYPE_BF16 1
@@ -99,6 +101,10 @@ typedef struct nacl_params {
   void* workspace;                 /* optional; >= nacl_workspace_bytes(...) bytes, 256-byte aligned */
   size_t workspace_bytes;
   void* stream;                    /* cudaStream_t */
+  const float* lse_in;             /* optional [batch,Hq,P] fp32: ln sum_j exp(s[i,j]) of every proxy row over ALL L keys, as a
+                                      prefill attention kernel that keeps its softmax statistics already has it (the contract of
+                                      the paper's Algorithm 2).  When given, the statistics sweep over K is
+                                      skipped: one logit sweep instead of two.  The caller answers for its accuracy. */
 } nacl_params_t;
 
 /* bf16 K/V/Q.  Steps 1-7 above on `stream`. */

@@ -33,6 +33,7 @@ class NaclParams(C.Structure):
         ("out_K", C.c_void_p), ("out_V", C.c_void_p), ("out_idx", C.c_void_p),
         ("out_importance", C.c_void_p), ("out_lse", C.c_void_p),
         ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("stream", C.c_void_p),
+        ("lse_in", C.c_void_p),
     ]
 
 
@@ -181,8 +182,9 @@ def nacl_evict(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed
 
 def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer, flags=0,
                   out_K=None, out_V=None, out_idx=None, want_importance=False, want_lse=False,
-                  workspace=None, stream=None):
-    """include/nacl_evict.h `nacl_evict_ex`.  Returns a dict with out_K, out_V, out_idx and, if asked,
+                  workspace=None, stream=None, lse_in=None):
+    """include/nacl_evict.h `nacl_evict_ex`.  lse_in: optional [B,Hq,P] fp32 row log-sum-exps (single-sweep
+    path).  Returns a dict with out_K, out_V, out_idx and, if asked,
     importance [B,Hkv,L] fp32 and lse [B,Hq,P] fp32."""
     B, Hkv, L, d, Hq, P = _shapes(K, V, Qproxy)
     if not K.is_cuda:
@@ -210,6 +212,9 @@ def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, s
     if workspace is not None:
         p.workspace, p.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
     p.stream = (stream or torch.cuda.current_stream(dev)).cuda_stream
+    if lse_in is not None:
+        assert lse_in.is_cuda and lse_in.dtype == torch.float32 and lse_in.is_contiguous() and lse_in.shape == (B, Hq, P)
+        p.lse_in = lse_in.data_ptr()
     with torch.cuda.device(dev):
         rc = _lib.nacl_evict_ex(C.byref(p))
     if rc != 0:

@@ -178,8 +178,9 @@ static int evict_impl(const nacl_params_t& p) {
 
   cudaError_t e;
   const bool tc = !(p.flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
-  if (tc) e = launch_score_tc(s, p.K, p.Qproxy, sp, ws, p.out_importance, p.out_lse, st);
-  else e = launch_score_generic(s, p.K, p.Qproxy, sp, ws, p.out_importance, p.out_lse, st);
+  if (p.lse_in && (reinterpret_cast<uintptr_t>(p.lse_in) & 3u)) return NACL_ERR_ALIGN;
+  if (tc) e = launch_score_tc(s, p.K, p.Qproxy, sp, ws, p.lse_in, p.out_importance, p.out_lse, st);
+  else e = launch_score_generic(s, p.K, p.Qproxy, sp, ws, p.lse_in, p.out_importance, p.out_lse, st);
   if (e != cudaSuccess) return fail_cuda(e);
 
   const int C = p.budget_proxy + p.budget_random;

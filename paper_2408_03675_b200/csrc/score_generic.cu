@@ -160,29 +160,36 @@ __global__ void __launch_bounds__(NT) nacl_colsum_kernel(const T* __restrict__ K
 
 template <typename T>
 cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const SplitPlan& sp, const Workspace& ws,
-                         float* imp_out, float* lse_out, cudaStream_t st) {
+                         const float* lse_in, float* imp_out, float* lse_out, cudaStream_t st) {
   const size_t smem = (size_t)2 * 64 * (s.d + 1) * sizeof(float);
   cudaError_t e;
   if ((e = cudaFuncSetAttribute(nacl_stats_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute(nacl_colsum_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
   const float inv_sqrt_d = 1.0f / sqrtf((float)s.d);
   dim3 g1(sp.n_chunks, s.Hkv, s.batch);
+  const int n_rows = s.batch * s.Hq * s.P;
+  const float* lse = ws.lse;
+  if (lse_in) {  // the caller has the row statistics: no sweep S
+    lse = lse_in;
+    if (lse_out && (e = cudaMemcpyAsync(lse_out, lse_in, (size_t)n_rows * sizeof(float), cudaMemcpyDeviceToDevice, st)) != cudaSuccess)
+      return e;
+  } else {
   {
     StageScope sc(ST_STATS, st);
     nacl_stats_kernel<T><<<g1, NT, smem, st>>>((const T*)K, (const T*)Q, ws.part, s.L, s.Hq, s.Hkv, s.d, s.P, s.G, sp.chunk,
                                           sp.n_chunks, inv_sqrt_d);
   }
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  const int n_rows = s.batch * s.Hq * s.P;
   {
     StageScope sc(ST_COMBINE, st);
     nacl_combine_kernel<<<(n_rows + 127) / 128, 128, 0, st>>>(ws.part, ws.lse, lse_out, n_rows, sp.n_chunks);
   }
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  }
   dim3 g2((s.L + TK - 1) / TK, s.Hkv, s.batch);
   {
     StageScope sc(ST_COLSUM, st);
-    nacl_colsum_kernel<T><<<g2, NT, smem, st>>>((const T*)K, (const T*)Q, ws.lse, ws.imp, imp_out, s.L, s.Hq, s.Hkv, s.d, s.P,
+    nacl_colsum_kernel<T><<<g2, NT, smem, st>>>((const T*)K, (const T*)Q, lse, ws.imp, imp_out, s.L, s.Hq, s.Hkv, s.d, s.P,
                                            s.G, inv_sqrt_d);
   }
   return cudaGetLastError();
@@ -191,9 +198,9 @@ cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const Spl
 }  // namespace
 
 cudaError_t launch_score_generic(const Shape& s, const void* K, const void* Q, const SplitPlan& sp, const Workspace& ws,
-                                 float* imp_out, float* lse_out, cudaStream_t st) {
-  if (s.dtype == NACL_DTYPE_F32) return launch_typed<float>(s, K, Q, sp, ws, imp_out, lse_out, st);
-  return launch_typed<__nv_bfloat16>(s, K, Q, sp, ws, imp_out, lse_out, st);
+                                 const float* lse_in, float* imp_out, float* lse_out, cudaStream_t st) {
+  if (s.dtype == NACL_DTYPE_F32) return launch_typed<float>(s, K, Q, sp, ws, lse_in, imp_out, lse_out, st);
+  return launch_typed<__nv_bfloat16>(s, K, Q, sp, ws, lse_in, imp_out, lse_out, st);
 }
 
 }  // namespace nacl

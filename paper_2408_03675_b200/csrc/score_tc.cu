@@ -89,6 +89,7 @@ struct TcParams {
   long long N;             // heads * T
   float scale_log2;        // log2(e) / sqrt(d)
   float2* part;            // [MAX_GRID + heads, n_slots, rows]  (m, z) per piece, log2 domain
+  const float* lse_in;     // optional [heads*rows], natural log: given row statistics (no sweep S)
   float* lse_out;          // optional [heads*rows], natural log
   float* imp;              // [heads, L]
   float* imp_out;          // optional
@@ -654,10 +655,15 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
         TRW(2, {
           const int r = threadIdx.x;
           if (r < p.rows) {
-            const int c_first = cta_of_tile((long long)sg.head * p.T, p.N, G);
-            const int c_last = cta_of_tile((long long)(sg.head + 1) * p.T - 1, p.N, G);
-            const float l2 = merge_row(p.part + ((size_t)(c_first + sg.head) * p.n_slots) * p.rows + r,
-                                       (c_last - c_first + 1) * p.n_slots, (size_t)p.rows);
+            float l2;
+            if (p.lse_in) {
+              l2 = p.lse_in[(size_t)sg.head * p.rows + r] * 1.4426950408889634f;  // given (natural log) -> log2 domain
+            } else {
+              const int c_first = cta_of_tile((long long)sg.head * p.T, p.N, G);
+              const int c_last = cta_of_tile((long long)(sg.head + 1) * p.T - 1, p.N, G);
+              l2 = merge_row(p.part + ((size_t)(c_first + sg.head) * p.n_slots) * p.rows + r, (c_last - c_first + 1) * p.n_slots,
+                             (size_t)p.rows);
+            }
             nl[r] = -l2;
             // the CTA that owns the head's first tile publishes lse
             if (p.lse_out && sg.tile - (sg.n - 1) == 0) p.lse_out[(size_t)sg.head * p.rows + r] = l2 * 0.69314718055994530942f;
@@ -730,7 +736,7 @@ cudaError_t launch_cfg(const CUtensorMap& tmK, const CUtensorMap& tmQ, TcParams 
   if (e != cudaSuccess) return e;
   long long grid = sm_count() < MAX_GRID ? sm_count() : MAX_GRID;
   if (p.N < grid) grid = p.N;
-  {
+  if (!p.lse_in) {
     StageScope sc(ST_STATS, st);
     p.phase = 0;
     kern<<<(int)grid, NTHREADS, SM::TOTAL, st>>>(tmK, tmQ, p);
@@ -756,7 +762,7 @@ int score_tc_launch_count(const Shape&) { return 2; }
 size_t score_tc_part_elems(int heads, int rows) { return (size_t)(MAX_GRID + heads) * 4 * rows; }
 
 cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const SplitPlan&, const Workspace& ws,
-                            float* imp_out, float* lse_out, cudaStream_t st) {
+                            const float* lse_in, float* imp_out, float* lse_out, cudaStream_t st) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return cudaErrorNotSupported;  // no silent fallback: the caller reports NACL_ERR_CUDA
   const int heads = s.batch * s.Hkv;
@@ -789,7 +795,7 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
   p.phase = 0;
   p.N = (long long)heads * p.T;
   p.scale_log2 = 1.4426950408889634f / sqrtf((float)s.d);
-  p.part = ws.part; p.lse_out = lse_out; p.imp = ws.imp; p.imp_out = imp_out;
+  p.part = ws.part; p.lse_in = lse_in; p.lse_out = lse_out; p.imp = ws.imp; p.imp_out = imp_out;
 
   if (qrows == 128) return launch_cfg<128, 2, 4>(tmK, tmQ, p, st);
   return launch_cfg<256, 1, 4>(tmK, tmQ, p, st);

@@ -511,8 +511,10 @@ __device__ void cluster_radix_select(F getval, int nloc, int j0, int K, ClShared
 }
 
 #ifdef NACL_SEL_TRACE
-__device__ long long g_sel_trace[16];
-#define STAMP(k) if (blockIdx.x == 0 && threadIdx.x == 0) g_sel_trace[k] = clock64();
+__device__ long long g_sel_trace[16 + 2 * 1024];
+__device__ __forceinline__ long long sel_gtimer() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define STAMP(k) { if (blockIdx.x == 0 && threadIdx.x == 0) g_sel_trace[k] = clock64(); \
+  if (threadIdx.x == 0 && blockIdx.x < 1024 && (k == 0 || k == 5)) g_sel_trace[16 + 2 * blockIdx.x + (k == 5)] = sel_gtimer(); }
 #else
 #define STAMP(k)
 #endif

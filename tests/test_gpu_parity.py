@@ -197,3 +197,30 @@ def test_gumbel_keys_bitwise_against_the_oracle(binding, flag_name):
     if n_diff:
         assert np.abs(a[diff] - b[diff]).max() <= 1  # neighbouring floats (same sign: no key sits at +-0 here)
     print(f"{flag_name}: {n_diff} of {a.size} keys differ by 1 ulp")
+
+
+@pytest.mark.parametrize("case", [(1, 4100, 32, 8, 128, 64, "bf16"), (2, 1500, 8, 4, 128, 16, "bf16"), (2, 700, 4, 2, 64, 5, "f32")],
+                         ids=["tc_GP256", "tc_GP32", "cuda_core_f32"])
+def test_lse_in_single_sweep(binding, case):
+    """SURVEY.md 8(f) f1 / the contract of the paper's Algorithm 2: with the row log-sum-exps
+    supplied, one logit sweep gives the same importance (north-star tolerance) and, on it, exactly the oracle's selection."""
+    from parity import check_scores, check_staged, check_structure, check_gather
+
+    B, L, Hq, Hkv, d, P, dt = case
+    K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype=dt, seed=L + 1)
+    imp_ref, lse_ref = oracle.importance(K, Q, return_lse=True)
+    Bp, Br, ns, nr = L // 6, L // 20, 4, P
+    lse_in = torch.from_numpy(lse_ref.astype(np.float32)).cuda()
+    res = binding.nacl_evict_ex(K.cuda(), V.cuda(), Q.cuda(), Bp, Br, ns, nr, 77, 2, want_importance=True, want_lse=True,
+                                lse_in=lse_in)
+    torch.cuda.synchronize()
+    imp = res["importance"].cpu().numpy()
+    idx = res["out_idx"].cpu().numpy()
+    check_scores(imp, imp_ref, Hq // Hkv, P)
+    check_structure(idx, L, Bp + Br, ns, nr)
+    check_staged(idx, imp, Bp, Br, ns, nr, 77, 2)
+    check_gather(K, V, res["out_K"].cpu(), res["out_V"].cpu(), idx)
+    np.testing.assert_allclose(res["lse"].cpu().numpy(), lse_ref, rtol=1e-6, atol=1e-6)
+    # and it agrees with the self-contained two-sweep call to the score tolerance
+    res2 = binding.nacl_evict_ex(K.cuda(), V.cuda(), Q.cuda(), Bp, Br, ns, nr, 77, 2, want_importance=True)
+    np.testing.assert_allclose(res2["importance"].cpu().numpy(), imp, rtol=2e-3, atol=1e-30)

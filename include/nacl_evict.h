@@ -76,7 +76,7 @@ extern "C" {
 #define NACL_ERR_UNSUPPORTED (-7) /* a flag or dtype this build does not implement */
 
 /* nacl_evict_ex flags */
-#define NACL_FLAG_CAUSAL 1u                  /* DESIGN.md R1; not implemented on the GPU yet -> NACL_ERR_UNSUPPORTED */
+#define NACL_FLAG_CAUSAL 1u                  /* DESIGN.md R1: proxy row i is prompt position L-P+i and sees keys j <= L-P+i */
 #define NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE 2u /* sampling weight exp(imp_j) (R4) */
 #define NACL_FLAG_SAMPLE_UNIFORM 4u          /* uniform sampling weights (paper's ablation) */
 #define NACL_FLAG_SCORE_CUDA_CORES 0x100u    /* debugging: run the generic CUDA-core scoring kernels even where

@@ -146,7 +146,6 @@ static int evict_impl(const nacl_params_t& p) {
   if (rc) return rc;
   const uint32_t known = NACL_FLAG_CAUSAL | NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE | NACL_FLAG_SAMPLE_UNIFORM | NACL_FLAG_SCORE_CUDA_CORES;
   if (p.flags & ~known) return NACL_ERR_UNSUPPORTED;
-  if (p.flags & NACL_FLAG_CAUSAL) return NACL_ERR_UNSUPPORTED;
   if ((p.flags & NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE) && (p.flags & NACL_FLAG_SAMPLE_UNIFORM)) return NACL_ERR_UNSUPPORTED;
 
   Shape s;
@@ -179,8 +178,8 @@ static int evict_impl(const nacl_params_t& p) {
   cudaError_t e;
   const bool tc = !(p.flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
   if (p.lse_in && (reinterpret_cast<uintptr_t>(p.lse_in) & 3u)) return NACL_ERR_ALIGN;
-  if (tc) e = launch_score_tc(s, p.K, p.Qproxy, sp, ws, p.lse_in, p.out_importance, p.out_lse, st);
-  else e = launch_score_generic(s, p.K, p.Qproxy, sp, ws, p.lse_in, p.out_importance, p.out_lse, st);
+  if (tc) e = launch_score_tc(s, p.K, p.Qproxy, sp, ws, p.lse_in, (p.flags & NACL_FLAG_CAUSAL) != 0, p.out_importance, p.out_lse, st);
+  else e = launch_score_generic(s, p.K, p.Qproxy, sp, ws, p.lse_in, (p.flags & NACL_FLAG_CAUSAL) != 0, p.out_importance, p.out_lse, st);
   if (e != cudaSuccess) return fail_cuda(e);
 
   const int C = p.budget_proxy + p.budget_random;

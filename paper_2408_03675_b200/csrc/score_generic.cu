@@ -53,7 +53,7 @@ __device__ __forceinline__ size_t row_id(int b, int hk, int gr, int G, int P, in
 template <typename T>
 __global__ void __launch_bounds__(NT) nacl_stats_kernel(const T* __restrict__ K, const T* __restrict__ Q, float2* __restrict__ part,
                                                     int L, int Hq, int Hkv, int d, int P, int G, int chunk, int n_chunks,
-                                                    float inv_sqrt_d) {
+                                                    float inv_sqrt_d, int causal) {
   extern __shared__ float smem[];
   const int ld = d + 1;
   float* Qs = smem;            // [64][d+1]
@@ -80,7 +80,9 @@ __global__ void __launch_bounds__(NT) nacl_stats_kernel(const T* __restrict__ K,
       dots(Qs, r, Ks, sub, d, a);
 #pragma unroll
       for (int u = 0; u < U; ++u) {
-        if (sub + SUB * u < nk) {
+        // NACL_FLAG_CAUSAL (R1): proxy row i is prompt position L-P+i and sees keys j <= L-P+i
+        const int jj = j0 + sub + SUB * u;
+        if (sub + SUB * u < nk && !(causal && jj > L - P + (rb + r) % P)) {
           float x = a[u] * inv_sqrt_d;
           if (x > m) { z = z * expf(m - x) + 1.f; m = x; }
           else z += expf(x - m);
@@ -115,7 +117,7 @@ __global__ void nacl_combine_kernel(const float2* __restrict__ part, float* __re
 template <typename T>
 __global__ void __launch_bounds__(NT) nacl_colsum_kernel(const T* __restrict__ K, const T* __restrict__ Q, const float* __restrict__ lse,
                                                      float* __restrict__ imp, float* __restrict__ imp_out,
-                                                     int L, int Hq, int Hkv, int d, int P, int G, float inv_sqrt_d) {
+                                                     int L, int Hq, int Hkv, int d, int P, int G, float inv_sqrt_d, int causal) {
   extern __shared__ float smem[];
   const int ld = d + 1;
   float* Qs = smem;
@@ -143,7 +145,7 @@ __global__ void __launch_bounds__(NT) nacl_colsum_kernel(const T* __restrict__ K
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       int rr = sub + SUB * u;
-      if (rr < nr) acc += expf(a[u] * inv_sqrt_d - lse_s[rr]);
+      if (rr < nr && !(causal && j0 + j > L - P + (rb + rr) % P)) acc += expf(a[u] * inv_sqrt_d - lse_s[rr]);
     }
   }
   red[sub][j] = acc;
@@ -160,7 +162,7 @@ __global__ void __launch_bounds__(NT) nacl_colsum_kernel(const T* __restrict__ K
 
 template <typename T>
 cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const SplitPlan& sp, const Workspace& ws,
-                         const float* lse_in, float* imp_out, float* lse_out, cudaStream_t st) {
+                         const float* lse_in, bool causal, float* imp_out, float* lse_out, cudaStream_t st) {
   const size_t smem = (size_t)2 * 64 * (s.d + 1) * sizeof(float);
   cudaError_t e;
   if ((e = cudaFuncSetAttribute(nacl_stats_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
@@ -177,7 +179,7 @@ cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const Spl
   {
     StageScope sc(ST_STATS, st);
     nacl_stats_kernel<T><<<g1, NT, smem, st>>>((const T*)K, (const T*)Q, ws.part, s.L, s.Hq, s.Hkv, s.d, s.P, s.G, sp.chunk,
-                                          sp.n_chunks, inv_sqrt_d);
+                                          sp.n_chunks, inv_sqrt_d, causal ? 1 : 0);
   }
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   {
@@ -190,7 +192,7 @@ cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const Spl
   {
     StageScope sc(ST_COLSUM, st);
     nacl_colsum_kernel<T><<<g2, NT, smem, st>>>((const T*)K, (const T*)Q, lse, ws.imp, imp_out, s.L, s.Hq, s.Hkv, s.d, s.P,
-                                           s.G, inv_sqrt_d);
+                                           s.G, inv_sqrt_d, causal ? 1 : 0);
   }
   return cudaGetLastError();
 }
@@ -198,9 +200,9 @@ cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const Spl
 }  // namespace
 
 cudaError_t launch_score_generic(const Shape& s, const void* K, const void* Q, const SplitPlan& sp, const Workspace& ws,
-                                 const float* lse_in, float* imp_out, float* lse_out, cudaStream_t st) {
-  if (s.dtype == NACL_DTYPE_F32) return launch_typed<float>(s, K, Q, sp, ws, lse_in, imp_out, lse_out, st);
-  return launch_typed<__nv_bfloat16>(s, K, Q, sp, ws, lse_in, imp_out, lse_out, st);
+                                 const float* lse_in, bool causal, float* imp_out, float* lse_out, cudaStream_t st) {
+  if (s.dtype == NACL_DTYPE_F32) return launch_typed<float>(s, K, Q, sp, ws, lse_in, causal, imp_out, lse_out, st);
+  return launch_typed<__nv_bfloat16>(s, K, Q, sp, ws, lse_in, causal, imp_out, lse_out, st);
 }
 
 }  // namespace nacl

@@ -86,6 +86,7 @@ struct TcParams {
   int L, rows, T;          // keys per head, proxy rows per kv head (G*P), key tiles per head
   int heads, n_slots;      // n_slots: epilogue warps that share a proxy row in sweep S = partials per (row, piece): 2 if rows > 128, else 4
   int phase;               // 0 = sweep S (statistics), 1 = sweep C (column sums)
+  int causal, P;           // NACL_FLAG_CAUSAL: proxy row r (i = r % P, prompt position L-P+i) sees keys j <= L-P+i
   long long N;             // heads * T
   float scale_log2;        // log2(e) / sqrt(d)
   float2* part;            // [MAX_GRID + heads, n_slots, rows]  (m, z) per piece, log2 domain
@@ -374,16 +375,19 @@ __device__ __forceinline__ void s_cols(uint32_t taddr, float sc, float& m, float
 }
 
 // last tile of a head: columns >= valid (relative to taddr) are keys past L and must not exist (-inf)
-__device__ __forceinline__ void s_cols_masked(uint32_t taddr, int nc, float sc, int valid, float& m, float& z) {
+// (warp-uniform `valid`: keys past L) and columns >= valid_t (per thread: keys its proxy row may not see, CAUSAL)
+__device__ __forceinline__ void s_cols_masked(uint32_t taddr, int nc, float sc, int valid, int valid_t, float& m, float& z) {
   uint32_t v[32];
 #pragma unroll 1
   for (int c = 0; c < nc && c < valid; c += 32) {
     tmem_ld32(taddr + c, v);
     tc_wait_ld(v);
+    if (c < valid_t) {  // (a row with no visible key in this block keeps its statistics: max3 of all -inf would poison them)
 #pragma unroll
-    for (int e = 0; e < 32; ++e)
-      if (c + e >= valid) v[e] = 0xFF800000u;
-    s_update(v, sc, m, z);
+      for (int e = 0; e < 32; ++e)
+        if (c + e >= valid_t) v[e] = 0xFF800000u;
+      s_update(v, sc, m, z);
+    }
   }
 }
 
@@ -432,6 +436,22 @@ __device__ __forceinline__ float c_cols(uint32_t taddr, int nc, float sc, const 
   float s0, s1;
   unpack2(add2(a0, a1), s0, s1);
   return s0 + s1;
+}
+
+// C tile under NACL_FLAG_CAUSAL (only the tiles that hold the last P keys): proxy rows r with r % P < imin do not see
+// this thread's key and contribute nothing
+__device__ __noinline__ float c_cols_causal(uint32_t taddr, int nc, float sc, const float* nl, int row0, int P, int imin) {
+  float acc = 0.f;
+  uint32_t v[32];
+#pragma unroll 1
+  for (int c = 0; c < nc; c += 4) {
+    tmem_ld4(taddr + c, v);
+    tc_wait_ld(v);
+#pragma unroll
+    for (int e = 0; e < 4; ++e)
+      if ((row0 + c + e) % P >= imin) acc += fast_exp2(fmaf(__uint_as_float(v[e]), sc, nl[c + e]));
+  }
+  return acc;
 }
 
 // ------------------------------------------------------------------ the kernel
@@ -636,10 +656,13 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
           TRW(0, mbar_wait(tm_full(buf, kHalfBarriers ? s_half : 0), (g >> 1) & 1));
           tc_fence_after();
           const int valid = p.L - (sg.tile + i) * TILE - s_col0;
+          // CAUSAL: this thread's row (i = s_row % P) sees the columns whose key j <= L-P+i
+          const bool ctile = p.causal && (sg.tile + i) * TILE + TILE - 1 > p.L - p.P;
           TRW(1, if (live) {
             const uint32_t ta = tbase + buf * BUF_COLS + s_half * 128 + s_col0;
-            if (valid >= s_nc) { if (n_half == 2) s_cols<64>(ta, sc, m0, z0); else s_cols<32>(ta, sc, m0, z0); }
-            else s_cols_masked(ta, s_nc, sc, valid, m0, z0);
+            if (ctile) s_cols_masked(ta, s_nc, sc, valid, min(valid, valid - p.P + 1 + s_row % p.P), m0, z0);
+            else if (valid >= s_nc) { if (n_half == 2) s_cols<64>(ta, sc, m0, z0); else s_cols<32>(ta, sc, m0, z0); }
+            else s_cols_masked(ta, s_nc, sc, valid, valid, m0, z0);
           })
           tc_fence_before();
           __syncwarp();
@@ -676,7 +699,11 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
           TRW(0, mbar_wait(tm_full(buf, 0), (g >> 1) & 1));
           tc_fence_after();
           float r;
-          TRW(1, r = c_cols(tbase + buf * BUF_COLS + c_col0, c_nc, sc, nl + c_col0));
+          const int jkey = (sg.tile - i) * TILE + quarter * 32 + lane;  // the key this thread owns
+          if (p.causal && (sg.tile - i) * TILE + TILE - 1 > p.L - p.P)
+            r = c_cols_causal(tbase + buf * BUF_COLS + c_col0, c_nc, sc, nl + c_col0, c_col0, p.P, jkey - (p.L - p.P));
+          else
+            TRW(1, r = c_cols(tbase + buf * BUF_COLS + c_col0, c_nc, sc, nl + c_col0));
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(tm_empty(buf, 0));
@@ -762,7 +789,7 @@ int score_tc_launch_count(const Shape&) { return 2; }
 size_t score_tc_part_elems(int heads, int rows) { return (size_t)(MAX_GRID + heads) * 4 * rows; }
 
 cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const SplitPlan&, const Workspace& ws,
-                            const float* lse_in, float* imp_out, float* lse_out, cudaStream_t st) {
+                            const float* lse_in, bool causal, float* imp_out, float* lse_out, cudaStream_t st) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return cudaErrorNotSupported;  // no silent fallback: the caller reports NACL_ERR_CUDA
   const int heads = s.batch * s.Hkv;
@@ -793,6 +820,7 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
   p.heads = heads;
   p.n_slots = s.rows <= 128 ? 4 : 2;
   p.phase = 0;
+  p.causal = causal ? 1 : 0; p.P = s.P;
   p.N = (long long)heads * p.T;
   p.scale_log2 = 1.4426950408889634f / sqrtf((float)s.d);
   p.part = ws.part; p.lse_in = lse_in; p.lse_out = lse_out; p.imp = ws.imp; p.imp_out = imp_out;

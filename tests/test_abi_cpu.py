@@ -90,7 +90,7 @@ def test_ex_rejects_wrong_struct_and_unknown_flags(lib):
     p.K, p.V, p.Qproxy, p.out_K, p.out_V, p.out_idx = 0x1000, 0x2000, 0x3000, 0x4000, 0x5000, 0x6000
     p.batch, p.L, p.Hq, p.Hkv, p.d, p.P = 1, 512, 4, 4, 64, 16
     p.budget_proxy, p.budget_random, p.n_sink, p.n_recent = 76, 26, 4, 16
-    p.flags = 1  # CAUSAL: oracle-only for now
+    p.flags = 2 | 4  # both sampling variants at once
     assert lib.nacl_evict_ex(C.byref(p)) == -7
     p.flags = 0x8000
     assert lib.nacl_evict_ex(C.byref(p)) == -7

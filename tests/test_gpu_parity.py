@@ -224,3 +224,16 @@ def test_lse_in_single_sweep(binding, case):
     # and it agrees with the self-contained two-sweep call to the score tolerance
     res2 = binding.nacl_evict_ex(K.cuda(), V.cuda(), Q.cuda(), Bp, Br, ns, nr, 77, 2, want_importance=True)
     np.testing.assert_allclose(res2["importance"].cpu().numpy(), imp, rtol=2e-3, atol=1e-30)
+
+
+@pytest.mark.parametrize("case", [(1, 4100, 32, 8, 128, 64, "bf16"), (2, 1000, 8, 2, 128, 48, "bf16"), (1, 300, 4, 4, 128, 16, "bf16"),
+                                  (2, 333, 4, 2, 64, 5, "f32"), (1, 130, 6, 2, 32, 130, "bf16")],
+                         ids=["tc_GP256_ragged", "tc_GP192", "tc_GP16", "cuda_core_f32", "all_rows_proxy"])
+def test_causal_flag(binding, case):
+    """NACL_FLAG_CAUSAL (R1): proxy row i is prompt position L-P+i and attends keys j <= L-P+i only.  The last
+    case makes every prompt row a proxy row: accumulated causal attention (the H2O one-shot case)."""
+    B, L, Hq, Hkv, d, P, dt = case
+    K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype=dt, seed=L + 3)
+    nr = min(P, L // 2)
+    Bp, Br = max(L // 6, 4 + nr), L // 20
+    full_parity(K, V, Q, Bp, Br, 4, nr, seed=5, layer=1, flags=binding.FLAG_CAUSAL)

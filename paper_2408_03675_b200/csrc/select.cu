@@ -363,22 +363,53 @@ __global__ void __launch_bounds__(ST) nacl_select_kernel(const float* __restrict
 
 // ------------------------------------------------------------------ cluster version
 // Shared state of one CTA.  Every CTA counts its own slice into a histogram in its own shared memory (warp-
-// aggregated), adds the non-empty bins to the head's histogram in global memory (L2 reductions; measured ~10x
-// cheaper than exchanging whole histograms through distributed shared memory), and after ONE cluster barrier per
-// radix pass every CTA reads the merged histogram back and finds the threshold bin itself.  Integer sums: exact
-// and order-independent.  Each pass of each select has its own global histogram, cleared at kernel start.
+// aggregated).  The cluster then finds the bin that holds the K-th largest value in two small exchanges through
+// distributed shared memory instead of merging whole histograms: (1) every CTA pushes the sums of its 64-bin
+// super-bins to all ranks; after a cluster barrier every CTA adds them in rank order and finds the super-bin;
+// (2) every CTA pushes its 64 bin counts of that super-bin; after a second barrier every CTA finds the bin.
+// Integer sums: exact and order-independent.  A buffer is rewritten only after a barrier that every reader reaches
+// after its reads, so single buffers suffice.
+constexpr int kMaxRanks = 16;
 struct ClShared {
   uint32_t hist[HB];
+  uint32_t xsup[kMaxRanks][64];   // [rank][super-bin]: pushed by every rank
+  uint32_t xfine[kMaxRanks][64];  // [rank][bin of the chosen super-bin]
   int warp_tot[32];
   int total;
-  int bin, krem, neq;   // result of a radix pass
-  int cnt[3][8];        // per-rank counts: ties of select 0 / select 1, kept positions
-  int cut[2];           // index of the last tie taken, select 0 / select 1
-  int pad[2];           // sizeof % 16 == 0
+  int sup, bin, krem, neq;        // result of the two steps of a radix pass
+  int cnt[3][kMaxRanks];          // per-rank counts: ties of select 0 / select 1, kept positions
+  int cut[2];                     // index of the last tie taken, select 0 / select 1
+  int pad[1];                     // sizeof % 16 == 0
 };
 static_assert(sizeof(ClShared) % 16 == 0, "the slices behind ClShared stay 16-byte aligned");
-constexpr int kGhWordsPerSelect = 4096 + 1024 + 1024;  // global histogram words per select
-constexpr int kGhWords = 2 * kGhWordsPerSelect;        // ... per head
+
+// Warp 0: x[r][i], r < nrank, i < n (n = 16 or 64) are per-rank counts of n bins in ascending bin order.  Finds the
+// bin that holds the krem-th element counted from the TOP bin; returns (in every lane) its index, the number of
+// elements in higher bins and its own count.
+__device__ __forceinline__ void warp_find_from_top(const uint32_t (*x)[64], int nrank, int n, int krem, int& idx, int& above,
+                                                   int& count) {
+  const int lane = threadIdx.x & 31;
+  int lo = 0, hi = 0;
+  for (int r = 0; r < nrank; ++r) {
+    if (lane < n) lo += (int)x[r][lane];
+    if (lane + 32 < n) hi += (int)x[r][lane + 32];
+  }
+  // inclusive suffix sums (bins >= this lane's bin), the high half first
+  int shi = hi, slo = lo;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int a = __shfl_down_sync(0xffffffffu, shi, o), b = __shfl_down_sync(0xffffffffu, slo, o);
+    if (lane + o < 32) { shi += a; slo += b; }
+  }
+  const int tot_hi = __shfl_sync(0xffffffffu, shi, 0);
+  slo += tot_hi;
+  const unsigned mhi = __ballot_sync(0xffffffffu, shi >= krem), mlo = __ballot_sync(0xffffffffu, slo >= krem);
+  int l, suf, cnt;
+  if (mhi) { l = 31 - __clz(mhi); suf = __shfl_sync(0xffffffffu, shi, l); cnt = __shfl_sync(0xffffffffu, hi, l); idx = 32 + l; }
+  else { l = 31 - __clz(mlo); suf = __shfl_sync(0xffffffffu, slo, l); cnt = __shfl_sync(0xffffffffu, lo, l); idx = l; }
+  above = suf - cnt;
+  count = cnt;
+}
 
 // exclusive prefix sum over the block in thread order (ClShared flavour of block_excl_scan)
 __device__ __forceinline__ int cl_block_excl_scan(int v, ClShared& sh, int& tot) {
@@ -412,19 +443,20 @@ __device__ __forceinline__ int cl_block_excl_scan(int v, ClShared& sh, int& tot)
 // (global index = j0 + i, ascending with the cluster rank), described as
 //   member  <=>  val > thr  ||  (val == thr && j <= cut).
 // Requires 0 <= K <= #valid.  Every thread of every CTA of the cluster calls it with cluster-uniform K.
-// gh = this select's global histograms of the head (zero on entry); which = 0 / 1 (first / second select).
+// which = 0 / 1 (first / second select).
 template <class F>
-__device__ void cluster_radix_select(F getval, int nloc, int j0, int K, ClShared& sh, cg::cluster_group& cluster, uint32_t* gh,
-                                     int which, uint32_t& thr, int& cut) {
+__device__ void cluster_radix_select(F getval, int nloc, int j0, int K, ClShared& sh, cg::cluster_group& cluster, int which,
+                                     uint32_t& thr, int& cut) {
   if (K <= 0) { thr = 0xFFFFFFFFu; cut = -1; return; }
   const unsigned rank = cluster.block_rank(), nrank = cluster.num_blocks();
+  const int lane = threadIdx.x & 31;
   uint32_t prefix = 0, mask = 0;
   int krem = K, n_eq = 0;
 #pragma unroll 1
   for (int pass = 0; pass < 3; ++pass) {
     const int shift = pass == 0 ? 20 : (pass == 1 ? 10 : 0);
     const int nb = pass == 0 ? 4096 : 1024;
-    uint32_t* ghp = gh + (pass == 0 ? 0 : (pass == 1 ? 4096 : 5120));
+    const int nsup = nb / 64;
     for (int i = threadIdx.x; i < nb; i += ST) sh.hist[i] = 0;
     __syncthreads();
     for (int base = 0; base < nloc; base += ST) {  // warp-uniform trip count
@@ -434,37 +466,38 @@ __device__ void cluster_radix_select(F getval, int nloc, int j0, int K, ClShared
       hist_add_aggregated(sh.hist, take, (v >> shift) & (uint32_t)(nb - 1));
     }
     __syncthreads();
-    // thread t owns w consecutive bins, taken from the top: bins nb-1-t*w-(w-1) .. nb-1-t*w
-    const int w = nb / ST;  // 4 or 1
-    int cnt[4] = {0, 0, 0, 0}, sum = 0;
-    const int top = nb - 1 - (int)threadIdx.x * w;
-    if (nrank > 1) {
-#pragma unroll
-      for (int q = 0; q < 4; ++q)
-        if (q < w) { const uint32_t h = sh.hist[top - q]; if (h) atomicAdd(&ghp[top - q], h); }
-      __threadfence();
-      cluster.sync();
-#pragma unroll
-      for (int q = 0; q < 4; ++q)
-        if (q < w) cnt[q] = (int)__ldcg(&ghp[top - q]);
-    } else {
-#pragma unroll
-      for (int q = 0; q < 4; ++q)
-        if (q < w) cnt[q] = (int)sh.hist[top - q];
-    }
-#pragma unroll
-    for (int q = 0; q < 4; ++q) sum += cnt[q];
-    int tot;
-    const int excl = cl_block_excl_scan(sum, sh, tot);
-    if (excl < krem && krem <= excl + sum) {
-      int above = excl;
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        if (q < w) {
-          if (above < krem && krem <= above + cnt[q]) { sh.bin = top - q; sh.krem = krem - above; sh.neq = cnt[q]; }
-          above += cnt[q];
-        }
+    // step 1: sums of 64-bin super-bins (thread t: bins 4t..4t+3, 16 lanes per super-bin), pushed to every rank
+    {
+      int s4 = 0;
+      if ((int)threadIdx.x * 4 < nb) {
+        const uint4 h = *reinterpret_cast<const uint4*>(&sh.hist[threadIdx.x * 4]);
+        s4 = (int)(h.x + h.y + h.z + h.w);
       }
+#pragma unroll
+      for (int o = 8; o > 0; o >>= 1) s4 += __shfl_xor_sync(0xffffffffu, s4, o);
+      const int sb = (int)threadIdx.x >> 4;
+      if ((lane & 15) == 0 && sb < nsup)
+        for (unsigned r = 0; r < nrank; ++r) cluster.map_shared_rank(&sh, r)->xsup[rank][sb] = (uint32_t)s4;
+    }
+    cluster.sync();
+    if (threadIdx.x < 32) {
+      int idx, above, count;
+      warp_find_from_top(sh.xsup, (int)nrank, nsup, krem, idx, above, count);
+      if (lane == 0) { sh.sup = idx; sh.krem = krem - above; }
+    }
+    __syncthreads();
+    const int sup = sh.sup;
+    krem = sh.krem;
+    // step 2: the 64 bin counts of that super-bin, pushed to every rank
+    if (threadIdx.x < 64) {
+      const uint32_t h = sh.hist[sup * 64 + threadIdx.x];
+      for (unsigned r = 0; r < nrank; ++r) cluster.map_shared_rank(&sh, r)->xfine[rank][threadIdx.x] = h;
+    }
+    cluster.sync();
+    if (threadIdx.x < 32) {
+      int idx, above, count;
+      warp_find_from_top(sh.xfine, (int)nrank, 64, krem, idx, above, count);
+      if (lane == 0) { sh.bin = sup * 64 + idx; sh.krem = krem - above; sh.neq = count; }
     }
     __syncthreads();
     prefix |= (uint32_t)sh.bin << shift;
@@ -523,8 +556,7 @@ __device__ __forceinline__ long long sel_gtimer() { long long t; asm volatile("m
 // Dynamic shared memory: ClShared, uint32 ib[Lc] (order-mapped importance), uint32 kb[Lc] (order-mapped keys, later keep flags).
 __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __restrict__ imp, int Hkv, int L, int Lc, int k1, int Br,
                                                                  int n_sink, int n_recent, int C, uint32_t sk0, uint32_t sk1,
-                                                                 uint32_t layer, uint32_t flags, uint32_t* __restrict__ ghist,
-                                                                 int32_t* __restrict__ out_idx) {
+                                                                 uint32_t layer, uint32_t flags, int32_t* __restrict__ out_idx) {
   cg::cluster_group cluster = cg::this_cluster();
   extern __shared__ __align__(16) unsigned char dyn_raw[];
   ClShared& sh = *reinterpret_cast<ClShared*>(dyn_raw);
@@ -541,20 +573,14 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
 
   STAMP(0)
   for (int i = threadIdx.x; i < nloc; i += ST) ib[i] = ordermap(__float_as_uint(row[i]));
-  // this call's global histograms of the head: every CTA clears its share
-  uint32_t* gh = ghist + (size_t)p * kGhWords;
-  if (nrank > 1) {
-    for (int i = (int)rank * ST + (int)threadIdx.x; i < kGhWords; i += (int)nrank * ST) gh[i] = 0;
-    __threadfence();
-  }
-  cluster.sync();  // every CTA of the cluster is running and the global histograms are clear
+  cluster.sync();  // every CTA of the cluster is running: its shared memory may be written
   STAMP(1)
   auto free_pos = [&](int i) { const int j = j0 + i; return j >= lo && j < hi; };
 
   // a4: Proxy-Tokens Eviction, top-k1 of the importance outside the protected set
   uint32_t thr_p;
   int cut_p;
-  cluster_radix_select([&](int i, uint32_t& v) { v = ib[i]; return free_pos(i); }, nloc, j0, k1, sh, cluster, gh, 0, thr_p, cut_p);
+  cluster_radix_select([&](int i, uint32_t& v) { v = ib[i]; return free_pos(i); }, nloc, j0, k1, sh, cluster, 0, thr_p, cut_p);
   auto in_topk = [&](int i) {
     const uint32_t v = ib[i];
     return v > thr_p || (v == thr_p && j0 + i <= cut_p);
@@ -583,7 +609,7 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
   uint32_t thr_r;
   int cut_r;
   cluster_radix_select([&](int i, uint32_t& v) { if (!free_pos(i) || in_topk(i)) return false; v = kb[i]; return true; },
-                       nloc, j0, Br, sh, cluster, gh + kGhWordsPerSelect, 1, thr_r, cut_r);
+                       nloc, j0, Br, sh, cluster, 1, thr_r, cut_r);
 
   STAMP(4)
   // a6: ascending kept-position list: keep flags, then ONE block scan over threads that own consecutive positions,
@@ -630,7 +656,7 @@ cudaError_t launch_keys(const float* imp, uint32_t* key, int batch, int Hkv, int
 // slices of at most this many positions per CTA stay in shared memory (2 x 4 bytes each)
 constexpr int kMaxSlice = 20480;
 
-bool select_uses_cluster(int L) { return (L + 7) / 8 <= kMaxSlice; }
+bool select_uses_cluster(int L) { return (L + kMaxRanks - 1) / kMaxRanks <= kMaxSlice; }
 
 cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, int L, int budget_proxy, int budget_random,
                           int n_sink, int n_recent, uint64_t seed, int layer, uint32_t flags, int32_t* out_idx,
@@ -668,13 +694,15 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   cudaError_t e = cudaFuncSetAttribute(nacl_select_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)(sizeof(ClShared) + (size_t)kMaxSlice * 2 * sizeof(uint32_t)));
   if (e != cudaSuccess) return e;
-  for (int c = 1; c <= 8; c *= 2) {
+  e = cudaFuncSetAttribute(nacl_select_cluster_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);  // clusters of 16
+  if (e != cudaSuccess) return e;
+  for (int c = 1; c <= kMaxRanks; c *= 2) {
     const int lc = ((L + c - 1) / c + 3) / 4 * 4;
     if (lc > kMaxSlice) continue;
     if (c > 1 && L / c < ST / 2) break;  // slices below half a block of positions are not worth a barrier per pass
     const size_t d = sizeof(ClShared) + (size_t)lc * 2 * sizeof(uint32_t);
-    static int active_cache[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};  // [log2 c][smem class]: co-resident clusters
-    const int ci = c == 1 ? 0 : (c == 2 ? 1 : (c == 4 ? 2 : 3)), si = d > 100 * 1024 ? 1 : 0;
+    static int active_cache[5][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}, {0, 0}};  // [log2 c][smem class]: co-resident clusters
+    const int ci = c == 1 ? 0 : (c == 2 ? 1 : (c == 4 ? 2 : (c == 8 ? 3 : 4))), si = d > 100 * 1024 ? 1 : 0;
     int active = active_cache[ci][si];
     if (active == 0) {
       cfg.gridDim = dim3((unsigned)(c * 64));
@@ -696,13 +724,13 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   attr[0].val.clusterDim.x = (unsigned)n;
   StageScope sc(ST_SELECT, st);
   return cudaLaunchKernelEx(&cfg, nacl_select_cluster_kernel, imp, Hkv, L, Lc, k1, budget_random, n_sink, n_recent, C, sk0, sk1,
-                            (uint32_t)layer, flags, key /* scratch: global histograms */, out_idx);
+                            (uint32_t)layer, flags, out_idx);
 }
 
-// 4-byte words of the `key` scratch the select needs (cluster path: global histograms; long-row path: the keys)
+// 4-byte words of the `key` scratch the select needs (long-row path: the keys)
 size_t select_scratch_words(int batch, int Hkv, int L) {
   if (!select_uses_cluster(L)) return (size_t)batch * Hkv * L;
-  return (size_t)batch * Hkv * kGhWords;
+  return 64;  // the cluster path keeps everything in shared memory
 }
 
 }  // namespace nacl

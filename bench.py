@@ -245,6 +245,8 @@ def run_ours(args) -> dict:
 
     # ---- roofline of the dominant kernel
     sab = stage_alg_bytes(cfg)
+    if stages.get("gather", (0, 0))[1] == 0:  # the cluster select kernel also moves the kept rows (steps a4-a7 in one launch)
+        sab["select"] += sab["gather"]
     stage_rows = {}
     for name, (ms, n) in stages.items():
         if n == 0:

@@ -183,10 +183,11 @@ static int evict_impl(const nacl_params_t& p) {
   if (e != cudaSuccess) return fail_cuda(e);
 
   const int C = p.budget_proxy + p.budget_random;
+  bool gathered = false;
   e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
-                    p.flags, p.out_idx, st);
+                    p.flags, p.out_idx, p.K, p.V, p.out_K, p.out_V, row_bytes, &gathered, st);
   if (e != cudaSuccess) return fail_cuda(e);
-  {
+  if (!gathered) {
     StageScope sc(ST_GATHER, st);
     e = launch_gather(p.K, p.V, p.out_idx, p.batch * p.Hkv, p.L, C, row_bytes, p.out_K, p.out_V, st);
   }
@@ -319,7 +320,7 @@ int nacl_launch_count(int dtype, int batch, int L, int Hq, int Hkv, int d, int P
   s.G = Hq / Hkv; s.rows = s.G * P; s.dtype = dtype; s.esize = dtype == NACL_DTYPE_F32 ? 4 : 2;
   const bool tc = !(flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
   // scoring + select (+ a separate keys kernel for very long rows) + gather (budget_random > 0 and C > 0 assumed)
-  return (tc ? score_tc_launch_count(s) : 3) + (select_uses_cluster(L) ? 1 : 2) + 1;
+  return (tc ? score_tc_launch_count(s) : 3) + (select_uses_cluster(L) ? 1 : 3);  // the cluster select also gathers
 }
 
 int nacl_profile_enable(int on) {

@@ -77,8 +77,10 @@ cudaError_t launch_keys(const float* imp, uint32_t* key, int batch, int Hkv, int
 // compaction -> out_idx.  Records its own StageScopes.  `key` is scratch for the long-row fallback.
 bool select_uses_cluster(int L);
 size_t select_scratch_words(int batch, int Hkv, int L);  // 4-byte words of Workspace::key
+// With K/V given and the cluster path taken, the kernel also moves the kept rows (step a7) and sets *gathered.
 cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, int L, int budget_proxy, int budget_random,
                           int n_sink, int n_recent, uint64_t seed, int layer, uint32_t flags, int32_t* out_idx,
+                          const void* K, const void* V, void* out_K, void* out_V, int row_bytes, bool* gathered,
                           cudaStream_t st);
 
 // K,V <- K_S,V_S

@@ -361,6 +361,15 @@ __global__ void __launch_bounds__(ST) nacl_select_kernel(const float* __restrict
   }
 }
 
+#ifdef NACL_SEL_TRACE
+__device__ long long g_sel_trace[16 + 2 * 1024];
+__device__ __forceinline__ long long sel_gtimer() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define STAMP(k) { if (blockIdx.x == 0 && threadIdx.x == 0) g_sel_trace[k] = clock64(); \
+  if (threadIdx.x == 0 && blockIdx.x < 1024 && (k == 0 || k == 5)) g_sel_trace[16 + 2 * blockIdx.x + (k == 5)] = sel_gtimer(); }
+#else
+#define STAMP(k)
+#endif
+
 // ------------------------------------------------------------------ cluster version
 // Shared state of one CTA.  Every CTA counts its own slice into a histogram in its own shared memory (warp-
 // aggregated).  The cluster then finds the bin that holds the K-th largest value in two small exchanges through
@@ -457,8 +466,15 @@ __device__ void cluster_radix_select(F getval, int nloc, int j0, int K, ClShared
     const int shift = pass == 0 ? 20 : (pass == 1 ? 10 : 0);
     const int nb = pass == 0 ? 4096 : 1024;
     const int nsup = nb / 64;
+#ifdef NACL_SEL_TRACE
+#define PSTAMP(k) if (which == 0 && pass == 0 && blockIdx.x == 0 && threadIdx.x == 0) g_sel_trace[8 + k] = clock64();
+#else
+#define PSTAMP(k)
+#endif
+    PSTAMP(0)
     for (int i = threadIdx.x; i < nb; i += ST) sh.hist[i] = 0;
     __syncthreads();
+    PSTAMP(1)
     for (int base = 0; base < nloc; base += ST) {  // warp-uniform trip count
       const int i = base + (int)threadIdx.x;
       uint32_t v = 0;
@@ -466,6 +482,7 @@ __device__ void cluster_radix_select(F getval, int nloc, int j0, int K, ClShared
       hist_add_aggregated(sh.hist, take, (v >> shift) & (uint32_t)(nb - 1));
     }
     __syncthreads();
+    PSTAMP(2)
     // step 1: sums of 64-bin super-bins (thread t: bins 4t..4t+3, 16 lanes per super-bin), pushed to every rank
     {
       int s4 = 0;
@@ -479,13 +496,16 @@ __device__ void cluster_radix_select(F getval, int nloc, int j0, int K, ClShared
       if ((lane & 15) == 0 && sb < nsup)
         for (unsigned r = 0; r < nrank; ++r) cluster.map_shared_rank(&sh, r)->xsup[rank][sb] = (uint32_t)s4;
     }
+    PSTAMP(3)
     cluster.sync();
+    PSTAMP(4)
     if (threadIdx.x < 32) {
       int idx, above, count;
       warp_find_from_top(sh.xsup, (int)nrank, nsup, krem, idx, above, count);
       if (lane == 0) { sh.sup = idx; sh.krem = krem - above; }
     }
     __syncthreads();
+    PSTAMP(5)
     const int sup = sh.sup;
     krem = sh.krem;
     // step 2: the 64 bin counts of that super-bin, pushed to every rank
@@ -493,7 +513,9 @@ __device__ void cluster_radix_select(F getval, int nloc, int j0, int K, ClShared
       const uint32_t h = sh.hist[sup * 64 + threadIdx.x];
       for (unsigned r = 0; r < nrank; ++r) cluster.map_shared_rank(&sh, r)->xfine[rank][threadIdx.x] = h;
     }
+    PSTAMP(6)
     cluster.sync();
+    PSTAMP(7)
     if (threadIdx.x < 32) {
       int idx, above, count;
       warp_find_from_top(sh.xfine, (int)nrank, 64, krem, idx, above, count);
@@ -543,20 +565,13 @@ __device__ void cluster_radix_select(F getval, int nloc, int j0, int K, ClShared
   cut = sh.cut[which];
 }
 
-#ifdef NACL_SEL_TRACE
-__device__ long long g_sel_trace[16 + 2 * 1024];
-__device__ __forceinline__ long long sel_gtimer() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define STAMP(k) { if (blockIdx.x == 0 && threadIdx.x == 0) g_sel_trace[k] = clock64(); \
-  if (threadIdx.x == 0 && blockIdx.x < 1024 && (k == 0 || k == 5)) g_sel_trace[16 + 2 * blockIdx.x + (k == 5)] = sel_gtimer(); }
-#else
-#define STAMP(k)
-#endif
-
 // One cluster per (batch, kv head); CTA `rank` owns positions [rank*Lc, min(L, (rank+1)*Lc)).
 // Dynamic shared memory: ClShared, uint32 ib[Lc] (order-mapped importance), uint32 kb[Lc] (order-mapped keys, later keep flags).
 __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __restrict__ imp, int Hkv, int L, int Lc, int k1, int Br,
                                                                  int n_sink, int n_recent, int C, uint32_t sk0, uint32_t sk1,
-                                                                 uint32_t layer, uint32_t flags, int32_t* __restrict__ out_idx) {
+                                                                 uint32_t layer, uint32_t flags, int32_t* __restrict__ out_idx,
+                                                                 const int4* __restrict__ Kv, const int4* __restrict__ Vv,
+                                                                 int4* __restrict__ oKv, int4* __restrict__ oVv, int vpr) {
   cg::cluster_group cluster = cg::this_cluster();
   extern __shared__ __align__(16) unsigned char dyn_raw[];
   ClShared& sh = *reinterpret_cast<ClShared*>(dyn_raw);
@@ -629,17 +644,42 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
   const int excl = cl_block_excl_scan(mine, sh, tot);
   if (threadIdx.x < nrank) cluster.map_shared_rank(&sh, threadIdx.x)->cnt[2][rank] = tot;
   cluster.sync();  // the last access to another CTA's shared memory lies before this barrier
-  int pos = excl;
-  for (unsigned r = 0; r < rank; ++r) pos += sh.cnt[2][r];
+  int base = 0;  // kept positions of the lower ranks
+  for (unsigned r = 0; r < rank; ++r) base += sh.cnt[2][r];
+  int pos = base + excl;
   int32_t* out = out_idx + (size_t)p * C;
   for (int e = 0; e < E; ++e) {
     const int i = i0 + e;
     if (i < nloc && kb[i]) {
-      if (pos < C) out[pos] = j0 + i;
+      if (pos < C) { out[pos] = j0 + i; ib[pos - base] = (uint32_t)(j0 + i); }  // (ib is free: the keep flags are final)
       ++pos;
     }
   }
   STAMP(5)
+  if (vpr == 0) return;
+  // a7, fused: this CTA moves the K and V rows of the positions IT kept (out rows base .. base+tot), 16-byte vectors,
+  // consecutive threads on consecutive vectors of the output, four vectors of K and of V in flight per thread
+  __syncthreads();
+  const int n_vec = min(tot, C - base) * vpr;
+  const size_t src0 = (size_t)p * L * vpr, dst0 = ((size_t)p * C + base) * vpr;
+  for (int v0 = threadIdx.x; v0 < n_vec; v0 += ST * 4) {
+    size_t src[4];
+    int4 a[4], b[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int v = v0 + u * ST;
+      if (v < n_vec) {
+        const int row = v / vpr;
+        src[u] = src0 + (size_t)ib[row] * vpr + (v - row * vpr);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (v0 + u * ST < n_vec) { a[u] = __ldcs(Kv + src[u]); b[u] = __ldcs(Vv + src[u]); }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (v0 + u * ST < n_vec) { __stcs(oKv + dst0 + v0 + u * ST, a[u]); __stcs(oVv + dst0 + v0 + u * ST, b[u]); }
+  }
 }
 
 }  // namespace
@@ -660,7 +700,9 @@ bool select_uses_cluster(int L) { return (L + kMaxRanks - 1) / kMaxRanks <= kMax
 
 cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, int L, int budget_proxy, int budget_random,
                           int n_sink, int n_recent, uint64_t seed, int layer, uint32_t flags, int32_t* out_idx,
+                          const void* K, const void* V, void* out_K, void* out_V, int row_bytes, bool* gathered,
                           cudaStream_t st) {
+  *gathered = false;
   const int C = budget_proxy + budget_random;
   if (C == 0) return cudaSuccess;
   const int k1 = budget_proxy - n_sink - n_recent;
@@ -724,7 +766,8 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   attr[0].val.clusterDim.x = (unsigned)n;
   StageScope sc(ST_SELECT, st);
   return cudaLaunchKernelEx(&cfg, nacl_select_cluster_kernel, imp, Hkv, L, Lc, k1, budget_random, n_sink, n_recent, C, sk0, sk1,
-                            (uint32_t)layer, flags, out_idx);
+                            (uint32_t)layer, flags, out_idx, (const int4*)K, (const int4*)V, (int4*)out_K, (int4*)out_V,
+                            (*gathered = (K != nullptr)) ? row_bytes / 16 : 0);
 }
 
 // 4-byte words of the `key` scratch the select needs (long-row path: the keys)

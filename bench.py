@@ -261,9 +261,24 @@ def run_ours(args) -> dict:
     roofline = None
     if dom:
         ach = stage_rows[dom]["alg_GBps"]
-        roofline = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                    "frac": round(ach / peaks["hbm_gbs"], 4), "traffic": load_traffic(cfg.name, dom),
-                    "peak_source": peaks["source"], "alg_bytes_per_launch": sab.get(dom, 0)}
+        hbm = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": round(ach / peaks["hbm_gbs"], 4),
+               "alg_bytes_per_launch": sab.get(dom, 0)}
+        roofline = dict(hbm)
+        if dom in ("score_stats", "score_colsum", "score_fused") and cfg.dtype == "bf16":
+            # the scoring sweeps are a dense bf16 contraction as well: 2*B*Hq*P*L*d flop per sweep.  The
+            # kernel is timed inside a long step, so the sustained bf16 figure is the denominator; the roofline reported
+            # is the one the kernel sits closer to
+            flop = 2.0 * cfg.batch * cfg.Hq * cfg.P * cfg.L * cfg.d * (2 if dom == "score_fused" else 1)
+            tf = flop / (stage_rows[dom]["avg_us"] * 1e-6) / 1e12
+            peak_tf = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])
+            tensor = {"bound": "tensor", "achieved": round(tf, 1), "peak": peak_tf, "unit": "TFLOP/s", "frac": round(tf / peak_tf, 4),
+                      "alg_flop_per_launch": flop, "peak_kind": "bf16 dense, sustained (kernel timed inside a long step)"}
+            if tensor["frac"] > hbm["frac"]:
+                roofline = dict(tensor)
+                roofline["hbm"] = hbm
+            else:
+                roofline["tensor"] = tensor
+        roofline.update({"kernel": dom, "traffic": load_traffic(cfg.name, dom), "peak_source": peaks["source"]})
 
     # ---- end to end through the host entry point: pinned host buffers, H2D + D2H inside the timed region
     e2e = run_e2e(binding, cfg, layers, data, Bp, Br, dev, args, world)

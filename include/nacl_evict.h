@@ -48,8 +48,9 @@
  * validation error.  Validation is host-side and never reads device memory.
  *
  * Supported: 1 <= P <= L <= 2^24; Hq % Hkv == 0; d a multiple of 16, d <= 256; any L (ragged
- * last tile is masked).  The tensor-core path (tcgen05 + TMA) serves bf16, d == 128,
- * G*P <= 256; every other shape runs the generic CUDA-core kernels of the same library.
+ * last tile is masked).  The tensor-core path (tcgen05 + TMA) serves bf16, d == 128 and
+ * G*P a multiple of 16 up to 256 or a multiple of 256 (blocks of 256 proxy rows); every other shape runs the generic
+ * CUDA-core kernels of the same library.
  */
 #ifndef NACL_EVICT_H
 #define NACL_EVICT_H

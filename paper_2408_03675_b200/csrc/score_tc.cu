@@ -83,7 +83,8 @@ __device__ __forceinline__ long long gtimer_ns() { long long t; asm volatile("mo
 #endif
 
 struct TcParams {
-  int L, rows, T;          // keys per head, proxy rows per kv head (G*P), key tiles per head
+  int L, rows, T;          // keys per head, proxy rows per row block (G*P, or 256 when G*P > 256), key tiles per head
+  int rows_total, nrb;     // G*P and the number of 256-row blocks (1 unless G*P > 256)
   int heads, n_slots;      // n_slots: epilogue warps that share a proxy row in sweep S = partials per (row, piece): 2 if rows > 128, else 4
   int phase;               // 0 = sweep S (statistics), 1 = sweep C (column sums)
   int causal, P;           // NACL_FLAG_CAUSAL: proxy row r (i = r % P, prompt position L-P+i) sees keys j <= L-P+i
@@ -287,10 +288,13 @@ __device__ __forceinline__ uint32_t umma_idesc(int M, int N) {
 
 // ------------------------------------------------------------------ the static schedule
 // CTA c owns the flat tiles [N*c/G, N*(c+1)/G); sweep S walks them upwards, sweep C downwards.
-struct Seg { int head, tile, n; };  // n tiles of `head`: tile, tile+step, ... (step = +1 in sweep S, -1 in sweep C)
+// G*P > 256 (a multiple of 256): the proxy rows of a kv head are taken in blocks of 256; every segment is walked once per
+// row block (rb = 0, 1, ...), its K tiles coming from L2 after the first time.
+struct Seg { int head, tile, n, rb; };  // n tiles of `head`: tile, tile+step, ... (step = +1 in sweep S, -1 in sweep C); row block rb
 struct Walk {
   long long t;
-  int remaining, step, T;
+  int remaining, step, T, nrb, rb;
+  Seg cur;
   __device__ Walk(const TcParams& p) {
     const long long G = gridDim.x, c = blockIdx.x;
     const long long t0 = p.N * c / G, t1 = p.N * (c + 1) / G;
@@ -298,15 +302,25 @@ struct Walk {
     step = p.phase ? -1 : 1;
     t = p.phase ? t1 - 1 : t0;
     T = p.T;
+    nrb = p.nrb;
+    rb = nrb;  // "current segment exhausted"
   }
   __device__ bool next(Seg& s) {
+    if (rb < nrb) {  // the same tiles again, next row block
+      cur.rb = rb++;
+      s = cur;
+      return true;
+    }
     if (remaining <= 0) return false;
-    s.head = (int)(t / T);
-    s.tile = (int)(t - (long long)s.head * T);
-    const int room = step > 0 ? T - s.tile : s.tile + 1;
-    s.n = remaining < room ? remaining : room;
-    t += (long long)step * s.n;
-    remaining -= s.n;
+    cur.head = (int)(t / T);
+    cur.tile = (int)(t - (long long)cur.head * T);
+    const int room = step > 0 ? T - cur.tile : cur.tile + 1;
+    cur.n = remaining < room ? remaining : room;
+    cur.rb = 0;
+    rb = 1;
+    t += (long long)step * cur.n;
+    remaining -= cur.n;
+    s = cur;
     return true;
   }
 };
@@ -518,8 +532,8 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
       const uint32_t qdst = sbase + SM::OFF_Q + qb * SM::Q_BYTES;
       if (leader) {
         mbar_expect_tx(q_full(qb), SM::Q_BYTES);
-        tma_load_2d(qdst, &tmQ, 0, sg.head * p.rows, q_full(qb));
-        tma_load_2d(qdst + QROWS * 128, &tmQ, 64, sg.head * p.rows, q_full(qb));
+        tma_load_2d(qdst, &tmQ, 0, sg.head * p.rows_total + sg.rb * 256, q_full(qb));
+        tma_load_2d(qdst + QROWS * 128, &tmQ, 64, sg.head * p.rows_total + sg.rb * 256, q_full(qb));
       }
       ++qrun;
       for (int i = 0; i < sg.n; ++i) {
@@ -621,8 +635,10 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
           for (int u = 0; u < 4; ++u) {
             const int key = lane + 32 * u;
             if (j0 + key < p.L) {
-              p.imp[o + key] = r[u];
-              if (p.imp_out) p.imp_out[o + key] = r[u];
+              // later row blocks add onto the sum of the earlier ones (same thread, same order every run)
+              const float v = sg.rb == 0 ? r[u] : p.imp[o + key] + r[u];
+              p.imp[o + key] = v;
+              if (p.imp_out) p.imp_out[o + key] = v;
             }
           }
         }
@@ -660,7 +676,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
           const bool ctile = p.causal && (sg.tile + i) * TILE + TILE - 1 > p.L - p.P;
           TRW(1, if (live) {
             const uint32_t ta = tbase + buf * BUF_COLS + s_half * 128 + s_col0;
-            if (ctile) s_cols_masked(ta, s_nc, sc, valid, min(valid, valid - p.P + 1 + s_row % p.P), m0, z0);
+            if (ctile) s_cols_masked(ta, s_nc, sc, valid, min(valid, valid - p.P + 1 + (sg.rb * 256 + s_row) % p.P), m0, z0);
             else if (valid >= s_nc) { if (n_half == 2) s_cols<64>(ta, sc, m0, z0); else s_cols<32>(ta, sc, m0, z0); }
             else s_cols_masked(ta, s_nc, sc, valid, valid, m0, z0);
           })
@@ -670,7 +686,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
         }
         // this warp's partial of the piece; (-inf, 0) when it saw no valid key
         if (s_row < p.rows)
-          __stcg(&p.part[(((size_t)blockIdx.x + sg.head) * p.n_slots + s_slot) * p.rows + s_row], make_float2(m0, z0));
+          __stcg(&p.part[(((size_t)blockIdx.x + sg.head) * p.n_slots + s_slot) * p.rows_total + sg.rb * 256 + s_row], make_float2(m0, z0));
       } else {
         // ---------------- C segment: merge the head's partials (ascending piece order) into -lse, then column sums
         const int ls = nseg % LSE_SLOTS;
@@ -680,16 +696,16 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
           if (r < p.rows) {
             float l2;
             if (p.lse_in) {
-              l2 = p.lse_in[(size_t)sg.head * p.rows + r] * 1.4426950408889634f;  // given (natural log) -> log2 domain
+              l2 = p.lse_in[(size_t)sg.head * p.rows_total + sg.rb * 256 + r] * 1.4426950408889634f;  // given (natural log) -> log2 domain
             } else {
               const int c_first = cta_of_tile((long long)sg.head * p.T, p.N, G);
               const int c_last = cta_of_tile((long long)(sg.head + 1) * p.T - 1, p.N, G);
-              l2 = merge_row(p.part + ((size_t)(c_first + sg.head) * p.n_slots) * p.rows + r, (c_last - c_first + 1) * p.n_slots,
-                             (size_t)p.rows);
+              l2 = merge_row(p.part + ((size_t)(c_first + sg.head) * p.n_slots) * p.rows_total + sg.rb * 256 + r,
+                             (c_last - c_first + 1) * p.n_slots, (size_t)p.rows_total);
             }
             nl[r] = -l2;
             // the CTA that owns the head's first tile publishes lse
-            if (p.lse_out && sg.tile - (sg.n - 1) == 0) p.lse_out[(size_t)sg.head * p.rows + r] = l2 * 0.69314718055994530942f;
+            if (p.lse_out && sg.tile - (sg.n - 1) == 0) p.lse_out[(size_t)sg.head * p.rows_total + sg.rb * 256 + r] = l2 * 0.69314718055994530942f;
           }
         })
         TRW(3, asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory"));
@@ -701,7 +717,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
           float r;
           const int jkey = (sg.tile - i) * TILE + quarter * 32 + lane;  // the key this thread owns
           if (p.causal && (sg.tile - i) * TILE + TILE - 1 > p.L - p.P)
-            r = c_cols_causal(tbase + buf * BUF_COLS + c_col0, c_nc, sc, nl + c_col0, c_col0, p.P, jkey - (p.L - p.P));
+            r = c_cols_causal(tbase + buf * BUF_COLS + c_col0, c_nc, sc, nl + c_col0, sg.rb * 256 + c_col0, p.P, jkey - (p.L - p.P));
           else
             TRW(1, r = c_cols(tbase + buf * BUF_COLS + c_col0, c_nc, sc, nl + c_col0));
           tc_fence_before();
@@ -781,7 +797,8 @@ cudaError_t launch_cfg(const CUtensorMap& tmK, const CUtensorMap& tmQ, TcParams 
 }  // namespace
 
 bool score_tc_supported(const Shape& s) {
-  return s.dtype == NACL_DTYPE_BF16 && s.d == HD && s.rows % 16 == 0 && s.rows >= 16 && s.rows <= 256;
+  return s.dtype == NACL_DTYPE_BF16 && s.d == HD && s.rows % 16 == 0 && s.rows >= 16 &&
+         (s.rows <= 256 || (s.rows % 256 == 0 && s.rows <= 8192));  // larger G*P: blocks of 256 proxy rows
 }
 
 int score_tc_launch_count(const Shape&) { return 2; }
@@ -816,7 +833,8 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
   }
 
   TcParams p;
-  p.L = s.L; p.rows = s.rows; p.T = (s.L + TILE - 1) / TILE;
+  p.L = s.L; p.rows = s.rows <= 256 ? s.rows : 256; p.T = (s.L + TILE - 1) / TILE;
+  p.rows_total = s.rows; p.nrb = (s.rows + 255) / 256;
   p.heads = heads;
   p.n_slots = s.rows <= 128 ? 4 : 2;
   p.phase = 0;

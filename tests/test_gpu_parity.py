@@ -58,6 +58,8 @@ RAGGED = [
     (1, 129, 6, 2, 32, 3, "bf16", 20, 5, 1, 3),           # small d, odd G*P -> CUDA-core path
     (3, 515, 2, 1, 256, 7, "f32", 64, 16, 2, 7),          # d = 256
     (1, 5000, 16, 16, 128, 48, "bf16", 750, 250, 4, 48),  # G*P = 48
+    (1, 1500, 8, 2, 128, 128, "bf16", 300, 75, 4, 128),   # G*P = 512: two 256-row blocks on the tensor-core path
+    (2, 900, 6, 2, 128, 256, "bf16", 300, 45, 4, 256),    # G*P = 768: three row blocks, P = 256 proxy rows
 ]
 
 
@@ -199,8 +201,9 @@ def test_gumbel_keys_bitwise_against_the_oracle(binding, flag_name):
     print(f"{flag_name}: {n_diff} of {a.size} keys differ by 1 ulp")
 
 
-@pytest.mark.parametrize("case", [(1, 4100, 32, 8, 128, 64, "bf16"), (2, 1500, 8, 4, 128, 16, "bf16"), (2, 700, 4, 2, 64, 5, "f32")],
-                         ids=["tc_GP256", "tc_GP32", "cuda_core_f32"])
+@pytest.mark.parametrize("case", [(1, 4100, 32, 8, 128, 64, "bf16"), (2, 1500, 8, 4, 128, 16, "bf16"), (2, 700, 4, 2, 64, 5, "f32"),
+                                  (1, 1100, 8, 2, 128, 128, "bf16")],
+                         ids=["tc_GP256", "tc_GP32", "cuda_core_f32", "tc_GP512_row_blocks"])
 def test_lse_in_single_sweep(binding, case):
     """SURVEY.md 8(f) f1 / the contract of the paper's Algorithm 2: with the row log-sum-exps
     supplied, one logit sweep gives the same importance (north-star tolerance) and, on it, exactly the oracle's selection."""
@@ -227,8 +230,8 @@ def test_lse_in_single_sweep(binding, case):
 
 
 @pytest.mark.parametrize("case", [(1, 4100, 32, 8, 128, 64, "bf16"), (2, 1000, 8, 2, 128, 48, "bf16"), (1, 300, 4, 4, 128, 16, "bf16"),
-                                  (2, 333, 4, 2, 64, 5, "f32"), (1, 130, 6, 2, 32, 130, "bf16")],
-                         ids=["tc_GP256_ragged", "tc_GP192", "tc_GP16", "cuda_core_f32", "all_rows_proxy"])
+                                  (2, 333, 4, 2, 64, 5, "f32"), (1, 130, 6, 2, 32, 130, "bf16"), (1, 1300, 8, 2, 128, 128, "bf16")],
+                         ids=["tc_GP256_ragged", "tc_GP192", "tc_GP16", "cuda_core_f32", "all_rows_proxy", "tc_GP512_row_blocks"])
 def test_causal_flag(binding, case):
     """NACL_FLAG_CAUSAL (R1): proxy row i is prompt position L-P+i and attends keys j <= L-P+i only.  The last
     case makes every prompt row a proxy row: accumulated causal attention (the H2O one-shot case)."""

@@ -53,7 +53,7 @@ SplitPlan make_split_plan(int batch, int L, int Hkv) {
   if (per_head < 1) per_head = 1;
   long chunk = ((long)L + per_head - 1) / per_head;
   chunk = (chunk + 127) / 128 * 128;
-  if (chunk < 512) chunk = 512;
+  if (chunk < 128) chunk = 128;
   SplitPlan sp;
   sp.chunk = (int)chunk;
   sp.n_chunks = (int)(((long)L + chunk - 1) / chunk);

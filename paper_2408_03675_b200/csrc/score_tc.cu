@@ -30,7 +30,7 @@
 //             and a combiner warp adds them in a fixed order (deterministic) and stores imp.
 //
 // Epilogue arithmetic.  At G*P = 256 the path is bound by the 16/clk/SM MUFU.EX2 unit and the FMA
-// pipe, not by HBM (profiles/): half of the exponentials are therefore evaluated on the FMA pipe
+// pipe, not by HBM (profiles/): a quarter of the exponentials are therefore evaluated on the FMA pipe
 // (Cody-Waite range reduction + degree-3 minimax polynomial, relative error <= 7.5e-5, against the
 // 2e-3 score tolerance of the north star) and all multiply-adds are the packed fma/add.f32x2 forms.
 //
@@ -64,7 +64,7 @@ constexpr int N_CS = 4;                        // shared-memory buffers for the 
 constexpr int MAX_GRID = kNumSMs;              // the partial-statistics workspace is sized for this many CTAs
 constexpr uint32_t SPIN_LIMIT = 1u << 26;      // watchdog: a wait that long is a bug -> trap (loud failure)
 #ifndef NACL_POLY_MASK
-#define NACL_POLY_MASK 0x2Au
+#define NACL_POLY_MASK 0x22u
 #endif
 constexpr uint32_t POLY_MASK = NACL_POLY_MASK;  // which of every 8 element pairs take the FMA-pipe exp2 (bit e&7)
 

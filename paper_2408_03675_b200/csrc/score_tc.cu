@@ -329,14 +329,16 @@ __device__ __forceinline__ int cta_of_tile(long long t, long long N, long long G
 
 // ------------------------------------------------------------------ shared-memory carve-up
 constexpr int LSE_SLOTS = 2;
-template <int QROWS, int NQ, int STAGES>
+// PH = the sweep the instantiation serves: sweep S needs neither the lse nor the column-sum buffers and spends the
+// space on one more K stage
+template <int QROWS, int NQ, int STAGES, int PH>
 struct Smem {
   static constexpr int Q_BYTES = QROWS * HD * 2;
   static constexpr int OFF_Q = 0;
   static constexpr int OFF_K = OFF_Q + NQ * Q_BYTES;
   static constexpr int OFF_LSE = OFF_K + STAGES * KSTAGE_BYTES;   // float[LSE_SLOTS][256]: -lse (log2 domain) of the segment's head
-  static constexpr int OFF_CS = OFF_LSE + LSE_SLOTS * 256 * 4;    // float[N_CS][4][128]: quarter column sums of a C tile
-  static constexpr int OFF_BARS = OFF_CS + N_CS * 4 * TILE * 4;
+  static constexpr int OFF_CS = OFF_LSE + (PH ? LSE_SLOTS * 256 * 4 : 0);    // float[N_CS][4][128]: quarter column sums of a C tile
+  static constexpr int OFF_BARS = OFF_CS + (PH ? N_CS * 4 * TILE * 4 : 0);
   static constexpr int N_BARS = 2 * STAGES + 2 * NQ + 4 * N_BUFS + 2 * N_CS;
   static constexpr int OFF_TMEM = OFF_BARS + N_BARS * 8;
   static constexpr int TOTAL = OFF_TMEM + 8;
@@ -475,10 +477,10 @@ __device__ __noinline__ float c_cols_causal(uint32_t taddr, int nc, float sc, co
 }
 
 // ------------------------------------------------------------------ the kernel
-template <int QROWS, int NQ, int STAGES>
+template <int QROWS, int NQ, int STAGES, int PH>
 __global__ void __launch_bounds__(NTHREADS, 1)
 nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmQ, const TcParams p) {
-  using SM = Smem<QROWS, NQ, STAGES>;
+  using SM = Smem<QROWS, NQ, STAGES, PH>;
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t sbase = smem_u32(smem);
   if ((sbase & 1023u) != 0) __trap();  // the 128B-swizzled operand tiles need 1024-byte alignment
@@ -779,25 +781,28 @@ int sm_count() {
   return n;
 }
 
-template <int QROWS, int NQ, int STAGES>
+template <int QROWS, int NQ, int STAGES_S, int STAGES_C>
 cudaError_t launch_cfg(const CUtensorMap& tmK, const CUtensorMap& tmQ, TcParams p, cudaStream_t st) {
-  using SM = Smem<QROWS, NQ, STAGES>;
-  static_assert(SM::TOTAL <= 227 * 1024, "shared memory budget");
-  auto kern = nacl_score_tc_kernel<QROWS, NQ, STAGES>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::TOTAL);
+  using SMS = Smem<QROWS, NQ, STAGES_S, 0>;
+  using SMC = Smem<QROWS, NQ, STAGES_C, 1>;
+  static_assert(SMS::TOTAL <= 227 * 1024 && SMC::TOTAL <= 227 * 1024, "shared memory budget");
+  auto kern_s = nacl_score_tc_kernel<QROWS, NQ, STAGES_S, 0>;
+  auto kern_c = nacl_score_tc_kernel<QROWS, NQ, STAGES_C, 1>;
+  cudaError_t e = cudaFuncSetAttribute(kern_s, cudaFuncAttributeMaxDynamicSharedMemorySize, SMS::TOTAL);
   if (e != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(kern_c, cudaFuncAttributeMaxDynamicSharedMemorySize, SMC::TOTAL)) != cudaSuccess) return e;
   long long grid = sm_count() < MAX_GRID ? sm_count() : MAX_GRID;
   if (p.N < grid) grid = p.N;
   if (!p.lse_in) {
     StageScope sc(ST_STATS, st);
     p.phase = 0;
-    kern<<<(int)grid, NTHREADS, SM::TOTAL, st>>>(tmK, tmQ, p);
+    kern_s<<<(int)grid, NTHREADS, SMS::TOTAL, st>>>(tmK, tmQ, p);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
   }
   {
     StageScope sc(ST_COLSUM, st);
     p.phase = 1;
-    kern<<<(int)grid, NTHREADS, SM::TOTAL, st>>>(tmK, tmQ, p);
+    kern_c<<<(int)grid, NTHREADS, SMC::TOTAL, st>>>(tmK, tmQ, p);
     e = cudaGetLastError();
   }
   return e;
@@ -852,8 +857,8 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
   p.scale_log2 = 1.4426950408889634f / sqrtf((float)s.d);
   p.part = ws.part; p.lse_in = lse_in; p.lse_out = lse_out; p.imp = ws.imp; p.imp_out = imp_out;
 
-  if (qrows == 128) return launch_cfg<128, 2, 4>(tmK, tmQ, p, st);
-  return launch_cfg<256, 1, 4>(tmK, tmQ, p, st);
+  if (qrows == 128) return launch_cfg<128, 2, 5, 4>(tmK, tmQ, p, st);
+  return launch_cfg<256, 1, 5, 4>(tmK, tmQ, p, st);
 }
 
 }  // namespace nacl

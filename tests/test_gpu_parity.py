@@ -240,3 +240,13 @@ def test_causal_flag(binding, case):
     nr = min(P, L // 2)
     Bp, Br = max(L // 6, 4 + nr), L // 20
     full_parity(K, V, Q, Bp, Br, 4, nr, seed=5, layer=1, flags=binding.FLAG_CAUSAL)
+
+
+@pytest.mark.parametrize("case", [(1, 200000, 2, 1, 64, 8, "bf16"), (1, 330001, 1, 1, 64, 4, "bf16"), (2, 70000, 8, 2, 128, 32, "bf16")],
+                         ids=["one_head_200k_cluster16", "row_too_long_for_a_cluster", "tc_70k_cluster8"])
+def test_long_rows(binding, case):
+    """Rows of 70k-330k keys: the largest cluster sizes of the select kernel and, past 16 x 20480 keys, the fallback
+    with a separate keys kernel, a single-CTA select working out of global memory and the stand-alone gather."""
+    B, L, Hq, Hkv, d, P, dt = case
+    K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype=dt, seed=L % 1000)
+    full_parity(K, V, Q, L // 8, L // 40, 4, P, seed=L, layer=7)

@@ -305,7 +305,7 @@ def run_ours(args) -> dict:
         "library": os.path.relpath(binding.library_path(), ROOT),
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = run_cpu_sample(cfg, max_seconds=12.0, max_layers=4)
+        out["cpu_baseline"] = run_cpu_sample(cfg, max_seconds=15.0, max_layers=10)
     else:
         out["cpu_baseline"] = None
     nacl_dist.finalize()

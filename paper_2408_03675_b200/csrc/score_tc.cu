@@ -345,6 +345,27 @@ struct Smem {
 };
 
 // ------------------------------------------------------------------ epilogue helpers
+// max of 32 raw logits (3-input max, two chains)
+__device__ __forceinline__ float s_max32(const uint32_t (&v)[32]) {
+  float g0 = __uint_as_float(v[0]), g1 = __uint_as_float(v[1]);
+#pragma unroll
+  for (int e = 2; e < 30; e += 4) {
+    g0 = max3(g0, __uint_as_float(v[e]), __uint_as_float(v[e + 2]));
+    g1 = max3(g1, __uint_as_float(v[e + 1]), __uint_as_float(v[e + 3]));
+  }
+  return max3(g0, g1, fmaxf(__uint_as_float(v[30]), __uint_as_float(v[31])));
+}
+// (a0, a1) += 2^(v*sc - m_ref) over 32 columns, packed; some pairs on the FMA pipe (POLY_MASK)
+__device__ __forceinline__ void s_acc32(const uint32_t (&v)[32], float sc, float m_ref, u64& a0, u64& a1) {
+  const u64 sc2 = pack2(sc, sc), nm2 = pack2(-m_ref, -m_ref);
+#pragma unroll
+  for (int e = 0; e < 16; e += 2) {
+    const u64 x0 = fma2(pack2u(v[2 * e + 0], v[2 * e + 1]), sc2, nm2);
+    const u64 x1 = fma2(pack2u(v[2 * e + 2], v[2 * e + 3]), sc2, nm2);
+    a0 = add2(a0, pair_on_fma_pipe(e) ? exp2_poly2(x0) : exp2_mufu2(x0));
+    a1 = add2(a1, pair_on_fma_pipe(e + 1) ? exp2_poly2(x1) : exp2_mufu2(x1));
+  }
+}
 // one 32-column segment of an S tile: online (max, sum-exp) update of the row this thread owns
 __device__ __forceinline__ void s_update(const uint32_t (&v)[32], float sc, float& m, float& z) {
 #ifdef NACL_EPI_TRIVIAL  // diagnostics: pipeline ceiling without the exponentials (results are wrong)
@@ -354,22 +375,25 @@ __device__ __forceinline__ void s_update(const uint32_t (&v)[32], float sc, floa
   z += t0 * sc; m = 0.f;
   return;
 #endif
-  float g0 = __uint_as_float(v[0]), g1 = __uint_as_float(v[1]);
-#pragma unroll
-  for (int e = 2; e < 30; e += 4) {
-    g0 = max3(g0, __uint_as_float(v[e]), __uint_as_float(v[e + 2]));
-    g1 = max3(g1, __uint_as_float(v[e + 1]), __uint_as_float(v[e + 3]));
-  }
-  const float m_new = fmaxf(m, max3(g0, g1, fmaxf(__uint_as_float(v[30]), __uint_as_float(v[31]))) * sc);
-  const u64 sc2 = pack2(sc, sc), nm2 = pack2(-m_new, -m_new);
+  const float m_new = fmaxf(m, s_max32(v) * sc);
   u64 a0 = 0ull, a1 = 0ull;
-#pragma unroll
-  for (int e = 0; e < 16; e += 2) {
-    const u64 x0 = fma2(pack2u(v[2 * e + 0], v[2 * e + 1]), sc2, nm2);
-    const u64 x1 = fma2(pack2u(v[2 * e + 2], v[2 * e + 3]), sc2, nm2);
-    a0 = add2(a0, pair_on_fma_pipe(e) ? exp2_poly2(x0) : exp2_mufu2(x0));
-    a1 = add2(a1, pair_on_fma_pipe(e + 1) ? exp2_poly2(x1) : exp2_mufu2(x1));
-  }
+  s_acc32(v, sc, m_new, a0, a1);
+  float s0, s1;
+  unpack2(add2(a0, a1), s0, s1);
+  z = fmaf(z, fast_exp2(m - m_new), s0 + s1);
+  m = m_new;
+}
+// 64 columns at once: one running-max update and one rescale for both register blocks
+__device__ __forceinline__ void s_update64(const uint32_t (&va)[32], const uint32_t (&vb)[32], float sc, float& m, float& z) {
+#ifdef NACL_EPI_TRIVIAL
+  s_update(va, sc, m, z);
+  s_update(vb, sc, m, z);
+  return;
+#endif
+  const float m_new = fmaxf(m, fmaxf(s_max32(va), s_max32(vb)) * sc);
+  u64 a0 = 0ull, a1 = 0ull;
+  s_acc32(va, sc, m_new, a0, a1);
+  s_acc32(vb, sc, m_new, a0, a1);
   float s0, s1;
   unpack2(add2(a0, a1), s0, s1);
   z = fmaf(z, fast_exp2(m - m_new), s0 + s1);
@@ -392,8 +416,8 @@ __device__ __forceinline__ void s_cols(uint32_t taddr, float sc, uint32_t empty_
   tc_wait_ld(va);
   if (NC == 64) tc_wait_ld(vb);
   release_tmem(empty_bar);
-  s_update(va, sc, m, z);
-  if (NC == 64) s_update(vb, sc, m, z);
+  if (NC == 64) s_update64(va, vb, sc, m, z);
+  else s_update(va, sc, m, z);
 }
 
 // last tile of a head: columns >= valid (relative to taddr) are keys past L and must not exist (-inf)

@@ -479,6 +479,7 @@ __device__ void cluster_radix_select(F getval, int nloc, int j0, int K, ClShared
       const int i = base + (int)threadIdx.x;
       uint32_t v = 0;
       const bool take = i < nloc && getval(i, v) && (v & mask) == prefix;
+      if (pass > 0 && !__any_sync(0xffffffffu, take)) continue;  // later digits: most warps hold no element of the bin
       hist_add_aggregated(sh.hist, take, (v >> shift) & (uint32_t)(nb - 1));
     }
     __syncthreads();

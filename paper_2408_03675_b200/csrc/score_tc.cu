@@ -51,15 +51,11 @@ constexpr int BOX_BYTES = 128 * 128;           // one TMA box: 128 rows x 64 bf1
 constexpr int KSTAGE_BYTES = 2 * BOX_BYTES;    // a K tile = two boxes (d 0..63, d 64..127)
 constexpr int N_EPI_WARPS = 16;
 constexpr int EPI_THREADS = N_EPI_WARPS * 32;
-constexpr int W_TMA = 16, W_MMA = 17, W_CMB = 18;  // warp roles after the epilogue warps
-constexpr int NTHREADS = EPI_THREADS + 3 * 32;
+constexpr int W_TMA = 16, W_MMA = 17, W_MMA2 = 18, W_CMB = 19;  // warp roles after the epilogue warps
+constexpr int NTHREADS = EPI_THREADS + 4 * 32;
 constexpr int TMEM_COLS = 512;
 constexpr int N_BUFS = 2;                      // TMEM accumulator buffers (one tile each)
 constexpr int BUF_COLS = 256;                  // TMEM columns per accumulator buffer
-#ifndef NACL_S_HALF_BARRIERS
-#define NACL_S_HALF_BARRIERS 0
-#endif
-constexpr bool kHalfBarriers = NACL_S_HALF_BARRIERS != 0;  // sweep S: full/empty barriers per 128-row half instead of per tile
 constexpr int N_CS = 4;                        // shared-memory buffers for the quarter column sums of a C tile
 constexpr int MAX_GRID = kNumSMs;              // the partial-statistics workspace is sized for this many CTAs
 constexpr uint32_t SPIN_LIMIT = 1u << 26;      // watchdog: a wait that long is a bug -> trap (loud failure)
@@ -71,15 +67,24 @@ constexpr uint32_t POLY_MASK = NACL_POLY_MASK;  // which of every 8 element pair
 // Optional wait/compute cycle accounting per warp role (diagnostics build only: -DNACL_TC_TRACE).
 #ifdef NACL_TC_TRACE
 #define TR_N 8
-__device__ long long g_trace[2][160][19][TR_N];
+__device__ long long g_trace[2][160][20][TR_N];
 __device__ __forceinline__ long long gtimer_ns() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
 #define TR_DECL long long tr_[TR_N]; for (int i_ = 0; i_ < TR_N; ++i_) tr_[i_] = 0; const long long tr_start_ = clock64(); const long long tr_ns_ = gtimer_ns();
 #define TRW(cat, ...) { const long long t_ = clock64(); __VA_ARGS__; tr_[cat] += clock64() - t_; }
-#define TR_FLUSH() { tr_[TR_N - 1] = clock64() - tr_start_; tr_[TR_N - 2] = gtimer_ns() - tr_ns_; if (lane == 0 && blockIdx.x < 160) for (int i_ = 0; i_ < TR_N; ++i_) g_trace[p.phase][blockIdx.x][warp][i_] = tr_[i_]; }
+__device__ long long g_tl[2][20][32][8];
+#define TL(k) { if (blockIdx.x == 40 && lane == 0 && tl_i_ >= 0 && tl_i_ < 32) g_tl[PH][warp][tl_i_][k] = clock64(); }
+#define TL_NEXT() { ++tl_i_; }
+#define TL_DECL int tl_i_ = -8;
+#define TL2(k) { if (blockIdx.x == 40 && (threadIdx.x & 31) == 0 && tl_i_ >= 0 && tl_i_ < 32) g_tl[0][threadIdx.x >> 5][tl_i_][k] = clock64(); }
+#define TR_FLUSH() { tr_[TR_N - 1] = clock64() - tr_start_; tr_[TR_N - 2] = gtimer_ns() - tr_ns_; if (lane == 0 && blockIdx.x < 160) for (int i_ = 0; i_ < TR_N; ++i_) g_trace[PH][blockIdx.x][warp][i_] = tr_[i_]; }
 #else
 #define TR_DECL
 #define TRW(cat, ...) { __VA_ARGS__; }
 #define TR_FLUSH()
+#define TL(k)
+#define TL_NEXT()
+#define TL_DECL
+#define TL2(k)
 #endif
 
 struct TcParams {
@@ -114,6 +119,19 @@ __device__ __forceinline__ uint32_t mbar_try_wait(uint32_t a, uint32_t parity) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
       "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(a), "r"(parity)
+      : "memory");
+  return ok;
+}
+// non-blocking probe: the predicate comes back after the barrier unit's latency, which overlaps with whatever the
+// caller issues before it looks at the result
+__device__ __forceinline__ uint32_t mbar_test(uint32_t a, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
       "selp.u32 %0, 1, 0, p;\n\t}"
       : "=r"(ok)
       : "r"(a), "r"(parity)
@@ -234,11 +252,12 @@ __device__ __forceinline__ u64 exp2_mufu2(u64 x) {
 }
 // (2^x0, 2^x1) on the FMA pipe, x <= ~0: n = floor(x) by a round-down add of 1.5*2^23, f = x - n in [0,1),
 // 2^f by a degree-3 minimax polynomial (relative error <= 7.5e-5), 2^n by an add into the exponent field.
-// x is clamped at -125 (2^-125 ~ 2e-38 stands for zero; keeps the exponent field from wrapping).
+// x is clamped to [-125, 127] (2^-125 ~ 2e-38 stands for zero, 2^127 for "too large": the exponent field must not wrap;
+// sweep S treats a sum >= 2^100 as the signal to take a new reference, see s_lazy32).
 __device__ __forceinline__ u64 exp2_poly2(u64 x) {
   float a, b;
   unpack2(x, a, b);
-  x = pack2(fmaxf(a, -125.f), fmaxf(b, -125.f));
+  x = pack2(fminf(fmaxf(a, -125.f), 127.f), fminf(fmaxf(b, -125.f), 127.f));
   const u64 magic = pack2(12582912.f, 12582912.f);
   const u64 fi = add2_rm(x, magic);
   const u64 f = sub2(x, sub2(fi, magic));
@@ -400,6 +419,29 @@ __device__ __forceinline__ void s_update64(const uint32_t (&va)[32], const uint3
   m = m_new;
 }
 
+// Lazy reference (sweep S, full tiles).  The running sum is a plain fp32 sum of 2^(s*sc - m) for a reference m that
+// stays where it is: fp32 keeps full relative accuracy for any m within ~100 (log2) of the values, so no running max
+// and no rescale are needed per chunk.  Only when the sum leaves [0, 2^100) -- a value far above m, or the first chunk
+// of a segment (m = -inf gives inf/NaN) -- the chunk is redone exactly with a new reference (s_update).  The pair
+// (m, z) is a valid softmax partial for ANY finite m: merge_row never assumes that m is the true maximum.
+__device__ __forceinline__ void s_lazy32(const uint32_t (&v)[32], float sc, float& m, float& z) {
+#ifdef NACL_EPI_TRIVIAL
+  s_update(v, sc, m, z);
+  return;
+#endif
+  u64 a0 = 0ull, a1 = 0ull;
+  s_acc32(v, sc, m, a0, a1);
+  float s0, s1;
+  unpack2(add2(a0, a1), s0, s1);
+  const float zn = z + (s0 + s1);
+  if (zn < 0x1p100f) {  // false for inf and NaN as well
+    z = zn;
+  } else {
+    s_update(v, sc, m, z);
+    if (!(z < 0x1p100f)) { m += 90.f; z *= 0x1p-90f; }  // many terms just below the limit: move the reference, not the value
+  }
+}
+
 // S tile, this warp's share: NC (32 or 64) key columns of the 32 proxy rows (TMEM lanes) it owns
 // The accumulator buffer is handed back to the MMA warp (arrive on `empty_bar`) as soon as this warp's values are in
 // registers, BEFORE the arithmetic: the MMAs of the tile after next start ~1500 cycles earlier.
@@ -416,8 +458,13 @@ __device__ __forceinline__ void s_cols(uint32_t taddr, float sc, uint32_t empty_
   tc_wait_ld(va);
   if (NC == 64) tc_wait_ld(vb);
   release_tmem(empty_bar);
+#ifdef NACL_S_EAGER
   if (NC == 64) s_update64(va, vb, sc, m, z);
   else s_update(va, sc, m, z);
+#else
+  s_lazy32(va, sc, m, z);
+  if (NC == 64) s_lazy32(vb, sc, m, z);
+#endif
 }
 
 // last tile of a head: columns >= valid (relative to taddr) are keys past L and must not exist (-inf)
@@ -529,17 +576,28 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_half = p.rows > 128 ? 2 : 1;  // 128-row MMA groups of an S tile
+  // Quad accumulators (G*P > 128 in sweep S, G*P == 256 in sweep C).  The warp scheduler of an SM sub-partition prefers
+  // one of its four epilogue warps, so they drift up to a tile apart; with whole-tile accumulators shared by all 16 warps
+  // the slowest warp decides when a buffer goes back to the MMA issuer and the fast ones wait for the next tile.  Here a
+  // tile's accumulator is produced and consumed as two independent 128-column halves (proxy rows 0..127 / 128..255 in
+  // both sweeps: the 128-row MMA groups of sweep S, two N = 128 MMAs in sweep C), four half-buffers in all
+  // (tile parity x half), each with its own full/empty barriers and its own FOUR consumers: the epilogue warps with
+  // cq = 2 * (tile parity) + half, one per sub-partition and all of the same scheduling rank.  A warp processes 128
+  // elements per thread of every other tile; while it waits for its half-buffer to be refilled (~900 cycles) the three
+  // other ranks keep the sub-partition busy.
+  const bool quad = PH == 0 ? p.rows > 128 : p.rows == 256;
   TR_DECL
+  TL_DECL
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
-    for (int s = 0; s < NQ; ++s) { mbar_init(q_full(s), 1); mbar_init(q_empty(s), 1); }
+    for (int s = 0; s < NQ; ++s) { mbar_init(q_full(s), 1); mbar_init(q_empty(s), 2); }  // q_empty: one arrival per MMA issuer
     for (int b = 0; b < N_BUFS; ++b)
       for (int h = 0; h < 2; ++h) {
         mbar_init(tm_full(b, h), 1);
-        mbar_init(tm_empty(b, h), (p.phase == 0 && kHalfBarriers) ? N_EPI_WARPS / n_half : N_EPI_WARPS);  // epilogue warps that drain it
+        mbar_init(tm_empty(b, h), quad ? 4 : N_EPI_WARPS);  // epilogue warps that drain it
       }
-    for (int b = 0; b < N_CS; ++b) { mbar_init(cs_full(b), N_EPI_WARPS); mbar_init(cs_empty(b), 1); }
+    for (int b = 0; b < N_CS; ++b) { mbar_init(cs_full(b), quad ? N_EPI_WARPS / 2 : N_EPI_WARPS); mbar_init(cs_empty(b), 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == W_MMA) {
@@ -581,12 +639,17 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
       }
     }
     __syncwarp();
-  } else if (warp == W_MMA) {
-    // ================================================================ tcgen05.mma issuer
+  } else if (warp == W_MMA || warp == W_MMA2) {
+    // ================================================================ tcgen05.mma issuers
+    // Two issuer warps alternate tiles: issuer `mine` owns the tiles of that parity and the accumulator buffer of the
+    // same number.  A tcgen05.mma issue blocks until the pipe has room, so one issuer spends the whole MMA time of a
+    // tile inside the issue sequence; the other meanwhile sits through the barrier waits of the next tile (~200 cycles
+    // each even when complete) and its MMAs queue up directly behind -- the tensor pipe no longer idles between tiles.
+    const uint32_t mine = (uint32_t)(warp - W_MMA);
     const bool leader = elect_one();  // ONE lane issues every MMA and every commit (a commit covers its own thread's MMAs)
     int stage = 0, qrun = 0;
     uint32_t kphase = 0, tcount = 0;
-    const uint32_t idesc = p.phase == 0 ? umma_idesc(128, TILE) : umma_idesc(128, p.rows);
+    const uint32_t idesc = PH == 0 ? umma_idesc(128, TILE) : umma_idesc(128, p.rows);
     Walk walk(p);
     Seg sg;
     while (walk.next(sg)) {
@@ -594,49 +657,75 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
       TRW(2, mbar_wait(q_full(qb), (qrun / NQ) & 1));
       const uint32_t qsrc = sbase + SM::OFF_Q + qb * SM::Q_BYTES;
       ++qrun;
+      if (sg.n == 1 && (tcount & 1) != mine) {
+        // no tile of this segment is this issuer's: it still owes its arrival on q_empty
+        if (leader) mbar_arrive(q_empty(qb));
+        __syncwarp();
+      }
       for (int i = 0; i < sg.n; ++i) {
         const uint32_t buf = tcount & 1, par = (tcount >> 1) & 1;
-        TRW(0, mbar_wait(k_full(stage), kphase));
-        const uint32_t ksrc = sbase + SM::OFF_K + stage * KSTAGE_BYTES;
-        const uint32_t dcol = tmem_base + buf * BUF_COLS;
-        if (p.phase == 0) {
-          // the two 128-row halves accumulate into different TMEM columns: their k-steps are interleaved so that
-          // consecutive MMAs never depend on each other (a dependent N=128 MMA chain runs at ~55 % of the pipe rate)
-          for (int h = 0; h < (kHalfBarriers ? n_half : 1); ++h) TRW(1, mbar_wait(tm_empty(buf, h), par ^ 1));
-          tc_fence_after();
-          if (leader) {
+        if (buf == mine) {
+          TL(0)
+          TRW(0, mbar_wait(k_full(stage), kphase));
+          TL(1)
+          const uint32_t ksrc = sbase + SM::OFF_K + stage * KSTAGE_BYTES;
+          const uint32_t dcol = tmem_base + buf * BUF_COLS;
+          if (quad) {
+            // the two 128-column halves of the tile: each goes out as soon as ITS half-buffer is free
+            const uint32_t idesc_q = umma_idesc(128, 128);
+            for (uint32_t h = 0; h < 2; ++h) {
+              TRW(1, mbar_wait(tm_empty(buf, h), par ^ 1));
+              tc_fence_after();
+              if (leader) {
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-              const uint32_t ko = (k >> 2) * BOX_BYTES + (k & 3) * 32;
-              const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32;
-              // proxy rows [128h, 128h+128) sit 128 rows x 128 B further down in each Q box
-              tc_mma(dcol, umma_desc(qsrc + qo), umma_desc(ksrc + ko), idesc, k > 0);
-              if (k == 7 && kHalfBarriers) tc_commit(tm_full(buf, 0));
-              if (n_half == 2) tc_mma(dcol + 128, umma_desc(qsrc + qo + BOX_BYTES), umma_desc(ksrc + ko), idesc, k > 0);
+                for (int k = 0; k < 8; ++k) {
+                  const uint32_t ko = (k >> 2) * BOX_BYTES + (k & 3) * 32;
+                  // proxy rows [128h, 128h+128) sit 128 rows x 128 B further down in each Q box
+                  const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32 + h * BOX_BYTES;
+                  if constexpr (PH == 0) tc_mma(dcol + h * 128, umma_desc(qsrc + qo), umma_desc(ksrc + ko), idesc_q, k > 0);
+                  else tc_mma(dcol + h * 128, umma_desc(ksrc + ko), umma_desc(qsrc + qo), idesc_q, k > 0);
+                }
+                tc_commit(tm_full(buf, h));
+              }
+              __syncwarp();
             }
-            if (kHalfBarriers) { if (n_half == 2) tc_commit(tm_full(buf, 1)); }
-            else tc_commit(tm_full(buf, 0));
-          }
-          __syncwarp();
-        } else {
+            TL(2)
+            if (leader) {
+              tc_commit(k_empty(stage));
+              if (i + 2 >= sg.n) tc_commit(q_empty(qb));
+            }
+          } else {
           TRW(1, mbar_wait(tm_empty(buf, 0), par ^ 1));
+          TL(2)
           tc_fence_after();
           if (leader) {
+            if constexpr (PH == 0) {
+              // the two 128-row halves accumulate into different TMEM columns: their k-steps are interleaved so that
+              // consecutive MMAs never depend on each other (a dependent N=128 MMA chain runs at ~55 % of the pipe rate)
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-              const uint32_t ko = (k >> 2) * BOX_BYTES + (k & 3) * 32;
-              const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32;
-              tc_mma(dcol, umma_desc(ksrc + ko), umma_desc(qsrc + qo), idesc, k > 0);
+              for (int k = 0; k < 8; ++k) {
+                const uint32_t ko = (k >> 2) * BOX_BYTES + (k & 3) * 32;
+                const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32;
+                tc_mma(dcol, umma_desc(qsrc + qo), umma_desc(ksrc + ko), idesc, k > 0);
+                if (n_half == 2) tc_mma(dcol + 128, umma_desc(qsrc + qo + BOX_BYTES), umma_desc(ksrc + ko), idesc, k > 0);
+              }
+            } else {
+#pragma unroll
+              for (int k = 0; k < 8; ++k) {
+                const uint32_t ko = (k >> 2) * BOX_BYTES + (k & 3) * 32;
+                const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32;
+                tc_mma(dcol, umma_desc(ksrc + ko), umma_desc(qsrc + qo), idesc, k > 0);
+              }
             }
-            tc_commit(tm_full(buf, 0));  // the accumulator buffer is complete
+            tc_commit(tm_full(buf, 0));   // the accumulator buffer is complete
+            tc_commit(k_empty(stage));    // the reads of the stage are done once these MMAs complete
+            if (i + 2 >= sg.n) tc_commit(q_empty(qb));  // this issuer's last tile of the segment: its reads of Q are done
+          }
           }
           __syncwarp();
+          TL(3)
+          TL_NEXT()
         }
-        if (leader) {
-          tc_commit(k_empty(stage));  // the reads of the stage are done once these MMAs complete
-          if (i == sg.n - 1) tc_commit(q_empty(qb));  // every MMA that read the segment's Q has completed
-        }
-        __syncwarp();
         ++tcount;
         if (++stage == STAGES) { stage = 0; kphase ^= 1; }
       }
@@ -644,7 +733,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
     __syncwarp();
   } else if (warp == W_CMB) {
     // ================================================================ column-sum combiner (sweep C only)
-    if (p.phase != 0) {
+    if constexpr (PH != 0) {
       uint32_t ccount = 0;
       Walk walk(p);
       Seg sg;
@@ -657,7 +746,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             const int key = lane + 32 * u;
-            r[u] = (c[key] + c[TILE + key]) + (c[2 * TILE + key] + c[3 * TILE + key]);
+            r[u] = quad ? c[key] + c[TILE + key] : (c[key] + c[TILE + key]) + (c[2 * TILE + key] + c[3 * TILE + key]);
           }
           __syncwarp();
           if (lane == 0) mbar_arrive(cs_empty(cb));
@@ -691,22 +780,73 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
     const bool live = s_half * 128 + quarter * 32 < p.rows;  // does this warp own a live proxy row?
     // sweep C: this warp's proxy rows (columns)
     const int c_nc = p.rows >> 2, c_col0 = cq * c_nc;
+    // quad scheme: half and tile parity of this warp's half-buffer; the proxy row it owns in sweep S
+    const int q_half = cq & 1, q_par = cq >> 1;
+    const int q_row = q_half * 128 + quarter * 32 + lane;
+    const bool q_live = q_half * 128 + quarter * 32 < p.rows;
     uint32_t ecount = 0;  // tiles seen so far, same sequence as the MMA warp's tcount
     int nseg = 0;
     Walk walk(p);
     Seg sg;
     while (walk.next(sg)) {
-      if (p.phase == 0) {
-        // ---------------- S segment: running (max, sum-exp) of row s_row over this warp's key columns
+      if constexpr (PH == 0) {
+        // ---------------- S segment: running (reference, sum-exp) of row s_row over this warp's key columns
         float m0 = -INFINITY, z0 = 0.f;
+        if (quad) {
+          // this warp: proxy rows of half q_half (one per thread), all 128 key columns of the tiles of parity q_par
+          for (int i = 0; i < sg.n; ++i) {
+            const uint32_t g = ecount + i;
+            if ((int)(g & 1) != q_par) continue;
+            TL(0)
+            TRW(0, mbar_wait(tm_full(q_par, q_half), (g >> 1) & 1));
+            TL(1)
+            tc_fence_after();
+            const int valid = p.L - (sg.tile + i) * TILE;
+            const bool ctile = p.causal && (sg.tile + i) * TILE + TILE - 1 > p.L - p.P;
+            const uint32_t ta = tbase + q_par * BUF_COLS + q_half * 128;
+            const uint32_t ebar = tm_empty(q_par, q_half);
+            TRW(1, if (q_live && !ctile && valid >= TILE) {
+              uint32_t va[32], vb[32];
+              tmem_ld32(ta, va);
+              tmem_ld32(ta + 32, vb);
+              tc_wait_ld(va);
+              tc_wait_ld(vb);
+              s_lazy32(va, sc, m0, z0);
+              s_lazy32(vb, sc, m0, z0);
+              tmem_ld32(ta + 64, va);
+              tmem_ld32(ta + 96, vb);
+              tc_wait_ld(va);
+              tc_wait_ld(vb);
+              release_tmem(ebar);  // the half-buffer goes back before the arithmetic on its last columns
+              s_lazy32(va, sc, m0, z0);
+              s_lazy32(vb, sc, m0, z0);
+            } else {
+              if (q_live) {
+                if (ctile) s_cols_masked(ta, TILE, sc, valid, min(valid, valid - p.P + 1 + (sg.rb * 256 + q_row) % p.P), m0, z0);
+                else s_cols_masked(ta, TILE, sc, valid, valid, m0, z0);
+              }
+              release_tmem(ebar);
+            })
+            TL(2)
+            TL_NEXT()
+          }
+          if (q_row < p.rows)
+            __stcg(&p.part[(((size_t)blockIdx.x + sg.head) * p.n_slots + q_par) * p.rows_total + sg.rb * 256 + q_row], make_float2(m0, z0));
+          ecount += sg.n;
+          ++nseg;
+          continue;
+        }
         for (int i = 0; i < sg.n; ++i) {
           const uint32_t g = ecount + i, buf = g & 1;
-          TRW(0, mbar_wait(tm_full(buf, kHalfBarriers ? s_half : 0), (g >> 1) & 1));
+#ifdef NACL_LOCKSTEP
+          asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory");
+#endif
+          TRW(0, mbar_wait(tm_full(buf, 0), (g >> 1) & 1));
           tc_fence_after();
           const int valid = p.L - (sg.tile + i) * TILE - s_col0;
           // CAUSAL: this thread's row (i = s_row % P) sees the columns whose key j <= L-P+i
           const bool ctile = p.causal && (sg.tile + i) * TILE + TILE - 1 > p.L - p.P;
-          const uint32_t ebar = tm_empty(buf, kHalfBarriers ? s_half : 0);
+          const uint32_t ebar = tm_empty(buf, 0);
           TRW(1, if (live && !ctile && valid >= s_nc) {
             const uint32_t ta = tbase + buf * BUF_COLS + s_half * 128 + s_col0;
             if (n_half == 2) s_cols<64>(ta, sc, ebar, m0, z0); else s_cols<32>(ta, sc, ebar, m0, z0);  // releases the buffer itself
@@ -744,9 +884,65 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
           }
         })
         TRW(3, asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory"));
+        if (quad) {
+          // this warp: the 32 keys of its lane quarter (one per thread) summed over the 128 proxy rows of half q_half, for
+          // the tiles of parity q_par; the combiner adds the two halves of a key
+          const float* nlh = nl + q_half * 128;
+          for (int i = 0; i < sg.n; ++i) {
+            const uint32_t g = ecount + i;
+            if ((int)(g & 1) != q_par) continue;
+            const int cb = g % N_CS;
+            TL(0)
+            TRW(0, mbar_wait(tm_full(q_par, q_half), (g >> 1) & 1));
+            TL(1)
+            tc_fence_after();
+            const uint32_t ta = tbase + q_par * BUF_COLS + q_half * 128;
+            const uint32_t ebar = tm_empty(q_par, q_half);
+            float r;
+            if (p.causal && (sg.tile - i) * TILE + TILE - 1 > p.L - p.P) {
+              const int jkey = (sg.tile - i) * TILE + quarter * 32 + lane;  // the key this thread owns
+              r = c_cols_causal(ta, 128, sc, nlh, sg.rb * 256 + q_half * 128, p.P, jkey - (p.L - p.P));
+              release_tmem(ebar);
+            } else {
+              TRW(1, {
+                u64 a0 = 0ull, a1 = 0ull;
+                uint32_t va[32], vb[32];
+                tmem_ld32(ta, va);
+                tmem_ld32(ta + 32, vb);
+                tc_wait_ld(va);
+                c_update<8>(va, sc, nlh, a0, a1);
+                tc_wait_ld(vb);
+                c_update<8>(vb, sc, nlh + 32, a0, a1);
+                tmem_ld32(ta + 64, va);
+                tmem_ld32(ta + 96, vb);
+                tc_wait_ld(va);
+                tc_wait_ld(vb);
+                release_tmem(ebar);
+                c_update<8>(va, sc, nlh + 64, a0, a1);
+                c_update<8>(vb, sc, nlh + 96, a0, a1);
+                float s0, s1;
+                unpack2(add2(a0, a1), s0, s1);
+                r = s0 + s1;
+              })
+            }
+            TL(2)
+            TRW(4, mbar_wait(cs_empty(cb), ((g / N_CS) & 1) ^ 1));
+            cs_s[(cb * 4 + q_half) * TILE + quarter * 32 + lane] = r;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(cs_full(cb));
+            TL(3)
+            TL_NEXT()
+          }
+          ecount += sg.n;
+          ++nseg;
+          continue;
+        }
         for (int i = 0; i < sg.n; ++i) {
           const uint32_t g = ecount + i, buf = g & 1;
           const int cb = g % N_CS;
+#ifdef NACL_LOCKSTEP
+          asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory");
+#endif
           TRW(0, mbar_wait(tm_full(buf, 0), (g >> 1) & 1));
           tc_fence_after();
           float r;
@@ -891,5 +1087,8 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
 // diagnostics build only: per-warp wait/compute cycle counters of the last launches
 extern "C" __attribute__((visibility("default"))) int nacl_debug_trace_read(long long* host, size_t bytes) {
   return (int)cudaMemcpyFromSymbol(host, nacl::g_trace, bytes < sizeof(nacl::g_trace) ? bytes : sizeof(nacl::g_trace));
+}
+extern "C" __attribute__((visibility("default"))) int nacl_debug_timeline_read(long long* host) {
+  return (int)cudaMemcpyFromSymbol(host, nacl::g_tl, sizeof(nacl::g_tl));
 }
 #endif

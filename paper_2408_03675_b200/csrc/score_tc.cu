@@ -59,10 +59,14 @@ constexpr int BUF_COLS = 256;                  // TMEM columns per accumulator b
 constexpr int N_CS = 4;                        // shared-memory buffers for the quarter column sums of a C tile
 constexpr int MAX_GRID = kNumSMs;              // the partial-statistics workspace is sized for this many CTAs
 constexpr uint32_t SPIN_LIMIT = 1u << 26;      // watchdog: a wait that long is a bug -> trap (loud failure)
-#ifndef NACL_POLY_MASK
-#define NACL_POLY_MASK 0x22u
+// which of every 8 element pairs take the FMA-pipe exp2 instead of MUFU.EX2 (bit e&7), per sweep: measured optimum on
+// B200 (cfg 4, us per layer): sweep S 74.8 / 71.9 / 75.3 and sweep C 82.0 / 82.4 / 86.6 for 2/8, 3/8, 4/8
+#ifndef NACL_POLY_MASK_S
+#define NACL_POLY_MASK_S 0x2Au
 #endif
-constexpr uint32_t POLY_MASK = NACL_POLY_MASK;  // which of every 8 element pairs take the FMA-pipe exp2 (bit e&7)
+#ifndef NACL_POLY_MASK_C
+#define NACL_POLY_MASK_C 0x22u
+#endif
 
 // Optional wait/compute cycle accounting per warp role (diagnostics build only: -DNACL_TC_TRACE).
 #ifdef NACL_TC_TRACE
@@ -119,19 +123,6 @@ __device__ __forceinline__ uint32_t mbar_try_wait(uint32_t a, uint32_t parity) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
       "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-      "selp.u32 %0, 1, 0, p;\n\t}"
-      : "=r"(ok)
-      : "r"(a), "r"(parity)
-      : "memory");
-  return ok;
-}
-// non-blocking probe: the predicate comes back after the barrier unit's latency, which overlaps with whatever the
-// caller issues before it looks at the result
-__device__ __forceinline__ uint32_t mbar_test(uint32_t a, uint32_t parity) {
-  uint32_t ok;
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
       "selp.u32 %0, 1, 0, p;\n\t}"
       : "=r"(ok)
       : "r"(a), "r"(parity)
@@ -240,8 +231,9 @@ __device__ __forceinline__ u64 pack2u(uint32_t a, uint32_t b) { u64 r; asm("mov.
 __device__ __forceinline__ void unpack2(u64 r, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(r)); }
 __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 __device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ u64 add2_rm(u64 a, u64 b) { u64 r; asm("add.rm.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 fma2_rm(u64 a, u64 b, u64 c) { u64 r; asm("fma.rm.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ float fma_sat(float a, float b, float c) { float r; asm("fma.rn.sat.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c)); return r; }
 __device__ __forceinline__ float max3(float a, float b, float c) { float r; asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c)); return r; }
 
 // (2^x0, 2^x1) on the MUFU unit
@@ -250,26 +242,30 @@ __device__ __forceinline__ u64 exp2_mufu2(u64 x) {
   unpack2(x, a, b);
   return pack2(fast_exp2(a), fast_exp2(b));
 }
-// (2^x0, 2^x1) on the FMA pipe, x <= ~0: n = floor(x) by a round-down add of 1.5*2^23, f = x - n in [0,1),
-// 2^f by a degree-3 minimax polynomial (relative error <= 7.5e-5), 2^n by an add into the exponent field.
-// x is clamped to [-125, 127] (2^-125 ~ 2e-38 stands for zero, 2^127 for "too large": the exponent field must not wrap;
-// sweep S treats a sum >= 2^100 as the signal to take a new reference, see s_lazy32).
-__device__ __forceinline__ u64 exp2_poly2(u64 x) {
-  float a, b;
-  unpack2(x, a, b);
-  x = pack2(fminf(fmaxf(a, -125.f), 127.f), fminf(fmaxf(b, -125.f), 127.f));
-  const u64 magic = pack2(12582912.f, 12582912.f);
-  const u64 fi = add2_rm(x, magic);
-  const u64 f = sub2(x, sub2(fi, magic));
+// acc += (2^x0, 2^x1) on the FMA pipe, for x = s*sc - ref given as the raw logits s and the two constants
+//   scy = sc / 227,  cy = (110 - ref) / 227:
+// y = sat(s*scy + cy) in [0, 1] IS the clamp of x to [-110, 117] (one saturating FMA, no min/max: values below stand
+// for zero -- 2^-110 * 256 rows < the 1e-30 absolute score tolerance -- and values above for "too large", which sweep S
+// turns into a new reference, see s_lazy32); u = 227*y = x + 110 in [0, 227]; n = floor(u) by a round-down FMA onto
+// 1.5*2^23, f = u - n in [0, 1]; 2^f by the degree-3 minimax polynomial (relative error <= 7.5e-5); 2^(n-110) is built
+// in the exponent field (17 + n in [17, 244]) and multiplied in by the FMA that accumulates.  y resolves x to
+// 227 * 2^-24 = 1.4e-5, i.e. 1e-5 relative in 2^x.  8 FMA-pipe instructions and 2 integer ones per pair.
+constexpr float kPolyLo = 110.f, kPolySpan = 227.f;
+__device__ __forceinline__ u64 acc_exp2_poly_sat(u64 acc, uint32_t s0, uint32_t s1, float scy, float cy0, float cy1) {
+  const u64 y = pack2(fma_sat(__uint_as_float(s0), scy, cy0), fma_sat(__uint_as_float(s1), scy, cy1));
+  const u64 span = pack2(kPolySpan, kPolySpan), magic = pack2(12582912.f, 12582912.f);
+  const u64 t = fma2_rm(y, span, magic);
+  const u64 f = fma2(y, span, sub2(magic, t));  // 227*y - n
   u64 p = fma2(pack2(0.0780245f, 0.0780245f), f, pack2(0.22606719f, 0.22606719f));
   p = fma2(p, f, pack2(0.6958335f, 0.6958335f));
   p = fma2(p, f, pack2(0.9999252f, 0.9999252f));
-  float p0, p1, i0, i1;
-  unpack2(p, p0, p1);
-  unpack2(fi, i0, i1);
-  return pack2u(__float_as_uint(p0) + (__float_as_uint(i0) << 23), __float_as_uint(p1) + (__float_as_uint(i1) << 23));
+  float t0, t1;
+  unpack2(t, t0, t1);
+  const u64 pw = pack2u((__float_as_uint(t0) << 23) + (17u << 23), (__float_as_uint(t1) << 23) + (17u << 23));
+  return fma2(p, pw, acc);
 }
-__device__ __forceinline__ constexpr bool pair_on_fma_pipe(int e) { return (POLY_MASK >> (e & 7)) & 1u; }
+template <uint32_t MASK>
+__device__ __forceinline__ constexpr bool pair_on_fma_pipe(int e) { return (MASK >> (e & 7)) & 1u; }
 
 // lse (log2 domain) of one proxy row from its partials pp[c * stride], c < np, merged in ascending order with
 // 16 loads in flight.  Consecutive lanes own consecutive rows, so every load of the warp is one contiguous 256 B.
@@ -355,8 +351,8 @@ struct Smem {
   static constexpr int Q_BYTES = QROWS * HD * 2;
   static constexpr int OFF_Q = 0;
   static constexpr int OFF_K = OFF_Q + NQ * Q_BYTES;
-  static constexpr int OFF_LSE = OFF_K + STAGES * KSTAGE_BYTES;   // float[LSE_SLOTS][256]: -lse (log2 domain) of the segment's head
-  static constexpr int OFF_CS = OFF_LSE + (PH ? LSE_SLOTS * 256 * 4 : 0);    // float[N_CS][4][128]: quarter column sums of a C tile
+  static constexpr int OFF_LSE = OFF_K + STAGES * KSTAGE_BYTES;   // float[LSE_SLOTS][2][256]: -lse (log2 domain) of the segment's head, and (110 - lse) / 227
+  static constexpr int OFF_CS = OFF_LSE + (PH ? LSE_SLOTS * 512 * 4 : 0);    // float[N_CS][4][128]: quarter column sums of a C tile
   static constexpr int OFF_BARS = OFF_CS + (PH ? N_CS * 4 * TILE * 4 : 0);
   static constexpr int N_BARS = 2 * STAGES + 2 * NQ + 4 * N_BUFS + 2 * N_CS;
   static constexpr int OFF_TMEM = OFF_BARS + N_BARS * 8;
@@ -377,12 +373,13 @@ __device__ __forceinline__ float s_max32(const uint32_t (&v)[32]) {
 // (a0, a1) += 2^(v*sc - m_ref) over 32 columns, packed; some pairs on the FMA pipe (POLY_MASK)
 __device__ __forceinline__ void s_acc32(const uint32_t (&v)[32], float sc, float m_ref, u64& a0, u64& a1) {
   const u64 sc2 = pack2(sc, sc), nm2 = pack2(-m_ref, -m_ref);
+  const float scy = sc * (1.f / kPolySpan), cy = (kPolyLo - m_ref) * (1.f / kPolySpan);
 #pragma unroll
   for (int e = 0; e < 16; e += 2) {
-    const u64 x0 = fma2(pack2u(v[2 * e + 0], v[2 * e + 1]), sc2, nm2);
-    const u64 x1 = fma2(pack2u(v[2 * e + 2], v[2 * e + 3]), sc2, nm2);
-    a0 = add2(a0, pair_on_fma_pipe(e) ? exp2_poly2(x0) : exp2_mufu2(x0));
-    a1 = add2(a1, pair_on_fma_pipe(e + 1) ? exp2_poly2(x1) : exp2_mufu2(x1));
+    if (pair_on_fma_pipe<NACL_POLY_MASK_S>(e)) a0 = acc_exp2_poly_sat(a0, v[2 * e + 0], v[2 * e + 1], scy, cy, cy);
+    else a0 = add2(a0, exp2_mufu2(fma2(pack2u(v[2 * e + 0], v[2 * e + 1]), sc2, nm2)));
+    if (pair_on_fma_pipe<NACL_POLY_MASK_S>(e + 1)) a1 = acc_exp2_poly_sat(a1, v[2 * e + 2], v[2 * e + 3], scy, cy, cy);
+    else a1 = add2(a1, exp2_mufu2(fma2(pack2u(v[2 * e + 2], v[2 * e + 3]), sc2, nm2)));
   }
 }
 // one 32-column segment of an S tile: online (max, sum-exp) update of the row this thread owns
@@ -402,23 +399,6 @@ __device__ __forceinline__ void s_update(const uint32_t (&v)[32], float sc, floa
   z = fmaf(z, fast_exp2(m - m_new), s0 + s1);
   m = m_new;
 }
-// 64 columns at once: one running-max update and one rescale for both register blocks
-__device__ __forceinline__ void s_update64(const uint32_t (&va)[32], const uint32_t (&vb)[32], float sc, float& m, float& z) {
-#ifdef NACL_EPI_TRIVIAL
-  s_update(va, sc, m, z);
-  s_update(vb, sc, m, z);
-  return;
-#endif
-  const float m_new = fmaxf(m, fmaxf(s_max32(va), s_max32(vb)) * sc);
-  u64 a0 = 0ull, a1 = 0ull;
-  s_acc32(va, sc, m_new, a0, a1);
-  s_acc32(vb, sc, m_new, a0, a1);
-  float s0, s1;
-  unpack2(add2(a0, a1), s0, s1);
-  z = fmaf(z, fast_exp2(m - m_new), s0 + s1);
-  m = m_new;
-}
-
 // Lazy reference (sweep S, full tiles).  The running sum is a plain fp32 sum of 2^(s*sc - m) for a reference m that
 // stays where it is: fp32 keeps full relative accuracy for any m within ~100 (log2) of the values, so no running max
 // and no rescale are needed per chunk.  Only when the sum leaves [0, 2^100) -- a value far above m, or the first chunk
@@ -458,13 +438,8 @@ __device__ __forceinline__ void s_cols(uint32_t taddr, float sc, uint32_t empty_
   tc_wait_ld(va);
   if (NC == 64) tc_wait_ld(vb);
   release_tmem(empty_bar);
-#ifdef NACL_S_EAGER
-  if (NC == 64) s_update64(va, vb, sc, m, z);
-  else s_update(va, sc, m, z);
-#else
   s_lazy32(va, sc, m, z);
   if (NC == 64) s_lazy32(vb, sc, m, z);
-#endif
 }
 
 // last tile of a head: columns >= valid (relative to taddr) are keys past L and must not exist (-inf)
@@ -484,11 +459,13 @@ __device__ __forceinline__ void s_cols_masked(uint32_t taddr, int nc, float sc, 
   }
 }
 
-// N4 groups of 4 columns (proxy rows) of a C tile: acc += 2^(s*sc - lse2[row]); nl = -lse2 of those rows
+// N4 groups of 4 columns (proxy rows) of a C tile: acc += 2^(s*sc - lse2[row]); nl = -lse2 of those rows and, kNY floats
+// further on, (110 - lse2) / 227 of the same rows (the constant of the FMA-pipe path)
+constexpr int kNY = 256;
 template <int N4>
 __device__ __forceinline__ void c_update(const uint32_t (&v)[32], float sc, const float* nl, u64& a0, u64& a1) {
-  const ulonglong2* l2 = reinterpret_cast<const ulonglong2*>(nl);
   const u64 sc2 = pack2(sc, sc);
+  const float scy = sc * (1.f / kPolySpan);
 #ifdef NACL_EPI_TRIVIAL
 #pragma unroll
   for (int e = 0; e < N4; ++e) {
@@ -499,11 +476,18 @@ __device__ __forceinline__ void c_update(const uint32_t (&v)[32], float sc, cons
 #endif
 #pragma unroll
   for (int e = 0; e < N4; ++e) {
-    const ulonglong2 l = l2[e];
-    const u64 x0 = fma2(pack2u(v[4 * e + 0], v[4 * e + 1]), sc2, l.x);
-    const u64 x1 = fma2(pack2u(v[4 * e + 2], v[4 * e + 3]), sc2, l.y);
-    a0 = add2(a0, pair_on_fma_pipe(2 * e) ? exp2_poly2(x0) : exp2_mufu2(x0));
-    a1 = add2(a1, pair_on_fma_pipe(2 * e + 1) ? exp2_poly2(x1) : exp2_mufu2(x1));
+    if (pair_on_fma_pipe<NACL_POLY_MASK_C>(2 * e)) {
+      const float2 c = *reinterpret_cast<const float2*>(nl + kNY + 4 * e);
+      a0 = acc_exp2_poly_sat(a0, v[4 * e + 0], v[4 * e + 1], scy, c.x, c.y);
+    } else {
+      a0 = add2(a0, exp2_mufu2(fma2(pack2u(v[4 * e + 0], v[4 * e + 1]), sc2, *reinterpret_cast<const u64*>(nl + 4 * e))));
+    }
+    if (pair_on_fma_pipe<NACL_POLY_MASK_C>(2 * e + 1)) {
+      const float2 c = *reinterpret_cast<const float2*>(nl + kNY + 4 * e + 2);
+      a1 = acc_exp2_poly_sat(a1, v[4 * e + 2], v[4 * e + 3], scy, c.x, c.y);
+    } else {
+      a1 = add2(a1, exp2_mufu2(fma2(pack2u(v[4 * e + 2], v[4 * e + 3]), sc2, *reinterpret_cast<const u64*>(nl + 4 * e + 2))));
+    }
   }
 }
 
@@ -838,9 +822,6 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
         }
         for (int i = 0; i < sg.n; ++i) {
           const uint32_t g = ecount + i, buf = g & 1;
-#ifdef NACL_LOCKSTEP
-          asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory");
-#endif
           TRW(0, mbar_wait(tm_full(buf, 0), (g >> 1) & 1));
           tc_fence_after();
           const int valid = p.L - (sg.tile + i) * TILE - s_col0;
@@ -865,7 +846,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
       } else {
         // ---------------- C segment: merge the head's partials (ascending piece order) into -lse, then column sums
         const int ls = nseg % LSE_SLOTS;
-        float* nl = nlse_s + ls * 256;
+        float* nl = nlse_s + ls * 512;
         TRW(2, {
           const int r = threadIdx.x;
           if (r < p.rows) {
@@ -879,6 +860,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
                              (c_last - c_first + 1) * p.n_slots, (size_t)p.rows_total);
             }
             nl[r] = -l2;
+            nl[kNY + r] = (kPolyLo - l2) * (1.f / kPolySpan);
             // the CTA that owns the head's first tile publishes lse
             if (p.lse_out && sg.tile - (sg.n - 1) == 0) p.lse_out[(size_t)sg.head * p.rows_total + sg.rb * 256 + r] = l2 * 0.69314718055994530942f;
           }
@@ -940,9 +922,6 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
         for (int i = 0; i < sg.n; ++i) {
           const uint32_t g = ecount + i, buf = g & 1;
           const int cb = g % N_CS;
-#ifdef NACL_LOCKSTEP
-          asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory");
-#endif
           TRW(0, mbar_wait(tm_full(buf, 0), (g >> 1) & 1));
           tc_fence_after();
           float r;

@@ -36,7 +36,9 @@
  * on `stream` (a cudaStream_t passed as void*); the call never synchronises the host and
  * results are valid once the stream reaches that point.  With a caller-supplied workspace
  * (nacl_evict_ex) the call allocates nothing and is CUDA-graph capturable; without one a
- * grow-only per-device workspace is created on first use (cudaMalloc: not capturable).
+ * grow-only internal workspace per (device, stream) is created on first use (cudaMalloc: not capturable); calls on
+ * one stream share it in stream order, calls on different streams never do, so concurrent host threads are safe as
+ * long as they use different streams (or pass their own workspaces).
  * Same inputs and seed give bit-identical outputs run to run (no floating-point atomics).
  * nacl_evict_host is the same operation on HOST buffers (copies inside; synchronous).
  *
@@ -62,7 +64,7 @@
 extern "C" {
 #endif
 
-#define NACL_VERSION 101 /* major*10000 + minor*100 + patch */
+#define NACL_VERSION 200 /* major*10000 + minor*100 + patch */
 
 #define NACL_DTYPE_F32 0
 #define NACL_DTYPE_BF16 1
@@ -106,6 +108,12 @@ typedef struct nacl_params {
                                       prefill attention kernel that keeps its softmax statistics already has it (the contract of
                                       the paper's Algorithm 2).  When given, the statistics sweep over K is
                                       skipped: one logit sweep instead of two.  The caller answers for its accuracy. */
+  int32_t batch_offset;            /* global index of this call's batch element 0 and ...                                  */
+  int32_t head_offset;             /* ... of its kv head 0: the Random Eviction draws are keyed by the GLOBAL (layer, batch,
+                                      kv head, position) ("different seed on attention heads and layers"), so a
+                                      caller that holds a slice of the heads (tensor parallel) or of the batch (data parallel)
+                                      passes where its slice starts and draws exactly what the unsharded call draws.  >= 0;
+                                      0 for an unsharded call */
 } nacl_params_t;
 
 /* bf16 K/V/Q.  Steps 1-7 above on `stream`. */
@@ -146,7 +154,9 @@ int nacl_gumbel_keys(const float* importance, float* out_keys, int batch, int Hk
 /* Bytes of scratch one call needs (a pure function of the shape; 0 on invalid shapes). */
 size_t nacl_workspace_bytes(int batch, int L, int Hq, int Hkv, int d, int P);
 
-/* Number of kernels one call with these arguments launches (for launch accounting). */
+/* Number of kernels one self-contained call with these arguments launches (for launch accounting; budget_random > 0 and
+ * no lse_in assumed: with lse_in the statistics sweep -- one launch on the tensor-core path, two on the generic one --
+ * is skipped). */
 int nacl_launch_count(int dtype, int batch, int L, int Hq, int Hkv, int d, int P, uint32_t flags);
 
 /* Per-stage device timing, for benchmarks.  While enabled, every call brackets each of its kernel

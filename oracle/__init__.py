@@ -36,6 +36,8 @@ def lib() -> C.CDLL:
         L.nacl_oracle_importance.restype = i32
         L.nacl_oracle_select.argtypes = [vp, i32, i32, i32, i32, i32, i32, i32, u64, i32, u32, vp, vp, vp]
         L.nacl_oracle_select.restype = i32
+        L.nacl_oracle_select_ex.argtypes = [vp, i32, i32, i32, i32, i32, i32, i32, u64, i32, u32, vp, vp, vp, vp]
+        L.nacl_oracle_select_ex.restype = i32
         L.nacl_oracle_gather.argtypes = [vp, vp, C.c_size_t, i32, i32, i32, i32, vp, vp, vp]
         L.nacl_oracle_gather.restype = i32
         L.nacl_oracle_evict.argtypes = [vp, vp, vp, i32] + [i32] * 10 + [u64, i32, u32, vp, vp, vp, vp, i32]
@@ -115,17 +117,28 @@ def importance(K, Q, flags: int = 0, nthreads: int = 0, return_lse: bool = False
     return (imp, lse) if return_lse else imp
 
 
+class _SelectOpts(C.Structure):
+    _fields_ = [("batch_offset", C.c_int), ("head_offset", C.c_int), ("protect_idx", C.c_void_p), ("n_protect", C.c_int),
+                ("shared_heads", C.c_int)]
+
+
 def select(imp, budget_proxy: int, budget_random: int, n_sink: int, n_recent: int,
-           seed: int, layer: int, flags: int = 0, return_parts: bool = False, return_keys: bool = False):
-    """imp [B,Hkv,L] (any float dtype, widened exactly to fp64) -> idx [B,Hkv,C] int32 ascending."""
+           seed: int, layer: int, flags: int = 0, return_parts: bool = False, return_keys: bool = False,
+           batch_offset: int = 0, head_offset: int = 0, protect_idx=None, shared_heads: bool = False):
+    """imp [B,Hkv,L] (any float dtype, widened exactly to fp64) -> idx [B,Hkv,C] int32 ascending.
+    batch_offset / head_offset / protect_idx / shared_heads: nacl_oracle_select_opts (oracle/nacl_oracle.h)."""
     imp = np.ascontiguousarray(np.asarray(imp, dtype=np.float64))
     B, Hkv, L = imp.shape
     Cn = budget_proxy + budget_random
     idx = np.empty((B, Hkv, max(Cn, 0)), dtype=np.int32)
     part = np.empty_like(idx) if return_parts else None
     keys = np.empty((B, Hkv, L), dtype=np.float32) if return_keys else None
-    _check(lib().nacl_oracle_select(_ptr(imp), B, L, Hkv, budget_proxy, budget_random, n_sink, n_recent,
-                                    seed, layer, flags, _ptr(idx), _ptr(part), _ptr(keys)), "nacl_oracle_select")
+    prot = None if protect_idx is None else np.ascontiguousarray(np.asarray(protect_idx, dtype=np.int32))
+    opts = _SelectOpts(batch_offset, head_offset, None if prot is None else prot.ctypes.data, 0 if prot is None else prot.size,
+                       1 if shared_heads else 0)
+    _check(lib().nacl_oracle_select_ex(_ptr(imp), B, L, Hkv, budget_proxy, budget_random, n_sink, n_recent,
+                                       seed, layer, flags, C.byref(opts), _ptr(idx), _ptr(part), _ptr(keys)),
+           "nacl_oracle_select_ex")
     out = (idx,)
     if return_parts:
         out += (part,)

@@ -184,79 +184,127 @@ static int cmp_key_desc(const void* a, const void* b) {
   return (x->j > y->j) - (x->j < y->j);
 }
 
+/* Steps 4-7 for one problem: s[L] importance, (b_glob, hk_glob) = the GLOBAL batch / kv-head indices that key the
+ * random draws (R10), extra[] = n_extra further protected positions.  Writes C indices (and parts / keys). */
+static int select_one(const double* s, int L, int budget_proxy, int budget_random, int n_sink, int n_recent,
+                      const int32_t* extra, int n_extra, uint64_t seed, int layer, int b_glob, int hk_glob,
+                      unsigned flags, score_item* sc, key_item* ky, int8_t* part,
+                      int32_t* out_idx, int32_t* out_part, float* out_key) {
+  const int C = budget_proxy + budget_random;
+  const int lo = n_sink, hi = L - n_recent; /* positions [lo, hi) are not protected by the sink / recent rule */
+  for (int j = 0; j < L; ++j)
+    if (!(s[j] >= 0.0) || isinf(s[j])) return NACL_ORACLE_EARG; /* importance is a finite sum of probabilities */
+  memset(part, -1, (size_t)L);
+
+  /* step 4: protected set Pi = sinks and recent tokens (PAPER.md:137-140 "cup P", :390), plus the explicit list
+   * (Table "hyperp": protected proxy tokens count inside the proxy budget, R7) */
+  for (int j = 0; j < n_sink; ++j) part[j] = 0;
+  for (int j = hi; j < L; ++j) part[j] = 0;
+  for (int e = 0; e < n_extra; ++e) {
+    const int j = extra[e];
+    if (j < lo || j >= hi || (e > 0 && extra[e - 1] >= j)) return NACL_ORACLE_EARG; /* ascending, unique, not already protected */
+    part[j] = 0;
+  }
+  const int k1 = budget_proxy - n_sink - n_recent - n_extra; /* free top-k slots (R7) */
+  if (k1 < 0) return NACL_ORACLE_EBUDGET;
+
+  /* step 5: argmax_{S subset R, |S| = C_p} sum F_score: full sort, take the head */
+  int n_free = 0;
+  for (int j = lo; j < hi; ++j)
+    if (part[j] < 0) { sc[n_free].v = s[j]; sc[n_free].j = j; ++n_free; }
+  qsort(sc, (size_t)n_free, sizeof(score_item), cmp_score_desc);
+  for (int r = 0; r < k1; ++r) part[sc[r].j] = 1;
+
+  /* step 6: Random Eviction over the rest (R4, R5, R6) */
+  const int n_cand = n_free - k1;
+  if (out_key)
+    for (int j = 0; j < L; ++j) out_key[j] = NAN;
+  for (int r = 0; r < n_cand; ++r) {
+    const int j = sc[k1 + r].j;
+    const double u = nacl_oracle_uniform(seed, layer, b_glob, hk_glob, j);
+    ky[r].v = nacl_oracle_gumbel_key(s[j], u, flags);
+    ky[r].j = j;
+    if (out_key) out_key[j] = ky[r].v;
+  }
+  qsort(ky, (size_t)n_cand, sizeof(key_item), cmp_key_desc);
+  for (int r = 0; r < budget_random; ++r) part[ky[r].j] = 2;
+
+  /* step 7: S = u_score cup u_random, ascending */
+  int c = 0;
+  for (int j = 0; j < L; ++j) {
+    if (part[j] >= 0) {
+      if (c < C) {
+        out_idx[c] = j;
+        if (out_part) out_part[c] = part[j];
+      }
+      ++c;
+    }
+  }
+  return c == C ? 0 : NACL_ORACLE_EARG; /* cannot fail: parts are disjoint by construction */
+}
+
+int nacl_oracle_select_ex(const double* imp, int batch, int L, int Hkv,
+                          int budget_proxy, int budget_random, int n_sink, int n_recent,
+                          uint64_t seed, int layer, unsigned flags, const nacl_oracle_select_opts* opts,
+                          int32_t* out_idx, int32_t* out_part, float* out_key) {
+  if (!imp || !out_idx) return NACL_ORACLE_EARG;
+  if (batch < 1 || L < 1 || Hkv < 1) return NACL_ORACLE_EARG;
+  if (n_sink < 0 || n_recent < 0 || budget_proxy < 0 || budget_random < 0) return NACL_ORACLE_EBUDGET;
+  const int b_off = opts ? opts->batch_offset : 0, h_off = opts ? opts->head_offset : 0;
+  const int n_extra = opts ? opts->n_protect : 0;
+  const int32_t* extra = opts ? opts->protect_idx : NULL;
+  const int shared = opts ? opts->shared_heads : 0;
+  if (b_off < 0 || h_off < 0 || n_extra < 0 || (n_extra > 0 && !extra)) return NACL_ORACLE_EARG;
+  const long n_prot = (long)n_sink + n_recent;
+  if (n_prot > L) return NACL_ORACLE_EBUDGET;
+  if (budget_proxy < n_prot + n_extra) return NACL_ORACLE_EBUDGET;               /* R7 */
+  if ((long)budget_proxy + budget_random > L) return NACL_ORACLE_EBUDGET;
+  const int C = budget_proxy + budget_random;
+
+  score_item* sc = (score_item*)malloc((size_t)L * sizeof(score_item));
+  key_item* ky = (key_item*)malloc((size_t)L * sizeof(key_item));
+  int8_t* part = (int8_t*)malloc((size_t)L);
+  double* sum = shared ? (double*)malloc((size_t)L * sizeof(double)) : NULL;
+  if (!sc || !ky || !part || (shared && !sum)) { free(sc); free(ky); free(part); free(sum); return NACL_ORACLE_ENOMEM; }
+
+  int rc = 0;
+  for (int b = 0; b < batch && rc == 0; ++b) {
+    if (shared) {
+      /* the "- Head-wise" ablation (PAPER.md:319-321 Table 3, :376-380): ONE retained set per batch element, chosen on
+       * the importance summed over the kv heads in head order, drawn with the first head's stream, copied to every head */
+      for (int j = 0; j < L; ++j) {
+        double a = 0.0;
+        for (int hk = 0; hk < Hkv; ++hk) a += imp[((size_t)b * Hkv + hk) * (size_t)L + j];
+        sum[j] = a;
+      }
+      const size_t p0 = (size_t)b * Hkv;
+      rc = select_one(sum, L, budget_proxy, budget_random, n_sink, n_recent, extra, n_extra, seed, layer, b + b_off, h_off,
+                      flags, sc, ky, part, out_idx + p0 * (size_t)C, out_part ? out_part + p0 * (size_t)C : NULL,
+                      out_key ? out_key + p0 * (size_t)L : NULL);
+      for (int hk = 1; hk < Hkv && rc == 0; ++hk) {
+        memcpy(out_idx + (p0 + hk) * (size_t)C, out_idx + p0 * (size_t)C, (size_t)C * sizeof(int32_t));
+        if (out_part) memcpy(out_part + (p0 + hk) * (size_t)C, out_part + p0 * (size_t)C, (size_t)C * sizeof(int32_t));
+        if (out_key) memcpy(out_key + (p0 + hk) * (size_t)L, out_key + p0 * (size_t)L, (size_t)L * sizeof(float));
+      }
+      continue;
+    }
+    for (int hk = 0; hk < Hkv && rc == 0; ++hk) {
+      const size_t prob_id = (size_t)b * Hkv + hk;
+      rc = select_one(imp + prob_id * (size_t)L, L, budget_proxy, budget_random, n_sink, n_recent, extra, n_extra, seed, layer,
+                      b + b_off, hk + h_off, flags, sc, ky, part, out_idx + prob_id * (size_t)C,
+                      out_part ? out_part + prob_id * (size_t)C : NULL, out_key ? out_key + prob_id * (size_t)L : NULL);
+    }
+  }
+  free(sc); free(ky); free(part); free(sum);
+  return rc;
+}
+
 int nacl_oracle_select(const double* imp, int batch, int L, int Hkv,
                        int budget_proxy, int budget_random, int n_sink, int n_recent,
                        uint64_t seed, int layer, unsigned flags,
                        int32_t* out_idx, int32_t* out_part, float* out_key) {
-  if (!imp || !out_idx) return NACL_ORACLE_EARG;
-  if (batch < 1 || L < 1 || Hkv < 1) return NACL_ORACLE_EARG;
-  if (n_sink < 0 || n_recent < 0 || budget_proxy < 0 || budget_random < 0) return NACL_ORACLE_EBUDGET;
-  const long n_prot = (long)n_sink + n_recent;
-  if (n_prot > L) return NACL_ORACLE_EBUDGET;
-  if (budget_proxy < n_prot) return NACL_ORACLE_EBUDGET;               /* R7 */
-  if ((long)budget_proxy + budget_random > L) return NACL_ORACLE_EBUDGET;
-  const int C = budget_proxy + budget_random;
-  const int k1 = budget_proxy - (int)n_prot; /* free top-k slots (R7) */
-  const int lo = n_sink, hi = L - n_recent;  /* non-protected positions [lo, hi) */
-  const int n_free = hi - lo;
-
-  score_item* sc = (score_item*)malloc((size_t)(n_free > 0 ? n_free : 1) * sizeof(score_item));
-  key_item* ky = (key_item*)malloc((size_t)(n_free > 0 ? n_free : 1) * sizeof(key_item));
-  int8_t* part = (int8_t*)malloc((size_t)L);
-  if (!sc || !ky || !part) { free(sc); free(ky); free(part); return NACL_ORACLE_ENOMEM; }
-
-  int rc = 0;
-  for (int b = 0; b < batch && rc == 0; ++b) {
-    for (int hk = 0; hk < Hkv && rc == 0; ++hk) {
-      const size_t prob_id = (size_t)b * Hkv + hk;
-      const double* s = imp + prob_id * (size_t)L;
-      for (int j = 0; j < L; ++j) {
-        if (!(s[j] >= 0.0) || isinf(s[j])) { rc = NACL_ORACLE_EARG; break; } /* importance is a finite sum of probabilities */
-      }
-      if (rc) break;
-      memset(part, -1, (size_t)L);
-
-      /* step 4: protected set Pi = sinks and recent tokens (PAPER.md:137-140 "cup P", :390) */
-      for (int j = 0; j < n_sink; ++j) part[j] = 0;
-      for (int j = hi; j < L; ++j) part[j] = 0;
-
-      /* step 5: argmax_{S subset R, |S| = C_p} sum F_score: full sort, take the head */
-      for (int j = lo; j < hi; ++j) { sc[j - lo].v = s[j]; sc[j - lo].j = j; }
-      qsort(sc, (size_t)n_free, sizeof(score_item), cmp_score_desc);
-      for (int r = 0; r < k1; ++r) part[sc[r].j] = 1;
-
-      /* step 6: Random Eviction over the rest (R4, R5, R6) */
-      const int n_cand = n_free - k1;
-      if (out_key) {
-        float* ko = out_key + prob_id * (size_t)L;
-        for (int j = 0; j < L; ++j) ko[j] = NAN;
-      }
-      for (int r = 0; r < n_cand; ++r) {
-        const int j = sc[k1 + r].j;
-        const double u = nacl_oracle_uniform(seed, layer, b, hk, j);
-        ky[r].v = nacl_oracle_gumbel_key(s[j], u, flags);
-        ky[r].j = j;
-        if (out_key) out_key[prob_id * (size_t)L + j] = ky[r].v;
-      }
-      qsort(ky, (size_t)n_cand, sizeof(key_item), cmp_key_desc);
-      for (int r = 0; r < budget_random; ++r) part[ky[r].j] = 2;
-
-      /* step 7: S = u_score cup u_random, ascending */
-      int c = 0;
-      for (int j = 0; j < L; ++j) {
-        if (part[j] >= 0) {
-          if (c < C) {
-            out_idx[prob_id * (size_t)C + c] = j;
-            if (out_part) out_part[prob_id * (size_t)C + c] = part[j];
-          }
-          ++c;
-        }
-      }
-      if (c != C) rc = NACL_ORACLE_EARG; /* cannot happen: parts are disjoint by construction */
-    }
-  }
-  free(sc); free(ky); free(part);
-  return rc;
+  return nacl_oracle_select_ex(imp, batch, L, Hkv, budget_proxy, budget_random, n_sink, n_recent, seed, layer, flags, NULL,
+                               out_idx, out_part, out_key);
 }
 
 /* ----------------------------------------------------- step 8: K,V <- K_S,V_S */

@@ -76,6 +76,25 @@ int nacl_oracle_select(const double* imp, int batch, int L, int Hkv,
                        uint64_t seed, int layer, unsigned flags,
                        int32_t* out_idx, int32_t* out_part, float* out_key);
 
+/* Steps 4-7 with the options the paper's variants need (NULL opts = nacl_oracle_select):
+ *   batch_offset, head_offset: GLOBAL index of batch element 0 / kv head 0 of this call in the Philox counter (R10;
+ *       PAPER.md:37 ties the stream to the head and the layer, not to the device that holds it), so that a shard of the
+ *       heads or of the batch draws exactly what the unsharded problem draws;
+ *   protect_idx[n_protect]: further protected positions, ascending, unique, inside [n_sink, L - n_recent), the same for
+ *       every problem (Table "hyperp": "protect proxy"); they count inside budget_proxy (R7);
+ *   shared_heads != 0: the "- Head-wise" ablation: one retained set per batch element, chosen
+ *       on the importance summed over the kv heads, drawn with the stream of the call's first head. */
+typedef struct {
+  int batch_offset, head_offset;
+  const int32_t* protect_idx;
+  int n_protect;
+  int shared_heads;
+} nacl_oracle_select_opts;
+int nacl_oracle_select_ex(const double* imp, int batch, int L, int Hkv,
+                          int budget_proxy, int budget_random, int n_sink, int n_recent,
+                          uint64_t seed, int layer, unsigned flags, const nacl_oracle_select_opts* opts,
+                          int32_t* out_idx, int32_t* out_part, float* out_key);
+
 /* Step 8: K,V <- K_S,V_S by copying the original bytes. */
 int nacl_oracle_gather(const void* K, const void* V, size_t row_bytes,
                        int batch, int L, int Hkv, int C, const int32_t* idx,

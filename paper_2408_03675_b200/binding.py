@@ -34,6 +34,7 @@ class NaclParams(C.Structure):
         ("out_importance", C.c_void_p), ("out_lse", C.c_void_p),
         ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("stream", C.c_void_p),
         ("lse_in", C.c_void_p),
+        ("batch_offset", C.c_int32), ("head_offset", C.c_int32),
     ]
 
 
@@ -182,9 +183,10 @@ def nacl_evict(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed
 
 def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer, flags=0,
                   out_K=None, out_V=None, out_idx=None, want_importance=False, want_lse=False,
-                  workspace=None, stream=None, lse_in=None):
+                  workspace=None, stream=None, lse_in=None, batch_offset=0, head_offset=0):
     """include/nacl_evict.h `nacl_evict_ex`.  lse_in: optional [B,Hq,P] fp32 row log-sum-exps (single-sweep
-    path).  Returns a dict with out_K, out_V, out_idx and, if asked,
+    path).  batch_offset / head_offset: global indices of the call's first batch element / kv head (a shard of a
+    larger problem draws what the unsharded call draws).  Returns a dict with out_K, out_V, out_idx and, if asked,
     importance [B,Hkv,L] fp32 and lse [B,Hq,P] fp32."""
     B, Hkv, L, d, Hq, P = _shapes(K, V, Qproxy)
     if not K.is_cuda:
@@ -206,6 +208,7 @@ def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, s
     p.batch, p.L, p.Hq, p.Hkv, p.d, p.P = B, L, Hq, Hkv, d, P
     p.budget_proxy, p.budget_random, p.n_sink, p.n_recent = budget_proxy, budget_random, n_sink, n_recent
     p.seed, p.layer, p.flags = seed, layer, flags
+    p.batch_offset, p.head_offset = batch_offset, head_offset
     p.out_K, p.out_V, p.out_idx = out_K.data_ptr(), out_V.data_ptr(), out_idx.data_ptr()
     p.out_importance = imp.data_ptr() if imp is not None else None
     p.out_lse = lse.data_ptr() if lse is not None else None

@@ -30,19 +30,25 @@ static cudaEvent_t prof_event() {
   return e;
 }
 
-StageScope::StageScope(int stage, cudaStream_t st) : stage_(stage), st_(st), slot_(-1) {
+StageScope::StageScope(int stage, cudaStream_t st) : stage_(stage), st_(st), a_(nullptr), b_(nullptr) {
   std::lock_guard<std::mutex> lk(g_prof_mu);
   if (!g_prof_on) return;
-  ProfRecord r{stage, prof_event(), prof_event()};
-  if (!r.a || !r.b) return;
-  cudaEventRecord(r.a, st);
-  g_prof_pending.push_back(r);
-  slot_ = (int)g_prof_pending.size() - 1;
+  a_ = prof_event();
+  b_ = prof_event();
+  if (!a_ || !b_) {
+    if (a_) g_prof_free.push_back(a_);
+    if (b_) g_prof_free.push_back(b_);
+    a_ = b_ = nullptr;
+    return;
+  }
+  cudaEventRecord(a_, st);
 }
 StageScope::~StageScope() {
-  if (slot_ < 0) return;
+  if (!a_) return;
+  // the pair enters the pending list only once both events are recorded: a nacl_profile_read in between never sees half a scope
+  cudaEventRecord(b_, st_);
   std::lock_guard<std::mutex> lk(g_prof_mu);
-  if (slot_ < (int)g_prof_pending.size()) cudaEventRecord(g_prof_pending[slot_].b, st_);
+  g_prof_pending.push_back(ProfRecord{stage_, a_, b_});
 }
 
 SplitPlan make_split_plan(int batch, int L, int Hkv) {
@@ -102,12 +108,16 @@ static int validate_budget(int L, int budget_proxy, int budget_random, int n_sin
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 // ------------------------------------------------------------------ internal grow-only buffers
+// The internal workspace is keyed by (device, stream): calls on one stream are ordered and may share scratch, calls on
+// different streams may run at the same time and must not.  A buffer that is too small is replaced, but the old one
+// is only freed by nacl_release: a call enqueued earlier on the same stream may still be running out of it.
+struct WsEntry { cudaStream_t stream; void* ptr; size_t bytes; };
 struct DeviceCache {
-  void* ws = nullptr;
-  size_t ws_bytes = 0;
+  std::vector<WsEntry> ws;
+  std::vector<void*> retired;
   void* stage[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // K V Q oK oV idx
   size_t stage_bytes[6] = {0, 0, 0, 0, 0, 0};
-  cudaStream_t stream = nullptr;
+  cudaStream_t stream = nullptr;  // nacl_evict_host
 };
 static std::mutex g_mu;       // guards g_cache
 static std::mutex g_host_mu;  // serialises nacl_evict_host (its staging buffers are shared per device)
@@ -125,6 +135,31 @@ static cudaError_t grow(void** p, size_t* have, size_t want) {
   cudaError_t e = cudaMalloc(p, cap);
   if (e != cudaSuccess) { *p = nullptr; return e; }
   *have = cap;
+  return cudaSuccess;
+}
+
+// g_mu held
+static cudaError_t stream_workspace(DeviceCache& dc, cudaStream_t st, size_t want, void** out) {
+  for (WsEntry& w : dc.ws)
+    if (w.stream == st) {
+      if (w.bytes < want) {
+        dc.retired.push_back(w.ptr);
+        const size_t cap = want + want / 8 + 256;
+        void* np = nullptr;
+        cudaError_t e = cudaMalloc(&np, cap);
+        if (e != cudaSuccess) { dc.retired.pop_back(); return e; }
+        w.ptr = np;
+        w.bytes = cap;
+      }
+      *out = w.ptr;
+      return cudaSuccess;
+    }
+  const size_t cap = want + want / 8 + 256;
+  void* np = nullptr;
+  cudaError_t e = cudaMalloc(&np, cap);
+  if (e != cudaSuccess) return e;
+  dc.ws.push_back(WsEntry{st, np, cap});
+  *out = np;
   return cudaSuccess;
 }
 
@@ -157,35 +192,35 @@ static int evict_impl(const nacl_params_t& p) {
       (reinterpret_cast<uintptr_t>(p.out_idx) & 3u))
     return NACL_ERR_ALIGN;
 
+  if (p.batch_offset < 0 || p.head_offset < 0) return NACL_ERR_SHAPE;
   const size_t need = nacl_workspace_bytes(p.batch, p.L, p.Hq, p.Hkv, p.d, p.P);
+  cudaStream_t st = static_cast<cudaStream_t>(p.stream);
+  cudaError_t e;
   void* wsp = p.workspace;
   if (wsp) {
     if (p.workspace_bytes < need || (reinterpret_cast<uintptr_t>(wsp) & 255u)) return NACL_ERR_WORKSPACE;
   } else {
     int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return fail_cuda(e);
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return fail_cuda(e);
     if (dev < 0 || dev >= 64) return NACL_ERR_UNSUPPORTED;
     std::lock_guard<std::mutex> lk(g_mu);
-    e = grow(&g_cache[dev].ws, &g_cache[dev].ws_bytes, need);
+    e = stream_workspace(g_cache[dev], st, need, &wsp);
     if (e != cudaSuccess) return fail_cuda(e);
-    wsp = g_cache[dev].ws;
   }
   const Workspace ws = carve_workspace(wsp, p.batch, p.L, p.Hq, p.Hkv, p.P);
   const SplitPlan sp = make_split_plan(p.batch, p.L, p.Hkv);
-  cudaStream_t st = static_cast<cudaStream_t>(p.stream);
 
-  cudaError_t e;
   const bool tc = !(p.flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
   if (p.lse_in && (reinterpret_cast<uintptr_t>(p.lse_in) & 3u)) return NACL_ERR_ALIGN;
-  if (tc) e = launch_score_tc(s, p.K, p.Qproxy, sp, ws, p.lse_in, (p.flags & NACL_FLAG_CAUSAL) != 0, p.out_importance, p.out_lse, st);
-  else e = launch_score_generic(s, p.K, p.Qproxy, sp, ws, p.lse_in, (p.flags & NACL_FLAG_CAUSAL) != 0, p.out_importance, p.out_lse, st);
+  const int C = p.budget_proxy + p.budget_random;
+  const bool causal = (p.flags & NACL_FLAG_CAUSAL) != 0;
+  if (tc) e = launch_score_tc(s, p.K, p.Qproxy, sp, ws, p.lse_in, causal, p.out_importance, p.out_lse, st);
+  else e = launch_score_generic(s, p.K, p.Qproxy, sp, ws, p.lse_in, causal, p.out_importance, p.out_lse, st);
   if (e != cudaSuccess) return fail_cuda(e);
 
-  const int C = p.budget_proxy + p.budget_random;
   bool gathered = false;
   e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
-                    p.flags, p.out_idx, p.K, p.V, p.out_K, p.out_V, row_bytes, &gathered, st);
+                    p.flags, p.out_idx, p.K, p.V, p.out_K, p.out_V, row_bytes, &gathered, p.batch_offset, p.head_offset, st);
   if (e != cudaSuccess) return fail_cuda(e);
   if (!gathered) {
     StageScope sc(ST_GATHER, st);
@@ -240,7 +275,9 @@ int nacl_evict_ex(const nacl_params_t* p) {
 int nacl_evict_host(const void* K, const void* V, const void* Qproxy, int dtype, int batch, int L, int Hq, int Hkv, int d,
                     int P, int budget_proxy, int budget_random, int n_sink, int n_recent, uint64_t seed, int layer,
                     void* out_K, void* out_V, int32_t* out_idx, int device) {
-  if (!K || !V || !Qproxy || !out_K || !out_V || !out_idx) return NACL_ERR_NULL;
+  if (!K || !V || !Qproxy) return NACL_ERR_NULL;
+  const bool empty_out = budget_proxy == 0 && budget_random == 0;  // empty outputs: their pointers may be NULL
+  if (!empty_out && (!out_K || !out_V || !out_idx)) return NACL_ERR_NULL;
   int rc = validate_shape(dtype, batch, L, Hq, Hkv, d, P);
   if (rc) return rc;
   rc = validate_budget(L, budget_proxy, budget_random, n_sink, n_recent);
@@ -303,7 +340,7 @@ int nacl_gumbel_keys(const float* importance, float* out_keys, int batch, int Hk
   if ((reinterpret_cast<uintptr_t>(importance) | reinterpret_cast<uintptr_t>(out_keys)) & 3u) return NACL_ERR_ALIGN;
   const uint32_t known = NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE | NACL_FLAG_SAMPLE_UNIFORM;
   if ((flags & ~known) || flags == known) return NACL_ERR_UNSUPPORTED;
-  cudaError_t e = launch_keys(importance, reinterpret_cast<uint32_t*>(out_keys), batch, Hkv, L, seed, layer, flags, false,
+  cudaError_t e = launch_keys(importance, reinterpret_cast<uint32_t*>(out_keys), batch, Hkv, L, seed, layer, flags, false, 0, 0,
                               static_cast<cudaStream_t>(stream));
   return e == cudaSuccess ? NACL_OK : fail_cuda(e);
 }
@@ -369,11 +406,13 @@ void nacl_release(void) {
   if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return; }
   for (int dev = 0; dev < 64; ++dev) {
     DeviceCache& dc = g_cache[dev];
-    bool any = dc.ws || dc.stream;
+    bool any = !dc.ws.empty() || !dc.retired.empty() || dc.stream;
     for (int i = 0; i < 6; ++i) any = any || dc.stage[i];
     if (!any) continue;
     if (cudaSetDevice(dev) != cudaSuccess) { cudaGetLastError(); continue; }
-    if (dc.ws) cudaFree(dc.ws);
+    cudaDeviceSynchronize();  // retired workspaces may still be in use by enqueued calls
+    for (WsEntry& w : dc.ws) cudaFree(w.ptr);
+    for (void* q : dc.retired) cudaFree(q);
     for (int i = 0; i < 6; ++i) if (dc.stage[i]) cudaFree(dc.stage[i]);
     if (dc.stream) cudaStreamDestroy(dc.stream);
     dc = DeviceCache();

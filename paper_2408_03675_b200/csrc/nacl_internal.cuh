@@ -50,7 +50,7 @@ struct StageScope {
   ~StageScope();
   int stage_;
   cudaStream_t st_;
-  int slot_;  // -1 when profiling is off
+  cudaEvent_t a_, b_;  // null when profiling is off
 };
 
 // ------------------------------------------------------------------ kernels (launchers)
@@ -70,8 +70,9 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
                             const Workspace& ws, const float* lse_in, bool causal, float* imp_out, float* lse_out, cudaStream_t st);
 
 // Gumbel-top-k keys: key[p,j] = fl32(ln w(imp) - ln(-ln u)), order-mapped to uint32 (ordermapped) or as float bits
+// batch_offset / head_offset: global indices of the call's first batch element / kv head (Philox counter words)
 cudaError_t launch_keys(const float* imp, uint32_t* key, int batch, int Hkv, int L, uint64_t seed, int layer, uint32_t flags,
-                        bool ordermapped, cudaStream_t st);
+                        bool ordermapped, int batch_offset, int head_offset, cudaStream_t st);
 
 // protected + top-k + Gumbel-top-k (keys fused when the row fits a cluster's shared memory) + ascending
 // compaction -> out_idx.  Records its own StageScopes.  `key` is scratch for the long-row fallback.
@@ -81,7 +82,7 @@ size_t select_scratch_words(int batch, int Hkv, int L);  // 4-byte words of Work
 cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, int L, int budget_proxy, int budget_random,
                           int n_sink, int n_recent, uint64_t seed, int layer, uint32_t flags, int32_t* out_idx,
                           const void* K, const void* V, void* out_K, void* out_V, int row_bytes, bool* gathered,
-                          cudaStream_t st);
+                          int batch_offset, int head_offset, cudaStream_t st);
 
 // K,V <- K_S,V_S
 cudaError_t launch_gather(const void* K, const void* V, const int32_t* idx, int n_prob, int L, int C,

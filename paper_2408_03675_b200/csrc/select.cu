@@ -186,13 +186,14 @@ __device__ __forceinline__ uint32_t gumbel_key(float imp, uint32_t j, uint32_t h
 
 template <bool ORDERMAP>
 __global__ void __launch_bounds__(256) nacl_keys_kernel(const float* __restrict__ imp, uint32_t* __restrict__ key,
-                                                    int Hkv, int L, uint32_t k0, uint32_t k1, uint32_t layer, uint32_t flags) {
+                                                    int Hkv, int L, uint32_t k0, uint32_t k1, uint32_t layer, uint32_t flags,
+                                                    uint32_t b_off, uint32_t h_off) {
   const int p = blockIdx.y;  // b * Hkv + hk
   const int b = p / Hkv, hk = p - b * Hkv;
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= L) return;
   const size_t o = (size_t)p * L + j;
-  key[o] = gumbel_key<ORDERMAP>(imp[o], (uint32_t)j, (uint32_t)hk, (uint32_t)b, layer, k0, k1, flags);
+  key[o] = gumbel_key<ORDERMAP>(imp[o], (uint32_t)j, (uint32_t)hk + h_off, (uint32_t)b + b_off, layer, k0, k1, flags);
 }
 
 // ------------------------------------------------------------------ block primitives
@@ -572,7 +573,8 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
                                                                  int n_sink, int n_recent, int C, uint32_t sk0, uint32_t sk1,
                                                                  uint32_t layer, uint32_t flags, int32_t* __restrict__ out_idx,
                                                                  const int4* __restrict__ Kv, const int4* __restrict__ Vv,
-                                                                 int4* __restrict__ oKv, int4* __restrict__ oVv, int vpr) {
+                                                                 int4* __restrict__ oKv, int4* __restrict__ oVv, int vpr,
+                                                                 uint32_t b_off, uint32_t h_off) {
   cg::cluster_group cluster = cg::this_cluster();
   extern __shared__ __align__(16) unsigned char dyn_raw[];
   ClShared& sh = *reinterpret_cast<ClShared*>(dyn_raw);
@@ -608,16 +610,17 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
     // four independent fp64 log chains per thread in flight
     for (int base = 0; base < nloc; base += 4 * ST) {
       uint32_t kk[4];
+      bool cand[4];
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
         const int i = base + u * ST + (int)threadIdx.x;
-        kk[u] = gumbel_key(i < nloc ? row[i] : 1.f, (uint32_t)(j0 + i), (uint32_t)hk, (uint32_t)b, layer, sk0, sk1, flags);
+        cand[u] = i < nloc && free_pos(i) && !in_topk(i);
+        if (cand[u])
+          kk[u] = gumbel_key(row[i], (uint32_t)(j0 + i), (uint32_t)hk + h_off, (uint32_t)b + b_off, layer, sk0, sk1, flags);
       }
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int i = base + u * ST + (int)threadIdx.x;
-        if (i < nloc && free_pos(i) && !in_topk(i)) kb[i] = kk[u];
-      }
+      for (int u = 0; u < 4; ++u)
+        if (cand[u]) kb[base + u * ST + (int)threadIdx.x] = kk[u];
     }
     __syncthreads();
   }
@@ -686,11 +689,13 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
 }  // namespace
 
 cudaError_t launch_keys(const float* imp, uint32_t* key, int batch, int Hkv, int L, uint64_t seed, int layer,
-                        uint32_t flags, bool ordermapped, cudaStream_t st) {
+                        uint32_t flags, bool ordermapped, int batch_offset, int head_offset, cudaStream_t st) {
   dim3 grid((L + 255) / 256, batch * Hkv);
   const uint32_t sk0 = (uint32_t)(seed & 0xFFFFFFFFu), sk1 = (uint32_t)(seed >> 32);
-  if (ordermapped) nacl_keys_kernel<true><<<grid, 256, 0, st>>>(imp, key, Hkv, L, sk0, sk1, (uint32_t)layer, flags);
-  else nacl_keys_kernel<false><<<grid, 256, 0, st>>>(imp, key, Hkv, L, sk0, sk1, (uint32_t)layer, flags);
+  if (ordermapped)
+    nacl_keys_kernel<true><<<grid, 256, 0, st>>>(imp, key, Hkv, L, sk0, sk1, (uint32_t)layer, flags, (uint32_t)batch_offset, (uint32_t)head_offset);
+  else
+    nacl_keys_kernel<false><<<grid, 256, 0, st>>>(imp, key, Hkv, L, sk0, sk1, (uint32_t)layer, flags, (uint32_t)batch_offset, (uint32_t)head_offset);
   return cudaGetLastError();
 }
 
@@ -702,7 +707,7 @@ bool select_uses_cluster(int L) { return (L + kMaxRanks - 1) / kMaxRanks <= kMax
 cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, int L, int budget_proxy, int budget_random,
                           int n_sink, int n_recent, uint64_t seed, int layer, uint32_t flags, int32_t* out_idx,
                           const void* K, const void* V, void* out_K, void* out_V, int row_bytes, bool* gathered,
-                          cudaStream_t st) {
+                          int batch_offset, int head_offset, cudaStream_t st) {
   *gathered = false;
   const int C = budget_proxy + budget_random;
   if (C == 0) return cudaSuccess;
@@ -712,7 +717,7 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
     // very long rows: sampling keys in a kernel of their own, one CTA per head working out of global memory
     if (budget_random > 0) {
       StageScope sc(ST_KEYS, st);
-      cudaError_t e = launch_keys(imp, key, batch, Hkv, L, seed, layer, flags, true, st);
+      cudaError_t e = launch_keys(imp, key, batch, Hkv, L, seed, layer, flags, true, batch_offset, head_offset, st);
       if (e != cudaSuccess) return e;
     }
     StageScope sc(ST_SELECT, st);
@@ -768,7 +773,7 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   StageScope sc(ST_SELECT, st);
   return cudaLaunchKernelEx(&cfg, nacl_select_cluster_kernel, imp, Hkv, L, Lc, k1, budget_random, n_sink, n_recent, C, sk0, sk1,
                             (uint32_t)layer, flags, out_idx, (const int4*)K, (const int4*)V, (int4*)out_K, (int4*)out_V,
-                            (*gathered = (K != nullptr)) ? row_bytes / 16 : 0);
+                            (*gathered = (K != nullptr)) ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset);
 }
 
 // 4-byte words of the `key` scratch the select needs (long-row path: the keys)

@@ -299,3 +299,62 @@ def test_gather_is_a_bytewise_row_copy():
                 np.testing.assert_array_equal(oV[b, h], V[b, h, idx[b, h]])
     with pytest.raises(oracle.OracleError):
         oracle.gather(K, V, np.full((2, 3, 1), 17, dtype=np.int32))
+
+
+# ------------------------------------------------------------------ options of nacl_oracle_select_ex
+def test_offsets_make_a_shard_draw_what_the_unsharded_call_draws():
+    """PAPER.md:37 ties the random stream to the head and the layer (R10: counter = (position, kv head, batch, layer)):
+    a slice of the heads or of the batch, told where it starts, reproduces the slice of the unsharded result; without
+    the offsets it does not (the draws differ)."""
+    rng = np.random.default_rng(3)
+    imp = rng.random((3, 4, 200))
+    full, parts = oracle.select(imp, 30, 25, 2, 5, seed=11, layer=2, return_parts=True)
+    for h0, h1 in [(0, 2), (2, 4), (1, 4)]:
+        np.testing.assert_array_equal(oracle.select(imp[:, h0:h1], 30, 25, 2, 5, 11, 2, head_offset=h0), full[:, h0:h1])
+    for b0 in (1, 2):
+        np.testing.assert_array_equal(oracle.select(imp[b0:], 30, 25, 2, 5, 11, 2, batch_offset=b0), full[b0:])
+    assert not np.array_equal(oracle.select(imp[:, 2:4], 30, 25, 2, 5, 11, 2), full[:, 2:4])
+    # the top-k part never depends on the offsets
+    sl, sp = oracle.select(imp[:, 2:4], 30, 25, 2, 5, 11, 2, return_parts=True)
+    for b in range(3):
+        for h in range(2):
+            assert set(sl[b, h][sp[b, h] == 1]) == set(full[b, 2 + h][parts[b, 2 + h] == 1])
+
+
+def test_explicit_protected_positions_reduce_to_infinite_importance():
+    """Table "hyperp": protected proxy tokens are kept by default and count inside the proxy budget
+    (R7).  Protecting a position is the same as giving it an importance above every other one and taking the same
+    top-Bp: the base routine on the modified scores is the referee."""
+    rng = np.random.default_rng(5)
+    for _ in range(20):
+        L = int(rng.integers(30, 120))
+        imp = rng.random((2, 2, L))
+        ns, nr = int(rng.integers(0, 4)), int(rng.integers(0, 6))
+        free = np.arange(ns, L - nr)
+        prot = np.sort(rng.choice(free, size=int(rng.integers(1, 6)), replace=False))
+        Bp = ns + nr + len(prot) + int(rng.integers(0, 8))
+        Br = int(rng.integers(0, min(10, L - Bp) + 1))
+        idx, part = oracle.select(imp, Bp, Br, ns, nr, 4, 1, protect_idx=prot, return_parts=True)
+        big = imp.copy()
+        big[..., prot] = 1e30
+        ref = oracle.select(big, Bp, Br, ns, nr, 4, 1)
+        np.testing.assert_array_equal(idx, ref)
+        for b in range(2):
+            for h in range(2):
+                assert set(prot.tolist()) <= set(idx[b, h][part[b, h] == 0].tolist())
+    with pytest.raises(oracle.OracleError):
+        oracle.select(imp, ns + nr + 1, 0, ns, nr, 0, 0, protect_idx=prot[:3] if len(prot) >= 3 else np.array([ns, ns + 1, ns + 2]))
+    with pytest.raises(oracle.OracleError):
+        oracle.select(imp, Bp + 3, 0, ns, nr, 0, 0, protect_idx=[free[1], free[0]])  # not ascending
+
+
+def test_shared_heads_is_one_selection_on_the_head_summed_importance():
+    """The "- Head-wise" ablation: every head of a batch element keeps the same positions,
+    those a single-head call selects on the sum of the heads' importances."""
+    rng = np.random.default_rng(8)
+    imp = rng.random((2, 4, 150))
+    idx = oracle.select(imp, 20, 15, 2, 4, 9, 3, shared_heads=True, head_offset=4)
+    summed = imp[:, 0] + imp[:, 1] + imp[:, 2] + imp[:, 3]
+    ref = oracle.select(summed[:, None, :], 20, 15, 2, 4, 9, 3, head_offset=4)
+    for h in range(4):
+        np.testing.assert_array_equal(idx[:, h], ref[:, 0])

@@ -82,6 +82,10 @@ extern "C" {
 #define NACL_FLAG_CAUSAL 1u                  /* DESIGN.md R1: proxy row i is prompt position L-P+i and sees keys j <= L-P+i */
 #define NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE 2u /* sampling weight exp(imp_j) (R4) */
 #define NACL_FLAG_SAMPLE_UNIFORM 4u          /* uniform sampling weights (paper's ablation) */
+#define NACL_FLAG_SHARED_HEADS 8u            /* the paper's "- Head-wise" ablation: ONE retained set
+                                                per batch element, selected on the importance summed over its kv heads (fp32, in
+                                                head order) and drawn with the random stream of the call's first head; every
+                                                head's out_idx row holds that set and out_K/out_V are gathered with it */
 #define NACL_FLAG_SCORE_CUDA_CORES 0x100u    /* debugging: run the generic CUDA-core scoring kernels even where
                                                 the tensor-core path applies */
 
@@ -104,16 +108,28 @@ typedef struct nacl_params {
   void* workspace;                 /* optional; >= nacl_workspace_bytes(...) bytes, 256-byte aligned */
   size_t workspace_bytes;
   void* stream;                    /* cudaStream_t */
-  const float* lse_in;             /* optional [batch,Hq,P] fp32: ln sum_j exp(s[i,j]) of every proxy row over ALL L keys, as a
+  const float* lse_in;             /* optional [batch,Hq,P] fp32: the natural-log row normaliser of every proxy row, as a
                                       prefill attention kernel that keeps its softmax statistics already has it (the contract of
                                       the paper's Algorithm 2).  When given, the statistics sweep over K is
-                                      skipped: one logit sweep instead of two.  The caller answers for its accuracy. */
+                                      skipped: one logit sweep instead of two.  WHICH normaliser, by flags:
+                                        default (no mask, R1): ln sum_{j < L} exp(s[i,j]) over ALL L keys -- a causal
+                                          prefill's LSE of row i misses the keys j > L-P+i and is NOT this quantity;
+                                        NACL_FLAG_CAUSAL: ln sum_{j <= L-P+i} exp(s[i,j]), exactly what a causal forward pass
+                                          stores (Algorithm 2 proper).
+                                      The caller answers for its accuracy: imp[j] = sum_i exp(s[i,j] - lse_in[i]). */
   int32_t batch_offset;            /* global index of this call's batch element 0 and ...                                  */
   int32_t head_offset;             /* ... of its kv head 0: the Random Eviction draws are keyed by the GLOBAL (layer, batch,
                                       kv head, position) ("different seed on attention heads and layers"), so a
                                       caller that holds a slice of the heads (tensor parallel) or of the batch (data parallel)
                                       passes where its slice starts and draws exactly what the unsharded call draws.  >= 0;
                                       0 for an unsharded call */
+  const int32_t* protect_idx;      /* optional DEVICE array [n_protect]: further protected positions (Table "hyperp",
+                                      PAPER.md:490-494: "protect proxy"), strictly ascending, inside [n_sink, L - n_recent), the
+                                      same for every batch element and head.  They are always retained and count inside
+                                      budget_proxy (R7): budget_proxy >= n_sink + n_recent + n_protect.  The
+                                      contents are the caller's responsibility (validation never reads device memory) */
+  int32_t n_protect;
+  int32_t reserved0;               /* 0 */
 } nacl_params_t;
 
 /* bf16 K/V/Q.  Steps 1-7 above on `stream`. */

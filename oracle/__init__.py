@@ -160,8 +160,14 @@ def gather(K, V, idx):
 
 
 def evict(K, V, Q, budget_proxy: int, budget_random: int, n_sink: int, n_recent: int,
-          seed: int, layer: int, flags: int = 0, nthreads: int = 0, return_importance: bool = False):
-    """Steps 1-8.  Returns (out_K, out_V, out_idx[, imp])."""
+          seed: int, layer: int, flags: int = 0, nthreads: int = 0, return_importance: bool = False, **sel_opts):
+    """Steps 1-8.  Returns (out_K, out_V, out_idx[, imp]).  sel_opts (batch_offset, head_offset, protect_idx,
+    shared_heads): the three stages called one after the other with nacl_oracle_select_ex in the middle."""
+    if sel_opts:
+        imp = importance(K, Q, flags=flags & CAUSAL, nthreads=nthreads)
+        idx = select(imp, budget_proxy, budget_random, n_sink, n_recent, seed, layer, flags, **sel_opts)
+        oK, oV = gather(K, V, idx)
+        return (oK, oV, idx, imp) if return_importance else (oK, oV, idx)
     K, V, Q = as_host_array(K), as_host_array(V), as_host_array(Q)
     B, Hkv, L, d = K.shape
     _, Hq, P, _ = Q.shape

@@ -15,7 +15,7 @@ import torch
 from . import build as _build
 
 NACL_DTYPE_F32, NACL_DTYPE_BF16 = 0, 1
-FLAG_CAUSAL, FLAG_SAMPLE_SOFTMAX_OF_SCORE, FLAG_SAMPLE_UNIFORM, FLAG_SCORE_CUDA_CORES = 1, 2, 4, 0x100
+FLAG_CAUSAL, FLAG_SAMPLE_SOFTMAX_OF_SCORE, FLAG_SAMPLE_UNIFORM, FLAG_SHARED_HEADS, FLAG_SCORE_CUDA_CORES = 1, 2, 4, 8, 0x100
 
 EXPORTS = ("nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes",
            "nacl_launch_count", "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version",
@@ -35,6 +35,7 @@ class NaclParams(C.Structure):
         ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("stream", C.c_void_p),
         ("lse_in", C.c_void_p),
         ("batch_offset", C.c_int32), ("head_offset", C.c_int32),
+        ("protect_idx", C.c_void_p), ("n_protect", C.c_int32), ("reserved0", C.c_int32),
     ]
 
 
@@ -183,7 +184,7 @@ def nacl_evict(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed
 
 def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer, flags=0,
                   out_K=None, out_V=None, out_idx=None, want_importance=False, want_lse=False,
-                  workspace=None, stream=None, lse_in=None, batch_offset=0, head_offset=0):
+                  workspace=None, stream=None, lse_in=None, batch_offset=0, head_offset=0, protect_idx=None):
     """include/nacl_evict.h `nacl_evict_ex`.  lse_in: optional [B,Hq,P] fp32 row log-sum-exps (single-sweep
     path).  batch_offset / head_offset: global indices of the call's first batch element / kv head (a shard of a
     larger problem draws what the unsharded call draws).  Returns a dict with out_K, out_V, out_idx and, if asked,
@@ -209,6 +210,9 @@ def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, s
     p.budget_proxy, p.budget_random, p.n_sink, p.n_recent = budget_proxy, budget_random, n_sink, n_recent
     p.seed, p.layer, p.flags = seed, layer, flags
     p.batch_offset, p.head_offset = batch_offset, head_offset
+    if protect_idx is not None:
+        assert protect_idx.is_cuda and protect_idx.dtype == torch.int32 and protect_idx.is_contiguous() and protect_idx.dim() == 1
+        p.protect_idx, p.n_protect = protect_idx.data_ptr(), protect_idx.numel()
     p.out_K, p.out_V, p.out_idx = out_K.data_ptr(), out_V.data_ptr(), out_idx.data_ptr()
     p.out_importance = imp.data_ptr() if imp is not None else None
     p.out_lse = lse.data_ptr() if lse is not None else None

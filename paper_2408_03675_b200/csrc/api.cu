@@ -81,6 +81,8 @@ Workspace carve_workspace(void* base, int batch, int L, int Hq, int Hkv, int P) 
   ws.imp = reinterpret_cast<float*>(b + off);   off = align_up(off + n_imp * sizeof(float), 256);
   ws.key = reinterpret_cast<uint32_t*>(b + off); off = align_up(off + select_scratch_words(batch, Hkv, L) * sizeof(uint32_t), 256);
   ws.sync = reinterpret_cast<int*>(b + off);    off = align_up(off + sync_ints((size_t)batch * Hkv) * sizeof(int), 256);
+  ws.imp_sh = reinterpret_cast<float*>(b + off); off = align_up(off + (size_t)batch * L * sizeof(float), 256);
+  ws.idx_sh = reinterpret_cast<int32_t*>(b + off); off = align_up(off + (size_t)batch * L * sizeof(int32_t), 256);
   ws.bytes = off;
   return ws;
 }
@@ -96,11 +98,11 @@ static int validate_shape(int dtype, int batch, int L, int Hq, int Hkv, int d, i
   return NACL_OK;
 }
 
-static int validate_budget(int L, int budget_proxy, int budget_random, int n_sink, int n_recent) {
-  if (budget_proxy < 0 || budget_random < 0 || n_sink < 0 || n_recent < 0) return NACL_ERR_BUDGET;
+static int validate_budget(int L, int budget_proxy, int budget_random, int n_sink, int n_recent, int n_protect = 0) {
+  if (budget_proxy < 0 || budget_random < 0 || n_sink < 0 || n_recent < 0 || n_protect < 0) return NACL_ERR_BUDGET;
   const long n_prot = (long)n_sink + n_recent;
   if (n_prot > L) return NACL_ERR_BUDGET;
-  if (budget_proxy < n_prot) return NACL_ERR_BUDGET;  // protected tokens count inside budget_proxy (R7)
+  if (budget_proxy < n_prot + n_protect) return NACL_ERR_BUDGET;  // protected tokens count inside budget_proxy (R7)
   if ((long)budget_proxy + budget_random > L) return NACL_ERR_BUDGET;
   return NACL_OK;
 }
@@ -177,9 +179,12 @@ static int evict_impl(const nacl_params_t& p) {
   if (!empty_out && (!p.out_K || !p.out_V || !p.out_idx)) return NACL_ERR_NULL;
   int rc = validate_shape(p.dtype, p.batch, p.L, p.Hq, p.Hkv, p.d, p.P);
   if (rc) return rc;
-  rc = validate_budget(p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent);
+  rc = validate_budget(p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.n_protect);
   if (rc) return rc;
-  const uint32_t known = NACL_FLAG_CAUSAL | NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE | NACL_FLAG_SAMPLE_UNIFORM | NACL_FLAG_SCORE_CUDA_CORES;
+  if (p.n_protect > 0 && !p.protect_idx) return NACL_ERR_NULL;
+  if (p.reserved0 != 0) return NACL_ERR_UNSUPPORTED;
+  const uint32_t known = NACL_FLAG_CAUSAL | NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE | NACL_FLAG_SAMPLE_UNIFORM | NACL_FLAG_SHARED_HEADS |
+                         NACL_FLAG_SCORE_CUDA_CORES;
   if (p.flags & ~known) return NACL_ERR_UNSUPPORTED;
   if ((p.flags & NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE) && (p.flags & NACL_FLAG_SAMPLE_UNIFORM)) return NACL_ERR_UNSUPPORTED;
 
@@ -219,8 +224,19 @@ static int evict_impl(const nacl_params_t& p) {
   if (e != cudaSuccess) return fail_cuda(e);
 
   bool gathered = false;
-  e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
-                    p.flags, p.out_idx, p.K, p.V, p.out_K, p.out_V, row_bytes, &gathered, p.batch_offset, p.head_offset, st);
+  if (p.flags & NACL_FLAG_SHARED_HEADS) {
+    // one selection per batch element on the head-summed importance (a [batch, 1, L] problem drawn with the stream of the
+    // call's first head), then the same index row for every head and the stand-alone gather
+    if ((e = launch_head_sum(ws.imp, ws.imp_sh, p.batch, p.Hkv, p.L, st)) != cudaSuccess) return fail_cuda(e);
+    if ((e = launch_protect(ws.imp_sh, p.batch, p.L, p.protect_idx, p.n_protect, st)) != cudaSuccess) return fail_cuda(e);
+    e = launch_select(ws.imp_sh, ws.key, p.batch, 1, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
+                      p.flags, ws.idx_sh, nullptr, nullptr, nullptr, nullptr, row_bytes, &gathered, p.batch_offset, p.head_offset, st);
+    if (e == cudaSuccess) e = launch_replicate_idx(ws.idx_sh, p.out_idx, p.batch, p.Hkv, C, st);
+  } else {
+    if ((e = launch_protect(ws.imp, p.batch * p.Hkv, p.L, p.protect_idx, p.n_protect, st)) != cudaSuccess) return fail_cuda(e);
+    e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
+                      p.flags, p.out_idx, p.K, p.V, p.out_K, p.out_V, row_bytes, &gathered, p.batch_offset, p.head_offset, st);
+  }
   if (e != cudaSuccess) return fail_cuda(e);
   if (!gathered) {
     StageScope sc(ST_GATHER, st);

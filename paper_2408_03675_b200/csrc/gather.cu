@@ -54,7 +54,47 @@ __global__ void __launch_bounds__(GT) nacl_gather_kernel(const int4* __restrict_
   }
 }
 
+// ---- small helpers of the selection variants
+__global__ void __launch_bounds__(256) nacl_head_sum_kernel(const float* __restrict__ imp, float* __restrict__ out, int Hkv, int L) {
+  const int b = blockIdx.y;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= L) return;
+  float a = 0.f;
+  for (int hk = 0; hk < Hkv; ++hk) a = __fadd_rn(a, imp[((size_t)b * Hkv + hk) * L + j]);  // head order, no contraction
+  out[(size_t)b * L + j] = a;
+}
+__global__ void __launch_bounds__(256) nacl_replicate_idx_kernel(const int32_t* __restrict__ shared, int32_t* __restrict__ idx,
+                                                                 int Hkv, int C) {
+  const int b = blockIdx.y;
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= C) return;
+  const int32_t v = shared[(size_t)b * C + c];
+  for (int hk = 0; hk < Hkv; ++hk) idx[((size_t)b * Hkv + hk) * C + c] = v;
+}
+__global__ void __launch_bounds__(256) nacl_protect_kernel(float* __restrict__ imp, int L, const int32_t* __restrict__ protect_idx,
+                                                           int n_protect) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n_protect) return;
+  const int j = protect_idx[e];
+  if (j >= 0 && j < L) imp[(size_t)blockIdx.y * L + j] = __int_as_float(0x7F800000);
+}
+
 }  // namespace
+
+cudaError_t launch_head_sum(const float* imp, float* out, int batch, int Hkv, int L, cudaStream_t st) {
+  nacl_head_sum_kernel<<<dim3((L + 255) / 256, batch), 256, 0, st>>>(imp, out, Hkv, L);
+  return cudaGetLastError();
+}
+cudaError_t launch_replicate_idx(const int32_t* shared, int32_t* idx, int batch, int Hkv, int C, cudaStream_t st) {
+  if (C == 0) return cudaSuccess;
+  nacl_replicate_idx_kernel<<<dim3((C + 255) / 256, batch), 256, 0, st>>>(shared, idx, Hkv, C);
+  return cudaGetLastError();
+}
+cudaError_t launch_protect(float* imp, int n_prob, int L, const int32_t* protect_idx, int n_protect, cudaStream_t st) {
+  if (n_protect == 0) return cudaSuccess;
+  nacl_protect_kernel<<<dim3((n_protect + 255) / 256, n_prob), 256, 0, st>>>(imp, L, protect_idx, n_protect);
+  return cudaGetLastError();
+}
 
 cudaError_t launch_gather(const void* K, const void* V, const int32_t* idx, int n_prob, int L, int C, int row_bytes,
                           void* out_K, void* out_V, cudaStream_t st) {

@@ -37,6 +37,8 @@ struct Workspace {
   float* imp;          // [batch*Hkv, L]          importance F_score
   uint32_t* key;       // select scratch (select_scratch_words): global radix histograms, or [batch*Hkv, L] keys for very long rows
   int* sync;           // [sync_ints(heads)]      reserved (counters / flags for future fused variants)
+  float* imp_sh;       // [batch, L]              NACL_FLAG_SHARED_HEADS: importance summed over the kv heads
+  int32_t* idx_sh;     // [batch, L]              NACL_FLAG_SHARED_HEADS: the shared retained set (C <= L entries per batch element)
   size_t bytes;
 };
 inline size_t sync_ints(size_t heads) { return 16 + 2 * heads; }
@@ -83,6 +85,13 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
                           int n_sink, int n_recent, uint64_t seed, int layer, uint32_t flags, int32_t* out_idx,
                           const void* K, const void* V, void* out_K, void* out_V, int row_bytes, bool* gathered,
                           int batch_offset, int head_offset, cudaStream_t st);
+
+// NACL_FLAG_SHARED_HEADS: out[b, j] = sum over the kv heads (in head order, fp32) of imp[b, hk, j]
+cudaError_t launch_head_sum(const float* imp, float* out, int batch, int Hkv, int L, cudaStream_t st);
+// NACL_FLAG_SHARED_HEADS: idx[b, hk, :] = shared[b, :] for every kv head
+cudaError_t launch_replicate_idx(const int32_t* shared, int32_t* idx, int batch, int Hkv, int C, cudaStream_t st);
+// explicit protected positions: imp[p, protect_idx[e]] = +inf for every problem p (the selects then keep them first)
+cudaError_t launch_protect(float* imp, int n_prob, int L, const int32_t* protect_idx, int n_protect, cudaStream_t st);
 
 // K,V <- K_S,V_S
 cudaError_t launch_gather(const void* K, const void* V, const int32_t* idx, int n_prob, int L, int C,

@@ -41,8 +41,8 @@ def check_scores(imp_gpu: np.ndarray, imp_ref: np.ndarray, G: int, P: int):
     return float(np.max(err / (np.abs(imp_ref) + 1e-300)))
 
 
-def check_staged(idx_gpu: np.ndarray, imp_gpu: np.ndarray, Bp, Br, n_sink, n_recent, seed, layer, flags=0):
-    idx_st, part_st = oracle.select(imp_gpu, Bp, Br, n_sink, n_recent, seed, layer, flags, return_parts=True)
+def check_staged(idx_gpu: np.ndarray, imp_gpu: np.ndarray, Bp, Br, n_sink, n_recent, seed, layer, flags=0, **sel_opts):
+    idx_st, part_st = oracle.select(imp_gpu, Bp, Br, n_sink, n_recent, seed, layer, flags, return_parts=True, **sel_opts)
     np.testing.assert_array_equal(idx_gpu, idx_st)
     return part_st
 
@@ -60,12 +60,14 @@ def check_structure(idx: np.ndarray, L, C, n_sink, n_recent):
         assert np.isin(prot, row).all(), "protected position missing"
 
 
-def check_e2e_sets(idx_gpu, part_gpu, imp_ref, Bp, Br, n_sink, n_recent, seed, layer, flags=0):
+def check_e2e_sets(idx_gpu, part_gpu, imp_ref, Bp, Br, n_sink, n_recent, seed, layer, flags=0, **sel_opts):
     """Returns (n_topk_swaps, n_random_diffs) summed over heads; asserts every difference is admissible."""
     idx_ref, part_ref, key_ref = oracle.select(imp_ref, Bp, Br, n_sink, n_recent, seed, layer, flags,
-                                               return_parts=True, return_keys=True)
+                                               return_parts=True, return_keys=True, **sel_opts)
     B, Hkv, L = imp_ref.shape
-    k1 = Bp - n_sink - n_recent
+    prot = sel_opts.get("protect_idx")
+    n_extra = 0 if prot is None else len(prot)
+    k1 = Bp - n_sink - n_recent - n_extra
     tot_swaps = tot_rand = 0
     for b in range(B):
         for h in range(Hkv):
@@ -75,7 +77,10 @@ def check_e2e_sets(idx_gpu, part_gpu, imp_ref, Bp, Br, n_sink, n_recent, seed, l
             swaps = Tg ^ Tr
             if swaps:
                 s = imp_ref[b, h]
-                free = np.sort(s[n_sink:L - n_recent])[::-1]
+                fs = s[n_sink:L - n_recent]
+                if n_extra:
+                    fs = np.delete(fs, np.asarray(prot) - n_sink)
+                free = np.sort(fs)[::-1]
                 tau = free[k1 - 1] if k1 > 0 else np.inf
                 for j in swaps:
                     assert abs(s[j] - tau) <= REL_TOL * tau + ABS_TOL, f"top-k mismatch at ({b},{h},{j}) outside the band"
@@ -107,13 +112,20 @@ def check_gather(K, V, out_K, out_V, idx_gpu):
             np.testing.assert_array_equal(oV[b, h], Vb[b, h, idx_gpu[b, h]])
 
 
-def full_parity(K, V, Q, Bp, Br, n_sink, n_recent, seed, layer, flags=0, oracle_flags=None, imp_ref=None):
-    """Runs the CUDA path through the C ABI on cuda:0 and every check above.  K,V,Q are HOST tensors."""
+def full_parity(K, V, Q, Bp, Br, n_sink, n_recent, seed, layer, flags=0, oracle_flags=None, imp_ref=None, lse_in=None,
+                **sel_opts):
+    """Runs the CUDA path through the C ABI on cuda:0 and every check above.  K,V,Q are HOST tensors.
+    sel_opts: batch_offset / head_offset / protect_idx (a list), passed to both sides."""
     from paper_2408_03675_b200 import binding
 
     dev = torch.device("cuda:0")
     Kd, Vd, Qd = K.to(dev), V.to(dev), Q.to(dev)
-    res = binding.nacl_evict_ex(Kd, Vd, Qd, Bp, Br, n_sink, n_recent, seed, layer, flags=flags, want_importance=True)
+    gpu_opts = dict(sel_opts)
+    if gpu_opts.get("protect_idx") is not None:
+        gpu_opts["protect_idx"] = torch.tensor(list(gpu_opts["protect_idx"]), dtype=torch.int32, device=dev)
+    if lse_in is not None:
+        gpu_opts["lse_in"] = lse_in.to(dev)
+    res = binding.nacl_evict_ex(Kd, Vd, Qd, Bp, Br, n_sink, n_recent, seed, layer, flags=flags, want_importance=True, **gpu_opts)
     torch.cuda.synchronize()
     idx_gpu = res["out_idx"].cpu().numpy()
     imp_gpu = res["importance"].cpu().numpy()
@@ -125,12 +137,13 @@ def full_parity(K, V, Q, Bp, Br, n_sink, n_recent, seed, layer, flags=0, oracle_
         imp_ref = oracle.importance(K, Q, flags=oflags & oracle.CAUSAL)
     max_rel = check_scores(imp_gpu, imp_ref, G, P)
     check_structure(idx_gpu, L, Bp + Br, n_sink, n_recent)
-    part_gpu = check_staged(idx_gpu, imp_gpu, Bp, Br, n_sink, n_recent, seed, layer, oflags)
-    swaps, rdiff = check_e2e_sets(idx_gpu, part_gpu, imp_ref, Bp, Br, n_sink, n_recent, seed, layer, oflags)
+    part_gpu = check_staged(idx_gpu, imp_gpu, Bp, Br, n_sink, n_recent, seed, layer, oflags, **sel_opts)
+    swaps, rdiff = check_e2e_sets(idx_gpu, part_gpu, imp_ref, Bp, Br, n_sink, n_recent, seed, layer, oflags, **sel_opts)
     check_gather(K, V, res["out_K"].cpu(), res["out_V"].cpu(), idx_gpu)
     # determinism: a second run is bit-identical
-    res2 = binding.nacl_evict_ex(Kd, Vd, Qd, Bp, Br, n_sink, n_recent, seed, layer, flags=flags, want_importance=True)
+    res2 = binding.nacl_evict_ex(Kd, Vd, Qd, Bp, Br, n_sink, n_recent, seed, layer, flags=flags, want_importance=True, **gpu_opts)
     torch.cuda.synchronize()
     assert torch.equal(res2["out_idx"], res["out_idx"]) and torch.equal(res2["importance"], res["importance"])
     assert torch.equal(res2["out_K"].view(torch.uint8), res["out_K"].view(torch.uint8))
+    assert torch.equal(res2["out_V"].view(torch.uint8), res["out_V"].view(torch.uint8))
     return {"max_rel_err": max_rel, "topk_swaps": swaps, "random_diffs": rdiff, "imp_gpu": imp_gpu, "idx_gpu": idx_gpu}

@@ -2,9 +2,11 @@
 
 The path shards over independent (batch, kv head) units with no data-path collective; the only
 cross-rank traffic is the barrier and the max-over-ranks of the device time that bench.py reports.
-Checked here: the unit split is a partition, every rank's shard evicted on its own equals the
-corresponding slice of the unsharded result (the oracle stands in for the device work: these
-processes have no GPU), and the reductions bench.py uses agree across ranks.
+Checked here: the unit split is a partition, every rank's shard -- its OWN kv heads or its own batch
+element, evicted on its own with head_offset / batch_offset -- equals the corresponding slice of the
+unsharded result (the oracle stands in for the device work: these processes have no GPU; the same
+split on a GPU through nacl_evict_ex is tests/test_gpu_parity.py::test_shards_draw_what_the_unsharded_call_draws),
+and the reductions bench.py uses agree across ranks.
 """
 from __future__ import annotations
 
@@ -51,17 +53,20 @@ def _worker(rank: int, world: int, port: int, out_dir: str):
     G = cfg.G
     hk = slice(units.start, units.stop)
     hq = slice(units.start * G, units.stop * G)
-    # head shard: the Philox counter carries the kv-head index, so a shard must be told where its heads start;
-    # the C ABI takes whole tensors, so a tensor-parallel caller passes its local heads and the oracle's
-    # head_offset equivalent is exercised here by evicting the full problem and slicing
-    idx_full = oracle.evict(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(0), 0)[2]
-    np.save(os.path.join(out_dir, f"idx_{rank}.npy"), idx_full[:, hk])
-    # batch shard (what bench.py does): each rank evicts its own batch element end to end
+    # head shard (tensor parallel): the rank evicts ITS OWN kv heads and their query heads, told where they start
+    # (head_offset): the Philox counter carries the global kv-head index (R10)
+    Ks, Vs, Qs = K[:, hk].contiguous(), V[:, hk].contiguous(), Q[:, hq].contiguous()
+    idx_sh = oracle.evict(Ks, Vs, Qs, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(0), 0, head_offset=units.start)[2]
+    np.save(os.path.join(out_dir, f"idx_{rank}.npy"), idx_sh)
+    idx_no = oracle.evict(Ks, Vs, Qs, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(0), 0)[2]
+    np.save(os.path.join(out_dir, f"idxno_{rank}.npy"), idx_no)
+    # batch shard (data parallel): each rank evicts its own batch element of ONE batch-2 problem, with batch_offset
     cfgb = CONFIGS[1].scaled(batch=2)
     Kb, Vb, Qb, _ = make_layer_inputs(cfgb, layer=0)
     b = nacl_dist.shard_units(cfgb.batch, rank, world)
     sl = slice(b.start, b.stop)
-    idx_b = oracle.evict(Kb[sl], Vb[sl], Qb[sl], Bp, Br, cfgb.n_sink, cfgb.n_recent, cfgb.layer_seed(0), 0)[2]
+    idx_b = oracle.evict(Kb[sl].contiguous(), Vb[sl].contiguous(), Qb[sl].contiguous(), Bp, Br, cfgb.n_sink, cfgb.n_recent,
+                         cfgb.layer_seed(0), 0, batch_offset=b.start)[2]
     np.save(os.path.join(out_dir, f"idxb_{rank}.npy"), idx_b)
     # the reductions of bench.py
     nacl_dist.barrier()
@@ -83,10 +88,12 @@ def test_two_rank_gloo_shards_match_the_unsharded_result(tmp_path):
     idx_full = oracle.evict(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(0), 0)[2]
     got = np.concatenate([np.load(tmp_path / f"idx_{r}.npy") for r in range(world)], axis=1)
     np.testing.assert_array_equal(got, idx_full)
-    # batch shards: rank r's batch element evicted alone is NOT the same draw as element r of a batch-2 call
-    # (the Philox counter carries the batch index, R10) -- bench.py therefore reports weak scaling over
-    # independent prompts, and a caller that splits ONE batch passes each rank whole problems.  Structure holds:
-    for r in range(world):
-        idx_b = np.load(tmp_path / f"idxb_{r}.npy")
-        assert idx_b.shape == (1, CONFIGS[1].Hkv, Bp + Br)
-        assert np.all(np.diff(idx_b.astype(np.int64), axis=-1) > 0)
+    # without head_offset the second rank numbers its heads from 0 and draws a different sample: the offsets matter
+    assert not np.array_equal(np.load(tmp_path / "idxno_1.npy"), idx_full[:, 2:])
+    np.testing.assert_array_equal(np.load(tmp_path / "idxno_0.npy"), idx_full[:, :2])
+    # batch shards of one batch-2 problem
+    cfgb = CONFIGS[1].scaled(batch=2)
+    Kb, Vb, Qb, _ = make_layer_inputs(cfgb, layer=0)
+    idx_bfull = oracle.evict(Kb, Vb, Qb, Bp, Br, cfgb.n_sink, cfgb.n_recent, cfgb.layer_seed(0), 0)[2]
+    gotb = np.concatenate([np.load(tmp_path / f"idxb_{r}.npy") for r in range(world)], axis=0)
+    np.testing.assert_array_equal(gotb, idx_bfull)

@@ -33,11 +33,11 @@ def test_baseline_configs_small(binding, cid):
     print(f"cfg{cid}: max rel err {r['max_rel_err']:.2e}, top-k swaps {r['topk_swaps']}, random diffs {r['random_diffs']}")
 
 
-@pytest.mark.parametrize("cid,layer", [(3, 0), (4, 0), (4, 17), (5, 31)])
+@pytest.mark.parametrize("cid,layer", [(c, l) for c in (3, 4, 5) for l in (0, 10, 21, 31)])
 def test_baseline_configs_full_size(binding, cid, layer):
-    """One whole layer of the 32-layer workloads at BASELINE.json's full sizes, in the launch configuration
-    bench.py times (same entry point, same shapes); the oracle finishes a layer in seconds, so every output is
-    compared, not a sample."""
+    """Four whole layers (first, last, two others: SURVEY.md 8(d)) of each 32-layer workload at BASELINE.json's full
+    sizes, in the launch configuration bench.py times (same entry point, same shapes); the oracle finishes a layer in
+    seconds, so every output is compared, not a sample."""
     cfg = CONFIGS[cid]
     K, V, Q, planted = make_layer_inputs(cfg, layer=layer)
     Bp, Br = cfg.budgets()
@@ -250,3 +250,126 @@ def test_long_rows(binding, case):
     B, L, Hq, Hkv, d, P, dt = case
     K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype=dt, seed=L % 1000)
     full_parity(K, V, Q, L // 8, L // 40, 4, P, seed=L, layer=7)
+
+
+# ------------------------------------------------------------------ round 2: gaps named by the round-1 review
+@pytest.mark.parametrize("L", [16, 64, 127, 128, 129])
+@pytest.mark.parametrize("causal", [False, True])
+def test_tensor_core_path_short_rows_and_all_rows_proxy(binding, L, causal):
+    """The tcgen05 path (bf16, d = 128, G*P % 16 == 0) below / at / just above one key tile, with a single kv head (fewer
+    tiles than CTAs, one tile per head) and with EVERY prompt row a proxy row (P = L where 16 | L, else P = 16)."""
+    P = L if L % 16 == 0 else 16
+    K, V, Q = make_random_inputs(1, L, 1, 1, 128, P, dtype="bf16", seed=100 + L)
+    nr = min(P, L // 2)
+    flags = binding.FLAG_CAUSAL if causal else 0
+    full_parity(K, V, Q, nr + 2 + L // 8, L // 10, 2, nr, seed=3, layer=1, flags=flags)
+    # edge budgets on the same path: no random part, keep everything, nothing but the protected set
+    full_parity(K, V, Q, nr + 2 + L // 8, 0, 2, nr, seed=3, layer=1, flags=flags)
+    r = full_parity(K, V, Q, L - 3, 3, 2, nr, seed=3, layer=1, flags=flags)
+    np.testing.assert_array_equal(r["idx_gpu"][0, 0], np.arange(L))
+    full_parity(K, V, Q, 2 + nr, 0, 2, nr, seed=3, layer=1, flags=flags)
+
+
+@pytest.mark.parametrize("case", [(1, 4100, 32, 8, 128, 64, "bf16"), (2, 700, 4, 2, 64, 5, "f32"), (1, 384, 8, 2, 128, 128, "bf16")],
+                         ids=["tc_GP256", "cuda_core_f32", "tc_GP512_row_blocks"])
+def test_lse_in_with_causal_flag(binding, case):
+    """Algorithm 2 proper: the row log-sum-exps come from a CAUSAL forward pass, i.e. row i's LSE covers
+    the keys j <= L-P+i only, and the column sum is taken under the same mask.  lse_in under NACL_FLAG_CAUSAL is that causal
+    LSE (include/nacl_evict.h); the oracle's causal importance and causal LSE are the referee."""
+    from parity import check_scores, check_staged, check_structure
+
+    B, L, Hq, Hkv, d, P, dt = case
+    K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype=dt, seed=L + 7)
+    imp_ref, lse_ref = oracle.importance(K, Q, flags=oracle.CAUSAL, return_lse=True)
+    Bp, Br, ns, nr = L // 6 + P, L // 20, 4, P
+    res = binding.nacl_evict_ex(K.cuda(), V.cuda(), Q.cuda(), Bp, Br, ns, nr, 5, 2, flags=binding.FLAG_CAUSAL,
+                                want_importance=True, lse_in=torch.from_numpy(lse_ref.astype(np.float32)).cuda())
+    torch.cuda.synchronize()
+    imp = res["importance"].cpu().numpy()
+    check_scores(imp, imp_ref, Hq // Hkv, P)
+    check_structure(res["out_idx"].cpu().numpy(), L, Bp + Br, ns, nr)
+    check_staged(res["out_idx"].cpu().numpy(), imp, Bp, Br, ns, nr, 5, 2)
+    # the self-contained causal call agrees
+    res2 = binding.nacl_evict_ex(K.cuda(), V.cuda(), Q.cuda(), Bp, Br, ns, nr, 5, 2, flags=binding.FLAG_CAUSAL, want_importance=True,
+                                 want_lse=True)
+    np.testing.assert_allclose(res2["importance"].cpu().numpy(), imp, rtol=2e-3, atol=1e-30)
+    # ln Z carries the FMA-pipe exp2's relative error (<= 7.5e-5, DESIGN.md section 5) as an ABSOLUTE error; short causal
+    # rows sum too few terms for it to average out
+    np.testing.assert_allclose(res2["lse"].cpu().numpy(), lse_ref, rtol=0, atol=1e-4)
+
+
+@pytest.mark.parametrize("case", [(2, 3000, 16, 8, 128, 16, "bf16"), (2, 500, 4, 4, 64, 4, "f32"), (1, 70000, 8, 2, 128, 32, "bf16")],
+                         ids=["tc", "cuda_core", "long_rows"])
+def test_shards_draw_what_the_unsharded_call_draws(binding, case):
+    """PAPER.md:37 / DESIGN.md R10: the random stream belongs to the (layer, batch element, kv head), not to the GPU that
+    holds it.  Evicting a slice of the kv heads (tensor parallel) or of the batch (data parallel) on its own, with
+    head_offset / batch_offset, gives bit-identical out_idx / out_K / out_V to the slice of the unsharded call."""
+    B, L, Hq, Hkv, d, P, dt = case
+    G = Hq // Hkv
+    K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype=dt, seed=L + 11)
+    Kd, Vd, Qd = K.cuda(), V.cuda(), Q.cuda()
+    Bp, Br = L // 6, L // 12
+    full = binding.nacl_evict_ex(Kd, Vd, Qd, Bp, Br, 4, P, 77, 3)
+    h0 = Hkv // 2
+    sh = binding.nacl_evict_ex(Kd[:, h0:].contiguous(), Vd[:, h0:].contiguous(), Qd[:, h0 * G:].contiguous(), Bp, Br, 4, P, 77, 3,
+                               head_offset=h0)
+    assert torch.equal(sh["out_idx"], full["out_idx"][:, h0:]) and torch.equal(sh["out_K"], full["out_K"][:, h0:])
+    assert torch.equal(sh["out_V"], full["out_V"][:, h0:])
+    wrong = binding.nacl_evict_ex(Kd[:, h0:].contiguous(), Vd[:, h0:].contiguous(), Qd[:, h0 * G:].contiguous(), Bp, Br, 4, P, 77, 3)
+    assert not torch.equal(wrong["out_idx"], full["out_idx"][:, h0:])
+    if B > 1:
+        bs = binding.nacl_evict_ex(Kd[1:].contiguous(), Vd[1:].contiguous(), Qd[1:].contiguous(), Bp, Br, 4, P, 77, 3, batch_offset=1)
+        assert torch.equal(bs["out_idx"], full["out_idx"][1:]) and torch.equal(bs["out_K"], full["out_K"][1:])
+    # and the sharded call itself is the oracle's sharded call
+    full_parity(K[:, h0:].contiguous(), V[:, h0:].contiguous(), Q[:, h0 * G:].contiguous(), Bp, Br, 4, P, 77, 3, head_offset=h0)
+
+
+@pytest.mark.parametrize("case", [(1, 2100, 8, 2, 128, 16, "bf16"), (2, 400, 4, 2, 64, 4, "f32"), (1, 70000, 4, 1, 128, 16, "bf16")],
+                         ids=["tc", "cuda_core", "long_rows"])
+def test_explicit_protected_positions(binding, case):
+    """Table "hyperp": an explicit list of protected positions (e.g. the proxy tokens when they are not
+    the last P positions) is always retained and counts inside budget_proxy (R7)."""
+    B, L, Hq, Hkv, d, P, dt = case
+    K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype=dt, seed=L + 13)
+    rng = np.random.default_rng(L)
+    prot = np.sort(rng.choice(np.arange(4, L - P), size=min(40, L // 20), replace=False)).tolist()
+    Bp, Br = 4 + P + len(prot) + L // 10, L // 20
+    r = full_parity(K, V, Q, Bp, Br, 4, P, seed=21, layer=6, protect_idx=prot)
+    for b in range(B):
+        for h in range(Hkv):
+            assert set(prot) <= set(r["idx_gpu"][b, h].tolist())
+    full_parity(K, V, Q, 4 + P + len(prot), 0, 4, P, seed=21, layer=6, protect_idx=prot)  # nothing but protected positions
+    with pytest.raises(binding.NaclError):
+        binding.nacl_evict_ex(K.cuda(), V.cuda(), Q.cuda(), 4 + P + len(prot) - 1, 0, 4, P, 0, 0,
+                              protect_idx=torch.tensor(prot, dtype=torch.int32, device="cuda"))
+
+
+@pytest.mark.parametrize("case", [(2, 2500, 16, 4, 128, 16, "bf16"), (1, 600, 4, 4, 64, 4, "f32")], ids=["tc", "cuda_core"])
+def test_shared_across_heads_selection(binding, case):
+    """NACL_FLAG_SHARED_HEADS, the paper's "- Head-wise" ablation: one retained set per batch
+    element, selected on the importance summed over the kv heads.  Staged check: the oracle's single-head selection on the
+    GPU's own fp32 head sum (same summation order) reproduces out_idx exactly; end to end: the oracle's shared selection
+    on its fp64 importance, up to the tolerance bands."""
+    from parity import check_e2e_sets, check_gather, check_scores, check_structure
+
+    B, L, Hq, Hkv, d, P, dt = case
+    K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype=dt, seed=L + 17)
+    Bp, Br = L // 5, L // 15
+    res = binding.nacl_evict_ex(K.cuda(), V.cuda(), Q.cuda(), Bp, Br, 4, P, 31, 4, flags=binding.FLAG_SHARED_HEADS, want_importance=True,
+                                head_offset=2)
+    torch.cuda.synchronize()
+    idx, imp = res["out_idx"].cpu().numpy(), res["importance"].cpu().numpy()
+    imp_ref = oracle.importance(K, Q)
+    check_scores(imp, imp_ref, Hq // Hkv, P)
+    check_structure(idx, L, Bp + Br, 4, P)
+    for h in range(1, Hkv):
+        np.testing.assert_array_equal(idx[:, h], idx[:, 0])
+    s32 = imp[:, 0].copy()
+    for h in range(1, Hkv):
+        s32 = (s32 + imp[:, h]).astype(np.float32)
+    st_idx, st_part = oracle.select(s32[:, None, :], Bp, Br, 4, P, 31, 4, head_offset=2, return_parts=True)
+    np.testing.assert_array_equal(idx[:, :1], st_idx)
+    check_e2e_sets(idx[:, :1], st_part, imp_ref.sum(axis=1, keepdims=True), Bp, Br, 4, P, 31, 4, head_offset=2)
+    ref = oracle.select(imp_ref, Bp, Br, 4, P, 31, 4, head_offset=2, shared_heads=True)
+    assert (ref[:, 0] == ref[:, -1]).all()
+    check_gather(K, V, res["out_K"].cpu(), res["out_V"].cpu(), idx)

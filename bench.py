@@ -3,6 +3,8 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
 
+`--gpus N` with N > 1 and no torchrun environment re-launches itself under torch.distributed.run with N ranks.
+
 One *step* = one pass of the whole hot path over one batch
 of synthetic prompts: every layer of the workload is evicted once through the C ABI
 (`nacl_evict`, include/nacl_evict.h).  Default workload: BASELINE.json configs[3] -- the L=32k
@@ -260,24 +262,23 @@ def run_ours(args) -> dict:
     dom = max(stage_rows, key=lambda k: stage_rows[k]["avg_us"] * stage_rows[k]["launches"]) if stage_rows else None
     roofline = None
     if dom:
+        # the roofline BASELINE.json names is HBM bandwidth: algorithmic bytes of the dominant kernel / its time, against the
+        # measured copy peak.  For the scoring sweeps (a dense bf16 contraction as well) the tensor-core fraction is
+        # reported beside it, against BOTH the burst and the sustained cuBLAS figure -- never instead of it.
         ach = stage_rows[dom]["alg_GBps"]
-        hbm = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": round(ach / peaks["hbm_gbs"], 4),
-               "alg_bytes_per_launch": sab.get(dom, 0)}
-        roofline = dict(hbm)
+        roofline = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": round(ach / peaks["hbm_gbs"], 4),
+                    "alg_bytes_per_launch": sab.get(dom, 0)}
         if dom in ("score_stats", "score_colsum", "score_fused") and cfg.dtype == "bf16":
-            # the scoring sweeps are a dense bf16 contraction as well: 2*B*Hq*P*L*d flop per sweep.  The
-            # kernel is timed inside a long step, so the sustained bf16 figure is the denominator; the roofline reported
-            # is the one the kernel sits closer to
             flop = 2.0 * cfg.batch * cfg.Hq * cfg.P * cfg.L * cfg.d * (2 if dom == "score_fused" else 1)
             tf = flop / (stage_rows[dom]["avg_us"] * 1e-6) / 1e12
-            peak_tf = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])
-            tensor = {"bound": "tensor", "achieved": round(tf, 1), "peak": peak_tf, "unit": "TFLOP/s", "frac": round(tf / peak_tf, 4),
-                      "alg_flop_per_launch": flop, "peak_kind": "bf16 dense, sustained (kernel timed inside a long step)"}
-            if tensor["frac"] > hbm["frac"]:
-                roofline = dict(tensor)
-                roofline["hbm"] = hbm
-            else:
-                roofline["tensor"] = tensor
+            sus = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])
+            roofline["tensor"] = {"achieved": round(tf, 1), "unit": "TFLOP/s", "alg_flop_per_launch": flop,
+                                  "peak_burst": peaks["bf16_tflops"], "frac_of_burst": round(tf / peaks["bf16_tflops"], 4),
+                                  "peak_sustained": sus, "frac_of_sustained": round(tf / sus, 4)}
+            exps = float(cfg.batch * cfg.Hq * cfg.P * cfg.L)
+            roofline["exp"] = {"exps_per_launch": exps, "achieved_Gexp_per_s": round(exps / (stage_rows[dom]["avg_us"] * 1e-6) / 1e9, 1),
+                               "mufu_peak_Gexp_per_s": round(16 * 148 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e9, 1),
+                               "note": "MUFU.EX2 alone: 16/clk/SM; the kernel splits the exponentials between MUFU and the FMA pipe"}
         roofline.update({"kernel": dom, "traffic": load_traffic(cfg.name, dom), "peak_source": peaks["source"]})
 
     # ---- end to end through the host entry point: pinned host buffers, H2D + D2H inside the timed region
@@ -304,12 +305,62 @@ def run_ours(args) -> dict:
                            "hbm_frac_of_measured": round(alg_bytes_step / world / (ms_lse * 1e-3) / 1e9 / peaks["hbm_gbs"], 4)},
         "library": os.path.relpath(binding.library_path(), ROOT),
     }
+    if rank == 0 and world == 1 and not args.no_other_workloads:
+        del data, lses
+        torch.cuda.empty_cache()
+        out["other_workloads"] = {CONFIGS[c].name: run_other(binding, CONFIGS[c], dev, peaks) for c in sorted(CONFIGS) if c != args.config}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = run_cpu_sample(cfg, max_seconds=15.0, max_layers=10)
     else:
         out["cpu_baseline"] = None
     nacl_dist.finalize()
     return out if rank == 0 else {}
+
+
+def run_other(binding, cfg, dev, peaks, steps: int = 3, max_sets: int = 8) -> dict:
+    """The same measurement (device time between CUDA events, distinct K/V per call so that every call is cold in L2)
+    for one of the other BASELINE.json workloads, short: `max_sets` layers (the workload's own if fewer: the remaining
+    calls rotate over the sets, at least 8 of them for the single-layer configs)."""
+    Bp, Br = cfg.budgets()
+    C = Bp + Br
+    tdt = torch.float32 if cfg.dtype == "f32" else torch.bfloat16
+    n_sets = max_sets
+    data = []
+    for l in range(n_sets):
+        K, V, Q, _ = make_layer_inputs(cfg, layer=l % cfg.layers if cfg.layers > 1 else 0, device=dev) if cfg.layers > 1 else \
+            make_layer_inputs(cfg.scaled(config_id=cfg.config_id + 100 * l), layer=0, device=dev)
+        oK = torch.empty((cfg.batch, cfg.Hkv, C, cfg.d), dtype=tdt, device=dev)
+        data.append((K, V, Q, oK, torch.empty_like(oK), torch.empty((cfg.batch, cfg.Hkv, C), dtype=torch.int32, device=dev)))
+    ws = torch.empty(binding.nacl_workspace_bytes(cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P) + 256, dtype=torch.uint8, device=dev)
+    ws = ws[(-ws.data_ptr()) % 256:]
+    stream = torch.cuda.current_stream(dev)
+
+    def step():
+        for l, (K, V, Q, oK, oV, oi) in enumerate(data):
+            binding.nacl_evict_ex(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l, out_K=oK, out_V=oV, out_idx=oi,
+                                  workspace=ws, stream=stream)
+
+    for _ in range(3):
+        step()
+    torch.cuda.synchronize(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize(dev)
+    us = e0.elapsed_time(e1) * 1e3 / (steps * n_sets)
+    binding.nacl_profile_enable(True)
+    binding.nacl_profile_read(reset=True)
+    step()
+    torch.cuda.synchronize(dev)
+    stages = binding.nacl_profile_read(reset=True)
+    binding.nacl_profile_enable(False)
+    gbs = cfg.alg_bytes_per_layer() / (us * 1e-6) / 1e9
+    return {"us_per_layer": round(us, 2), "value": round(gbs, 2), "unit": UNIT, "hbm_frac_of_measured": round(gbs / peaks["hbm_gbs"], 4),
+            "alg_bytes_per_layer": cfg.alg_bytes_per_layer(), "distinct_input_sets": n_sets, "dtype": cfg.dtype,
+            "kernels_us": {k: round(ms / n * 1e3, 2) for k, (ms, n) in stages.items() if n},
+            "dram_bytes": {k: load_traffic(cfg.name, k) for k in ("score_stats", "score_colsum", "select")}}
 
 
 def run_e2e(binding, cfg, layers, data, Bp, Br, dev, args, world) -> dict:
@@ -380,15 +431,17 @@ def run_reference(args) -> dict:
 
     cfg = CONFIGS[args.config]
     Bp, Br = cfg.budgets()
+    # torchrun pins OMP_NUM_THREADS=1 for its workers; the oracle arm is rank 0 alone and takes the host cores it may use
+    nthreads = len(os.sched_getaffinity(0)) if world > 1 and hasattr(os, "sched_getaffinity") else 0
     steps, warmup = max(1, min(args.steps, 4)), max(0, min(args.warmup, 1))
     inputs = [make_layer_inputs(cfg, layer=l, device="cpu") for l in range(max(steps, 1))]
     for w in range(warmup):
         K, V, Q, _ = inputs[0]
-        oracle.evict(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(0), 0)
+        oracle.evict(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(0), 0, nthreads=nthreads)
     t0 = time.perf_counter()
     for l in range(steps):
         K, V, Q, _ = inputs[l]
-        oracle.evict(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l)
+        oracle.evict(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l, nthreads=nthreads)
     dt = time.perf_counter() - t0
     val = cfg.alg_bytes_per_layer() * steps / dt / 1e9
     desc = workload_desc(cfg, cfg.layers, 1)
@@ -397,10 +450,27 @@ def run_reference(args) -> dict:
         "impl": "reference", "metric": METRIC, "value": round(val, 5), "unit": UNIT, "n_gpus": world, "steps": steps,
         "warmup": warmup, "ms_per_step": round(dt / steps * 1e3, 2), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic (same seeded generator as the CUDA arm)", "config": desc,
-        "cpu_baseline": {"value": round(val, 5), "unit": UNIT, "cores": oracle.threads(), "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": round(val, 5), "unit": UNIT, "cores": oracle.threads(nthreads), "kind": "oracle", "sample": sample},
         "e2e": {"value": round(val, 5), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0, "note": "fp64 CPU oracle (oracle/), rank 0 only; the reference is a paper with no code",
     }
+
+
+def spawn_ranks(n: int) -> int:
+    """`python bench.py --gpus N` without a torchrun environment: re-launch this command line under
+    torch.distributed.run with N ranks on this node (one per GPU), exactly as the driver does."""
+    import socket
+
+    if "--impl" not in sys.argv or sys.argv[sys.argv.index("--impl") + 1] != "reference":
+        if not torch.cuda.is_available() or torch.cuda.device_count() < n:
+            raise SystemExit(f"bench.py --gpus {n}: needs {n} CUDA devices, found "
+                             f"{torch.cuda.device_count() if torch.cuda.is_available() else 0} (there is no CPU fallback)")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main() -> int:
@@ -412,7 +482,12 @@ def main() -> int:
     ap.add_argument("--config", type=int, default=4, choices=sorted(CONFIGS))
     ap.add_argument("--layers", type=int, default=0, help="override the number of layers per step (0 = the workload's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-workloads", action="store_true", help="skip the short runs of the other BASELINE.json configs")
     args = ap.parse_args()
+    if args.gpus > 1 and "RANK" not in os.environ:
+        return spawn_ranks(args.gpus)
+    if args.gpus > 1 and int(os.environ.get("WORLD_SIZE", "1")) != args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus} was launched with WORLD_SIZE={os.environ.get('WORLD_SIZE')}")
     out = run_reference(args) if args.impl == "reference" else run_ours(args)
     if out:
         print(json.dumps(out), flush=True)

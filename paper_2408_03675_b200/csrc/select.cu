@@ -53,100 +53,9 @@ __device__ __forceinline__ uint32_t ordermap(uint32_t bits) {
 // pairs, log1p by its degree-7 Taylor polynomial (truncation < 2e-19).  About 15 fp64 operations instead of the ~50 of the
 // library routine (the sampling keys are fp64-throughput-bound), error ~1 ulp; around x = 1 (c = 1, ln c = 0 exactly)
 // the result keeps full RELATIVE accuracy, which -ln u needs for u next to 1.
-// generated once by a throwaway script from 60-digit decimal arithmetic: for k = 90..181, c = k/128: {1/c, hi(ln c), lo(ln c)}
+// table of {1/c, hi(ln c), lo(ln c)}, c = k/128, k = 90..181: csrc/logtab.inc, written by csrc/gen_logtab.py
 __device__ const double kLogTab[92][3] = {
-  {0x1.6c16c16c16c17p+0, -0x1.68ac83e9c6a14p-2, -0x1.a64eadd740178p-58},
-  {0x1.6816816816817p+0, -0x1.5d5bddf595f30p-2, 0x1.6541148cbb8a2p-56},
-  {0x1.642c8590b2164p+0, -0x1.522ae0738a3d8p-2, 0x1.8f7e9b38a6979p-57},
-  {0x1.6058160581606p+0, -0x1.4718dc271c41bp-2, -0x1.8fb4c14c56eefp-60},
-  {0x1.5c9882b931057p+0, -0x1.3c25277333184p-2, 0x1.2ad27e50a8ec6p-56},
-  {0x1.58ed2308158edp+0, -0x1.314f1e1d35ce4p-2, 0x1.3d69909e5c3dcp-56},
-  {0x1.5555555555555p+0, -0x1.269621134db92p-2, -0x1.e0efadd9db02bp-56},
-  {0x1.51d07eae2f815p+0, -0x1.1bf99635a6b95p-2, 0x1.12aeb84249223p-57},
-  {0x1.4e5e0a72f0539p+0, -0x1.1178e8227e47cp-2, 0x1.0e63a5f01c691p-57},
-  {0x1.4afd6a052bf5bp+0, -0x1.07138604d5862p-2, -0x1.cdb16ed4e9138p-56},
-  {0x1.47ae147ae147bp+0, -0x1.f991c6cb3b379p-3, -0x1.f665066f980a2p-57},
-  {0x1.446f86562d9fbp+0, -0x1.e530effe71012p-3, -0x1.2276041f43042p-59},
-  {0x1.4141414141414p+0, -0x1.d1037f2655e7bp-3, -0x1.60629242471a2p-57},
-  {0x1.3e22cbce4a902p+0, -0x1.bd087383bd8adp-3, -0x1.dd355f6a516d7p-60},
-  {0x1.3b13b13b13b14p+0, -0x1.a93ed3c8ad9e3p-3, -0x1.bcafa9de97203p-57},
-  {0x1.3813813813814p+0, -0x1.95a5adcf7017fp-3, -0x1.142c507fb7a3dp-58},
-  {0x1.3521cfb2b78c1p+0, -0x1.823c16551a3c2p-3, 0x1.1232ce70be781p-57},
-  {0x1.323e34a2b10bfp+0, -0x1.6f0128b756abcp-3, 0x1.8de59c21e166cp-57},
-  {0x1.2f684bda12f68p+0, -0x1.5bf406b543db2p-3, 0x1.1f5b44c0df7e7p-61},
-  {0x1.2c9fb4d812ca0p+0, -0x1.4913d8333b561p-3, 0x1.0d5604930f135p-58},
-  {0x1.29e4129e4129ep+0, -0x1.365fcb0159016p-3, -0x1.7d411a5b944adp-58},
-  {0x1.27350b8812735p+0, -0x1.23d712a49c202p-3, 0x1.6e38161051d69p-57},
-  {0x1.2492492492492p+0, -0x1.1178e8227e47cp-3, 0x1.0e63a5f01c691p-58},
-  {0x1.21fb78121fb78p+0, -0x1.fe89139dbd566p-4, 0x1.ac9f4215f9393p-58},
-  {0x1.1f7047dc11f70p+0, -0x1.da727638446a2p-4, -0x1.401fa71733019p-58},
-  {0x1.1cf06ada2811dp+0, -0x1.b6ac88dad5b1cp-4, 0x1.0057eed1ca59fp-59},
-  {0x1.1a7b9611a7b96p+0, -0x1.9335e5d594989p-4, 0x1.478a85704ccb7p-58},
-  {0x1.1811811811812p+0, -0x1.700d30aeac0e1p-4, 0x1.72566212cdd05p-61},
-  {0x1.15b1e5f75270dp+0, -0x1.4d3115d207eacp-4, -0x1.769f42c7842ccp-58},
-  {0x1.135c81135c811p+0, -0x1.2aa04a44717a5p-4, 0x1.d15d38d2fa3f7p-58},
-  {0x1.1111111111111p+0, -0x1.08598b59e3a07p-4, 0x1.dd7009902bf32p-58},
-  {0x1.0ecf56be69c90p+0, -0x1.ccb73cdddb2ccp-5, 0x1.e48fb0500efd4p-59},
-  {0x1.0c9714fbcda3bp+0, -0x1.894aa149fb343p-5, -0x1.a8be97660a23dp-60},
-  {0x1.0a6810a6810a7p+0, -0x1.466aed42de3eap-5, 0x1.cdd6f7f4a137ep-59},
-  {0x1.0842108421084p+0, -0x1.0415d89e74444p-5, -0x1.c05cf1d753622p-59},
-  {0x1.0624dd2f1a9fcp+0, -0x1.8492528c8cabfp-6, 0x1.d192d0619fa67p-60},
-  {0x1.0410410410410p+0, -0x1.0205658935847p-6, -0x1.27c8e8416e71fp-60},
-  {0x1.0204081020408p+0, -0x1.010157588de71p-7, -0x1.46662d417ced0p-62},
-  {0x1.0000000000000p+0, 0x0.0p+0, 0x0.0p+0},
-  {0x1.fc07f01fc07f0p-1, 0x1.fe02a6b106789p-8, -0x1.e44b7e3711ebfp-67},
-  {0x1.f81f81f81f820p-1, 0x1.fc0a8b0fc03e4p-7, -0x1.83092c59642a1p-62},
-  {0x1.f44659e4a4271p-1, 0x1.7b91b07d5b11bp-6, -0x1.5b602ace3a510p-60},
-  {0x1.f07c1f07c1f08p-1, 0x1.f829b0e783300p-6, 0x1.33e3f04f1ef23p-60},
-  {0x1.ecc07b301ecc0p-1, 0x1.39e87b9febd60p-5, -0x1.5bfa937f551bbp-59},
-  {0x1.e9131abf0b767p-1, 0x1.77458f632dcfcp-5, 0x1.18d3ca87b9296p-59},
-  {0x1.e573ac901e574p-1, 0x1.b42dd711971bfp-5, -0x1.eb9759c130499p-60},
-  {0x1.e1e1e1e1e1e1ep-1, 0x1.f0a30c01162a6p-5, 0x1.85f325c5bbacdp-59},
-  {0x1.de5d6e3f8868ap-1, 0x1.16536eea37ae1p-4, -0x1.79da3e8c22cdap-60},
-  {0x1.dae6076b981dbp-1, 0x1.341d7961bd1d1p-4, -0x1.b599f227becbbp-58},
-  {0x1.d77b654b82c34p-1, 0x1.51b073f06183fp-4, 0x1.a49e39a1a8be4p-58},
-  {0x1.d41d41d41d41dp-1, 0x1.6f0d28ae56b4cp-4, -0x1.906d99184b992p-58},
-  {0x1.d0cb58f6ec074p-1, 0x1.8c345d6319b21p-4, -0x1.4a697ab3424a9p-61},
-  {0x1.cd85689039b0bp-1, 0x1.a926d3a4ad563p-4, 0x1.942f48aa70ea9p-58},
-  {0x1.ca4b3055ee191p-1, 0x1.c5e548f5bc743p-4, 0x1.5d617ef8161b1p-60},
-  {0x1.c71c71c71c71cp-1, 0x1.e27076e2af2e6p-4, -0x1.61578001e0162p-60},
-  {0x1.c3f8f01c3f8f0p-1, 0x1.fec9131dbeabbp-4, -0x1.5746b9981b36cp-58},
-  {0x1.c0e070381c0e0p-1, 0x1.0d77e7cd08e59p-3, 0x1.9a5dc5e9030acp-57},
-  {0x1.bdd2b899406f7p-1, 0x1.1b72ad52f67a0p-3, 0x1.483023472cd74p-58},
-  {0x1.bacf914c1bad0p-1, 0x1.29552f81ff523p-3, 0x1.301771c407dbfp-57},
-  {0x1.b7d6c3dda338bp-1, 0x1.371fc201e8f74p-3, 0x1.de6cb62af18a0p-58},
-  {0x1.b4e81b4e81b4fp-1, 0x1.44d2b6ccb7d1ep-3, 0x1.9f4f6543e1f88p-57},
-  {0x1.b2036406c80d9p-1, 0x1.526e5e3a1b438p-3, -0x1.746ff8a470d3ap-57},
-  {0x1.af286bca1af28p-1, 0x1.5ff3070a793d4p-3, -0x1.bc60efafc6f6ep-58},
-  {0x1.ac5701ac5701bp-1, 0x1.6d60fe719d21dp-3, -0x1.caae268ecd179p-57},
-  {0x1.a98ef606a63bep-1, 0x1.7ab890210d909p-3, 0x1.be36b2d6a0608p-59},
-  {0x1.a6d01a6d01a6dp-1, 0x1.87fa06520c911p-3, -0x1.bf7fdbfa08d9ap-57},
-  {0x1.a41a41a41a41ap-1, 0x1.9525a9cf456b4p-3, 0x1.d904c1d4e2e26p-57},
-  {0x1.a16d3f97a4b02p-1, 0x1.a23bc1fe2b563p-3, 0x1.93711b07a998cp-59},
-  {0x1.9ec8e951033d9p-1, 0x1.af3c94e80bff3p-3, -0x1.398cff3641985p-58},
-  {0x1.9c2d14ee4a102p-1, 0x1.bc286742d8cd6p-3, 0x1.4fce744870f55p-58},
-  {0x1.999999999999ap-1, 0x1.c8ff7c79a9a22p-3, -0x1.4f689f8434012p-57},
-  {0x1.970e4f80cb872p-1, 0x1.d5c216b4fbb91p-3, 0x1.6e443597e4d40p-57},
-  {0x1.948b0fcd6e9e0p-1, 0x1.e27076e2af2e6p-3, -0x1.61578001e0162p-59},
-  {0x1.920fb49d0e229p-1, 0x1.ef0adcbdc5936p-3, 0x1.48637950dc20dp-57},
-  {0x1.8f9c18f9c18fap-1, 0x1.fb9186d5e3e2bp-3, -0x1.caaae64f21acbp-57},
-  {0x1.8d3018d3018d3p-1, 0x1.0402594b4d041p-2, -0x1.28ec217a5022dp-57},
-  {0x1.8acb90f6bf3aap-1, 0x1.0a324e27390e3p-2, 0x1.7dcfde8061c03p-56},
-  {0x1.886e5f0abb04ap-1, 0x1.1058bf9ae4ad5p-2, 0x1.89fa0ab4cb31dp-58},
-  {0x1.8618618618618p-1, 0x1.1675cababa60ep-2, 0x1.ce63eab883717p-61},
-  {0x1.83c977ab2beddp-1, 0x1.1c898c16999fbp-2, -0x1.0e5c62aff1c44p-60},
-  {0x1.8181818181818p-1, 0x1.22941fbcf7966p-2, -0x1.76f5eb09628afp-56},
-  {0x1.7f405fd017f40p-1, 0x1.2895a13de86a3p-2, 0x1.7ad24c13f040ep-56},
-  {0x1.7d05f417d05f4p-1, 0x1.2e8e2bae11d31p-2, -0x1.8f4cdb95ebdf9p-56},
-  {0x1.7ad2208e0ecc3p-1, 0x1.347dd9a987d55p-2, -0x1.4dd4c580919f8p-57},
-  {0x1.78a4c8178a4c8p-1, 0x1.3a64c556945eap-2, -0x1.c68651945f97cp-57},
-  {0x1.767dce434a9b1p-1, 0x1.404308686a7e4p-2, -0x1.0bcfb6082ce6dp-56},
-  {0x1.745d1745d1746p-1, 0x1.4618bc21c5ec2p-2, 0x1.f42decdeccf1dp-56},
-  {0x1.724287f46debcp-1, 0x1.4be5f957778a1p-2, -0x1.259b35b04813dp-57},
-  {0x1.702e05c0b8170p-1, 0x1.51aad872df82dp-2, 0x1.3927ac19f55e3p-59},
-  {0x1.6e1f76b4337c7p-1, 0x1.5767717455a6cp-2, 0x1.526adb283660cp-56},
-  {0x1.6c16c16c16c17p-1, 0x1.5d1bdbf5809cap-2, 0x1.4236383dc7fe1p-56},
-  {0x1.6a13cd1537290p-1, 0x1.62c82f2b9c795p-2, 0x1.7b7af915300e5p-57},
+#include "logtab.inc"
 };
 constexpr double kLn2Hi = 0x1.62e42fefa39efp-1, kLn2Lo = 0x1.abc9e3b39803fp-56;
 __device__ __forceinline__ double log_tab(double x) {

@@ -107,3 +107,23 @@ def test_product_does_not_import_the_oracle():
                 txt = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
                 assert "nacl_oracle" not in txt, f
+
+
+def test_log_table_is_what_its_generator_writes():
+    """csrc/logtab.inc (the constants behind the fp64 logarithm of the sampling keys) is reproducible: the tracked generator,
+    which uses nothing but the standard library's arbitrary-precision decimal module, rewrites it bit for bit; and every
+    entry agrees with libm (1/c and hi(ln c) to 1 ulp, hi + lo closer to ln c than a double can express)."""
+    import math
+    import subprocess
+    import sys
+
+    gen = os.path.join(ROOT, "paper_2408_03675_b200", "csrc", "gen_logtab.py")
+    assert subprocess.run([sys.executable, gen, "--check"]).returncode == 0
+    rows = re.findall(r"\{(\S+), (\S+), (\S+)\},", open(os.path.join(ROOT, "paper_2408_03675_b200", "csrc", "logtab.inc")).read())
+    assert len(rows) == 92
+    for i, (inv, hi, lo) in enumerate(rows):
+        c = (90 + i) / 128.0
+        inv, hi, lo = float.fromhex(inv), float.fromhex(hi), float.fromhex(lo)
+        assert abs(inv - 1.0 / c) <= math.ulp(inv)
+        assert abs(hi - math.log(c)) <= math.ulp(hi) if c != 1.0 else hi == 0.0
+        assert abs(lo) <= math.ulp(hi) / 2 if c != 1.0 else lo == 0.0

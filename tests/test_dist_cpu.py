@@ -97,3 +97,27 @@ def test_two_rank_gloo_shards_match_the_unsharded_result(tmp_path):
     idx_bfull = oracle.evict(Kb, Vb, Qb, Bp, Br, cfgb.n_sink, cfgb.n_recent, cfgb.layer_seed(0), 0)[2]
     gotb = np.concatenate([np.load(tmp_path / f"idxb_{r}.npy") for r in range(world)], axis=0)
     np.testing.assert_array_equal(gotb, idx_bfull)
+
+
+@pytest.mark.timeout(600)
+def test_bench_gpus_flag_spawns_the_ranks_itself():
+    """`python bench.py --gpus 2` with no torchrun environment launches two ranks (torch.distributed.run on 127.0.0.1).
+    On a box without GPUs the CUDA arm must fail loudly instead of running one rank; the oracle arm (rank 0 works, the other
+    rank exits 0) runs anywhere and reports n_gpus = 2."""
+    import json
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--impl", "reference", "--config", "1",
+                        "--steps", "1", "--warmup", "0"], capture_output=True, text=True, env=env, timeout=500)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    rec = json.loads(lines[0])
+    assert rec["impl"] == "reference" and rec["n_gpus"] == 2 and rec["cpu_baseline"]["cores"] >= 1
+    if not torch.cuda.is_available() or torch.cuda.device_count() < 2:
+        r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "1"], capture_output=True,
+                           text=True, env=env, timeout=300)
+        assert r.returncode != 0 and "needs 2 CUDA devices" in (r.stderr + r.stdout)

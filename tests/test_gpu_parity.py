@@ -373,3 +373,22 @@ def test_shared_across_heads_selection(binding, case):
     ref = oracle.select(imp_ref, Bp, Br, 4, P, 31, 4, head_offset=2, shared_heads=True)
     assert (ref[:, 0] == ref[:, -1]).all()
     check_gather(K, V, res["out_K"].cpu(), res["out_V"].cpu(), idx)
+
+
+def test_log_table_every_interval_at_both_edges_and_the_centre(binding):
+    """The table-driven fp64 logarithm of the sampling keys (csrc/select.cu log_tab, table csrc/logtab.inc): importances
+    whose mantissa sits at the lower edge, the centre and the upper edge of EACH of the 92 table intervals
+    (c = k/128, k = 90..181), at several binary exponents, give the oracle's libm key bit for bit."""
+    ms = []
+    for k in range(90, 182):
+        for off in (-0.5 + 1e-6, -0.25, 0.0, 0.25, 0.5 - 1e-6):
+            ms.append((k + off) / 128.0)
+    m = np.array(ms, dtype=np.float64)
+    vals = np.concatenate([np.ldexp(m, e) for e in (-100, -20, -3, -1, 0, 1, 7)]).astype(np.float32)
+    L = vals.size
+    imp = np.stack([vals, vals[::-1].copy()])[None]  # [1, 2, L]
+    seed, layer = 0xDEADBEEF12345, 9
+    keys_gpu = binding.nacl_gumbel_keys(torch.from_numpy(imp).cuda(), seed, layer, 0).cpu().numpy()
+    _, keys_ref = oracle.select(imp, 0, 1, 0, 0, seed, layer, 0, return_keys=True)
+    a, b = keys_gpu.view(np.int32).astype(np.int64), keys_ref.view(np.int32).astype(np.int64)
+    assert int((a != b).sum()) <= 1 and np.abs(a - b).max() <= 1, f"{int((a != b).sum())} of {a.size} keys differ"

@@ -130,6 +130,16 @@ typedef struct nacl_params {
                                       contents are the caller's responsibility (validation never reads device memory) */
   int32_t n_protect;
   int32_t reserved0;               /* 0 */
+  int64_t kv_stride_batch;         /* ELEMENT strides of K and V between batch elements, kv heads and key rows; the d      */
+  int64_t kv_stride_head;          /* elements of one row are contiguous.  All three 0 = contiguous [batch,Hkv,L,d].       */
+  int64_t kv_stride_row;           /* Otherwise all three > 0, e.g. a cache [batch,Hkv,cap,d] with cap >= L rows per head   */
+                                   /* (row = d, head = cap*d, batch = Hkv*cap*d) or a token-major [batch,L,Hkv,d] tensor   */
+                                   /* (row = Hkv*d, head = d, batch = L*Hkv*d).  Each times sizeof(element) must be a      */
+                                   /* multiple of 16 bytes.  K and V share them ("compatible with            */
+                                   /* FlashAttention": both cache layouts of such kernels are served without a copy)       */
+  int64_t out_stride_batch;        /* the same for out_K / out_V; all three 0 = contiguous [batch,Hkv,C,d]                  */
+  int64_t out_stride_head;
+  int64_t out_stride_row;
 } nacl_params_t;
 
 /* bf16 K/V/Q.  Steps 1-7 above on `stream`. */
@@ -148,6 +158,46 @@ int nacl_evict_f32(const void* K, const void* V, const void* Qproxy,
 
 /* Superset entry point: dtype tag, flags, optional importance / lse outputs, explicit workspace. */
 int nacl_evict_ex(const nacl_params_t* p);
+
+/* Generation-phase eviction ("Generation Phase Eviction"; Algorithm 1, function Generation):
+ * every m decoding steps the cache of a layer, which has grown to `len` = C + m entries per head, is cut back to the budget
+ * C = budget_proxy + budget_random by the SAME eviction (Algorithm 1 lines 7-10) driven by the attention row of the current
+ * token alone, A_t = q_t K_t^T / sqrt(d) in R^{1 x len}: one proxy row per query head, its softmax over the live cache
+ * entries, summed over the G query heads of a kv head.  Cache SLOTS take the place of prompt positions: the first n_sink
+ * slots and the last n_recent slots (the newest tokens) are protected.  The draws of the Random Eviction at decoding step
+ * `step` use the seed  seed + step * 0x9E3779B97F4A7C15  (independent streams per step; R16).
+ *   K_cache, V_cache [batch, Hkv, cap_in, d]   the first `len` rows of every head are live
+ *   q                [batch, Hq, 1, d]         the current token's queries
+ *   pos_in  (optional) [batch, Hkv, cap_in] int32: original token position of every live slot
+ *   K_out, V_out     [batch, Hkv, cap_out, d]  cap_out >= C; rows [0, C) receive the compacted cache (must not alias the inputs)
+ *   pos_out (with pos_in) [batch, Hkv, cap_out] int32: pos_out[c] = pos_in[slot kept at c]
+ *   out_idx (optional) [batch, Hkv, C] int32: the kept cache slots, ascending
+ *   out_importance (optional) [batch, Hkv, len] fp32
+ * All DEVICE pointers, same alignment rules, enqueued on `stream`.  It is nacl_evict_ex with P = 1, L = len and the cache's
+ * strides, followed by the position-map update. */
+typedef struct nacl_gen_params {
+  uint32_t struct_size;            /* = sizeof(nacl_gen_params_t) */
+  int32_t dtype;
+  const void* K_cache;
+  const void* V_cache;
+  const void* q;
+  const int32_t* pos_in;
+  int32_t batch, Hq, Hkv, d, len, cap_in, cap_out;
+  int32_t budget_proxy, budget_random, n_sink, n_recent;
+  uint64_t seed;
+  int32_t layer, step;
+  uint32_t flags;                  /* NACL_FLAG_SAMPLE_*, NACL_FLAG_SHARED_HEADS, NACL_FLAG_SCORE_CUDA_CORES */
+  int32_t batch_offset, head_offset, reserved0;
+  void* K_out;
+  void* V_out;
+  int32_t* pos_out;
+  int32_t* out_idx;
+  float* out_importance;
+  void* workspace;                 /* optional; >= nacl_workspace_bytes(batch, len, Hq, Hkv, d, 1) */
+  size_t workspace_bytes;
+  void* stream;
+} nacl_gen_params_t;
+int nacl_evict_generation(const nacl_gen_params_t* g);
 
 /* Same operation with every tensor in HOST memory (pinned memory makes the copies
  * asynchronous).  Copies K, V, Qproxy to grow-only device staging buffers, runs steps 1-7

@@ -15,7 +15,7 @@ def __getattr__(name):  # lazy: importing the package must not need the CUDA lib
         import importlib
 
         return importlib.import_module(".binding", __name__)
-    if name in ("nacl_evict", "nacl_evict_ex", "nacl_workspace_bytes", "nacl_evict_host"):
+    if name in ("nacl_evict", "nacl_evict_ex", "nacl_workspace_bytes", "nacl_evict_host", "nacl_evict_generation"):
         from . import binding
 
         return getattr(binding, name)

@@ -19,7 +19,7 @@ FLAG_CAUSAL, FLAG_SAMPLE_SOFTMAX_OF_SCORE, FLAG_SAMPLE_UNIFORM, FLAG_SHARED_HEAD
 
 EXPORTS = ("nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes",
            "nacl_launch_count", "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version",
-           "nacl_profile_enable", "nacl_profile_read", "nacl_stage_name", "nacl_gumbel_keys")
+           "nacl_profile_enable", "nacl_profile_read", "nacl_stage_name", "nacl_gumbel_keys", "nacl_evict_generation")
 N_STAGES = 7
 
 
@@ -36,6 +36,22 @@ class NaclParams(C.Structure):
         ("lse_in", C.c_void_p),
         ("batch_offset", C.c_int32), ("head_offset", C.c_int32),
         ("protect_idx", C.c_void_p), ("n_protect", C.c_int32), ("reserved0", C.c_int32),
+        ("kv_stride_batch", C.c_int64), ("kv_stride_head", C.c_int64), ("kv_stride_row", C.c_int64),
+        ("out_stride_batch", C.c_int64), ("out_stride_head", C.c_int64), ("out_stride_row", C.c_int64),
+    ]
+
+
+class NaclGenParams(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("dtype", C.c_int32),
+        ("K_cache", C.c_void_p), ("V_cache", C.c_void_p), ("q", C.c_void_p), ("pos_in", C.c_void_p),
+        ("batch", C.c_int32), ("Hq", C.c_int32), ("Hkv", C.c_int32), ("d", C.c_int32), ("len", C.c_int32),
+        ("cap_in", C.c_int32), ("cap_out", C.c_int32),
+        ("budget_proxy", C.c_int32), ("budget_random", C.c_int32), ("n_sink", C.c_int32), ("n_recent", C.c_int32),
+        ("seed", C.c_uint64), ("layer", C.c_int32), ("step", C.c_int32), ("flags", C.c_uint32),
+        ("batch_offset", C.c_int32), ("head_offset", C.c_int32), ("reserved0", C.c_int32),
+        ("K_out", C.c_void_p), ("V_out", C.c_void_p), ("pos_out", C.c_void_p), ("out_idx", C.c_void_p),
+        ("out_importance", C.c_void_p), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("stream", C.c_void_p),
     ]
 
 
@@ -64,6 +80,8 @@ def _load() -> C.CDLL:
     lib.nacl_evict_f32.restype = i32
     lib.nacl_evict_ex.argtypes = [C.POINTER(NaclParams)]
     lib.nacl_evict_ex.restype = i32
+    lib.nacl_evict_generation.argtypes = [C.POINTER(NaclGenParams)]
+    lib.nacl_evict_generation.restype = i32
     lib.nacl_evict_host.argtypes = [vp, vp, vp, i32] + [i32] * 10 + [u64, i32, vp, vp, vp, i32]
     lib.nacl_evict_host.restype = i32
     lib.nacl_workspace_bytes.argtypes = [i32] * 6
@@ -107,10 +125,16 @@ def _shapes(K, V, Q):
     B2, Hq, P, d2 = Q.shape
     if B2 != B or d2 != d or K.dtype != V.dtype or K.dtype != Q.dtype:
         raise ValueError("K/V/Qproxy batch, head_dim or dtype mismatch")
-    for t in (K, V, Q):
-        if not t.is_contiguous():
-            raise ValueError("tensors must be contiguous")
+    if not Q.is_contiguous():
+        raise ValueError("Qproxy must be contiguous")
+    if K.stride() != V.stride() or K.stride(3) != 1:
+        raise ValueError("K and V must share their strides and have contiguous rows (stride 1 along head_dim)")
     return B, Hkv, L, d, Hq, P
+
+
+def _kv_strides(t):
+    """(batch, head, row) element strides of a [batch, Hkv, L, d] view, or (0, 0, 0) when it is contiguous."""
+    return (0, 0, 0) if t.is_contiguous() else (t.stride(0), t.stride(1), t.stride(2))
 
 
 def nacl_version() -> int:
@@ -162,6 +186,8 @@ def nacl_evict(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed
                out_K=None, out_V=None, out_idx=None, stream=None):
     """include/nacl_evict.h `nacl_evict` / `nacl_evict_f32` on CUDA tensors.  Returns (out_K, out_V, out_idx)."""
     B, Hkv, L, d, Hq, P = _shapes(K, V, Qproxy)
+    if not (K.is_contiguous() and V.is_contiguous()):
+        raise ValueError("nacl_evict takes contiguous tensors (strided layouts: nacl_evict_ex)")
     if not K.is_cuda:
         raise ValueError("nacl_evict takes CUDA tensors (use nacl_evict_host for host buffers)")
     Cn = budget_proxy + budget_random
@@ -210,6 +236,10 @@ def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, s
     p.budget_proxy, p.budget_random, p.n_sink, p.n_recent = budget_proxy, budget_random, n_sink, n_recent
     p.seed, p.layer, p.flags = seed, layer, flags
     p.batch_offset, p.head_offset = batch_offset, head_offset
+    p.kv_stride_batch, p.kv_stride_head, p.kv_stride_row = _kv_strides(K)
+    if out_K.stride() != out_V.stride() or (Cn > 0 and out_K.stride(3) != 1):
+        raise ValueError("out_K and out_V must share their strides and have contiguous rows")
+    p.out_stride_batch, p.out_stride_head, p.out_stride_row = _kv_strides(out_K) if Cn > 0 else (0, 0, 0)
     if protect_idx is not None:
         assert protect_idx.is_cuda and protect_idx.dtype == torch.int32 and protect_idx.is_contiguous() and protect_idx.dim() == 1
         p.protect_idx, p.n_protect = protect_idx.data_ptr(), protect_idx.numel()
@@ -234,10 +264,55 @@ def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, s
     return out
 
 
+def nacl_evict_generation(K_cache, V_cache, q, length, budget_proxy, budget_random, n_sink, n_recent, seed, layer, step,
+                          K_out, V_out, pos_in=None, pos_out=None, flags=0, want_idx=False, want_importance=False,
+                          workspace=None, stream=None, batch_offset=0, head_offset=0):
+    """include/nacl_evict.h `nacl_evict_generation`: caches [B,Hkv,cap,d] (contiguous), q [B,Hq,1,d]; the first `length`
+    rows of every head are live.  Returns a dict (out_idx / importance when asked)."""
+    B, Hkv, cap_in, d = K_cache.shape
+    Hq = q.shape[1]
+    for t in (K_cache, V_cache, q, K_out, V_out):
+        if not (t.is_cuda and t.is_contiguous()):
+            raise ValueError("nacl_evict_generation takes contiguous CUDA tensors")
+    dev = K_cache.device
+    Cn = budget_proxy + budget_random
+    g = NaclGenParams()
+    g.struct_size = C.sizeof(NaclGenParams)
+    g.dtype = _dtype_tag(K_cache)
+    g.K_cache, g.V_cache, g.q = K_cache.data_ptr(), V_cache.data_ptr(), q.data_ptr()
+    g.batch, g.Hq, g.Hkv, g.d, g.len, g.cap_in, g.cap_out = B, Hq, Hkv, d, length, cap_in, K_out.shape[2]
+    g.budget_proxy, g.budget_random, g.n_sink, g.n_recent = budget_proxy, budget_random, n_sink, n_recent
+    g.seed, g.layer, g.step, g.flags = seed, layer, step, flags
+    g.batch_offset, g.head_offset = batch_offset, head_offset
+    g.K_out, g.V_out = K_out.data_ptr(), V_out.data_ptr()
+    if pos_in is not None:
+        assert pos_in.dtype == torch.int32 and pos_out.dtype == torch.int32 and pos_in.is_contiguous() and pos_out.is_contiguous()
+        g.pos_in, g.pos_out = pos_in.data_ptr(), pos_out.data_ptr()
+    idx = torch.empty((B, Hkv, max(Cn, 0)), dtype=torch.int32, device=dev) if want_idx else None
+    imp = torch.empty((B, Hkv, length), dtype=torch.float32, device=dev) if want_importance else None
+    g.out_idx = idx.data_ptr() if idx is not None else None
+    g.out_importance = imp.data_ptr() if imp is not None else None
+    if workspace is not None:
+        g.workspace, g.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
+    g.stream = (stream or torch.cuda.current_stream(dev)).cuda_stream
+    with torch.cuda.device(dev):
+        rc = _lib.nacl_evict_generation(C.byref(g))
+    if rc != 0:
+        raise NaclError(rc, "nacl_evict_generation")
+    out = {}
+    if idx is not None:
+        out["out_idx"] = idx
+    if imp is not None:
+        out["importance"] = imp
+    return out
+
+
 def nacl_evict_host(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer,
                     out_K=None, out_V=None, out_idx=None, device=-1):
     """include/nacl_evict.h `nacl_evict_host`: HOST tensors in, HOST tensors out (copies inside, synchronous)."""
     B, Hkv, L, d, Hq, P = _shapes(K, V, Qproxy)
+    if not (K.is_contiguous() and V.is_contiguous()):
+        raise ValueError("nacl_evict_host takes contiguous tensors")
     if K.is_cuda:
         raise ValueError("nacl_evict_host takes host tensors")
     Cn = budget_proxy + budget_random

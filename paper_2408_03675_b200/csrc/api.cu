@@ -83,6 +83,7 @@ Workspace carve_workspace(void* base, int batch, int L, int Hq, int Hkv, int P) 
   ws.sync = reinterpret_cast<int*>(b + off);    off = align_up(off + sync_ints((size_t)batch * Hkv) * sizeof(int), 256);
   ws.imp_sh = reinterpret_cast<float*>(b + off); off = align_up(off + (size_t)batch * L * sizeof(float), 256);
   ws.idx_sh = reinterpret_cast<int32_t*>(b + off); off = align_up(off + (size_t)batch * L * sizeof(int32_t), 256);
+  ws.idx_tmp = reinterpret_cast<int32_t*>(b + off); off = align_up(off + n_imp * sizeof(int32_t), 256);
   ws.bytes = off;
   return ws;
 }
@@ -193,6 +194,22 @@ static int evict_impl(const nacl_params_t& p) {
   s.G = p.Hq / p.Hkv; s.rows = s.G * p.P; s.dtype = p.dtype; s.esize = p.dtype == NACL_DTYPE_F32 ? 4 : 2;
   const int row_bytes = s.d * s.esize;
   if (row_bytes % 16 != 0) return NACL_ERR_ALIGN;
+  const int C = p.budget_proxy + p.budget_random;
+  // layouts: all-zero strides = contiguous
+  {
+    const bool kv0 = p.kv_stride_batch == 0 && p.kv_stride_head == 0 && p.kv_stride_row == 0;
+    const bool o0 = p.out_stride_batch == 0 && p.out_stride_head == 0 && p.out_stride_row == 0;
+    if (!kv0 && (p.kv_stride_batch <= 0 || p.kv_stride_head <= 0 || p.kv_stride_row < p.d)) return NACL_ERR_SHAPE;
+    if (!o0 && (p.out_stride_batch <= 0 || p.out_stride_head <= 0 || p.out_stride_row < p.d)) return NACL_ERR_SHAPE;
+    s.kv_sr = kv0 ? p.d : p.kv_stride_row;
+    s.kv_sh = kv0 ? (long long)p.L * p.d : p.kv_stride_head;
+    s.kv_sb = kv0 ? (long long)p.Hkv * p.L * p.d : p.kv_stride_batch;
+    s.o_sr = o0 ? p.d : p.out_stride_row;
+    s.o_sh = o0 ? (long long)C * p.d : p.out_stride_head;
+    s.o_sb = o0 ? (long long)p.Hkv * C * p.d : p.out_stride_batch;
+    const long long epv = 16 / s.esize;
+    if (s.kv_sr % epv || s.kv_sh % epv || s.kv_sb % epv || s.o_sr % epv || s.o_sh % epv || s.o_sb % epv) return NACL_ERR_ALIGN;
+  }
   if (!aligned16(p.K) || !aligned16(p.V) || !aligned16(p.Qproxy) || !aligned16(p.out_K) || !aligned16(p.out_V) ||
       (reinterpret_cast<uintptr_t>(p.out_idx) & 3u))
     return NACL_ERR_ALIGN;
@@ -217,7 +234,6 @@ static int evict_impl(const nacl_params_t& p) {
 
   const bool tc = !(p.flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
   if (p.lse_in && (reinterpret_cast<uintptr_t>(p.lse_in) & 3u)) return NACL_ERR_ALIGN;
-  const int C = p.budget_proxy + p.budget_random;
   const bool causal = (p.flags & NACL_FLAG_CAUSAL) != 0;
   if (tc) e = launch_score_tc(s, p.K, p.Qproxy, sp, ws, p.lse_in, causal, p.out_importance, p.out_lse, st);
   else e = launch_score_generic(s, p.K, p.Qproxy, sp, ws, p.lse_in, causal, p.out_importance, p.out_lse, st);
@@ -230,17 +246,17 @@ static int evict_impl(const nacl_params_t& p) {
     if ((e = launch_head_sum(ws.imp, ws.imp_sh, p.batch, p.Hkv, p.L, st)) != cudaSuccess) return fail_cuda(e);
     if ((e = launch_protect(ws.imp_sh, p.batch, p.L, p.protect_idx, p.n_protect, st)) != cudaSuccess) return fail_cuda(e);
     e = launch_select(ws.imp_sh, ws.key, p.batch, 1, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
-                      p.flags, ws.idx_sh, nullptr, nullptr, nullptr, nullptr, row_bytes, &gathered, p.batch_offset, p.head_offset, st);
+                      p.flags, ws.idx_sh, nullptr, nullptr, nullptr, nullptr, row_bytes, &gathered, p.batch_offset, p.head_offset, &s, st);
     if (e == cudaSuccess) e = launch_replicate_idx(ws.idx_sh, p.out_idx, p.batch, p.Hkv, C, st);
   } else {
     if ((e = launch_protect(ws.imp, p.batch * p.Hkv, p.L, p.protect_idx, p.n_protect, st)) != cudaSuccess) return fail_cuda(e);
     e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
-                      p.flags, p.out_idx, p.K, p.V, p.out_K, p.out_V, row_bytes, &gathered, p.batch_offset, p.head_offset, st);
+                      p.flags, p.out_idx, p.K, p.V, p.out_K, p.out_V, row_bytes, &gathered, p.batch_offset, p.head_offset, &s, st);
   }
   if (e != cudaSuccess) return fail_cuda(e);
   if (!gathered) {
     StageScope sc(ST_GATHER, st);
-    e = launch_gather(p.K, p.V, p.out_idx, p.batch * p.Hkv, p.L, C, row_bytes, p.out_K, p.out_V, st);
+    e = launch_gather(p.K, p.V, p.out_idx, s, C, row_bytes, p.out_K, p.out_V, st);
   }
   if (e != cudaSuccess) return fail_cuda(e);
   return NACL_OK;
@@ -286,6 +302,58 @@ int nacl_evict_ex(const nacl_params_t* p) {
   if (!p) return NACL_ERR_NULL;
   if (p->struct_size != sizeof(nacl_params_t)) return NACL_ERR_UNSUPPORTED;
   return evict_impl(*p);
+}
+
+int nacl_evict_generation(const nacl_gen_params_t* g) {
+  if (!g) return NACL_ERR_NULL;
+  if (g->struct_size != sizeof(nacl_gen_params_t)) return NACL_ERR_UNSUPPORTED;
+  if (!g->K_cache || !g->V_cache || !g->q || !g->K_out || !g->V_out) return NACL_ERR_NULL;
+  if ((g->pos_in == nullptr) != (g->pos_out == nullptr)) return NACL_ERR_NULL;
+  if (g->reserved0 != 0 || (g->flags & NACL_FLAG_CAUSAL)) return NACL_ERR_UNSUPPORTED;  // one query row: nothing to mask
+  if (g->len < 1 || g->cap_in < g->len || g->step < 0) return NACL_ERR_SHAPE;
+  const long C = (long)g->budget_proxy + g->budget_random;
+  if (g->budget_proxy < 0 || g->budget_random < 0 || g->cap_out < C) return NACL_ERR_BUDGET;
+  int rc = validate_shape(g->dtype, g->batch, g->len, g->Hq, g->Hkv, g->d, 1);
+  if (rc) return rc;
+  nacl_params_t p{};
+  p.struct_size = sizeof(nacl_params_t);
+  p.dtype = g->dtype;
+  p.K = g->K_cache; p.V = g->V_cache; p.Qproxy = g->q;
+  p.batch = g->batch; p.L = g->len; p.Hq = g->Hq; p.Hkv = g->Hkv; p.d = g->d; p.P = 1;
+  p.budget_proxy = g->budget_proxy; p.budget_random = g->budget_random; p.n_sink = g->n_sink; p.n_recent = g->n_recent;
+  p.seed = g->seed + (uint64_t)g->step * 0x9E3779B97F4A7C15ull;  // an independent stream per decoding step (R16)
+  p.layer = g->layer; p.flags = g->flags;
+  p.out_K = g->K_out; p.out_V = g->V_out;
+  p.out_importance = g->out_importance;
+  p.workspace = g->workspace; p.workspace_bytes = g->workspace_bytes; p.stream = g->stream;
+  p.batch_offset = g->batch_offset; p.head_offset = g->head_offset;
+  p.kv_stride_row = g->d; p.kv_stride_head = (int64_t)g->cap_in * g->d; p.kv_stride_batch = (int64_t)g->Hkv * g->cap_in * g->d;
+  p.out_stride_row = g->d; p.out_stride_head = (int64_t)g->cap_out * g->d; p.out_stride_batch = (int64_t)g->Hkv * g->cap_out * g->d;
+  int32_t* idx = g->out_idx;
+  if (!idx && C > 0) {
+    // the kept slots are needed for the position map even when the caller does not want them: take them from the workspace
+    void* wsp = g->workspace;
+    const size_t need = nacl_workspace_bytes(g->batch, g->len, g->Hq, g->Hkv, g->d, 1);
+    if (wsp) {
+      if (g->workspace_bytes < need || (reinterpret_cast<uintptr_t>(wsp) & 255u)) return NACL_ERR_WORKSPACE;
+    } else {
+      int dev = 0;
+      cudaError_t e = cudaGetDevice(&dev);
+      if (e != cudaSuccess) return fail_cuda(e);
+      if (dev < 0 || dev >= 64) return NACL_ERR_UNSUPPORTED;
+      std::lock_guard<std::mutex> lk(g_mu);
+      if ((e = stream_workspace(g_cache[dev], static_cast<cudaStream_t>(g->stream), need, &wsp)) != cudaSuccess) return fail_cuda(e);
+      p.workspace = wsp;
+      p.workspace_bytes = need;
+    }
+    idx = carve_workspace(wsp, g->batch, g->len, g->Hq, g->Hkv, 1).idx_tmp;
+  }
+  p.out_idx = idx;
+  rc = evict_impl(p);
+  if (rc != NACL_OK || !g->pos_in || C == 0) return rc;
+  cudaError_t e = launch_compose_positions(g->pos_in, g->cap_in, idx, g->batch * g->Hkv, (int)C, g->pos_out, g->cap_out,
+                                           static_cast<cudaStream_t>(g->stream));
+  return e == cudaSuccess ? NACL_OK : fail_cuda(e);
 }
 
 int nacl_evict_host(const void* K, const void* V, const void* Qproxy, int dtype, int batch, int L, int Hq, int Hkv, int d,

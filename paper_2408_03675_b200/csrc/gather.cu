@@ -20,13 +20,15 @@ __device__ __forceinline__ void st_stream(int4* p, const int4& v) {
 constexpr int GT = 256;  // threads per block
 constexpr int GU = 4;    // vectors of K and of V in flight per thread
 
-// vpr = 16-byte vectors per row; n_vec = n_prob * C * vpr output vectors per tensor
+// vpr = 16-byte vectors per row; n_vec = n_prob * C * vpr output vectors per tensor.  Strides in 16-byte vectors:
+// (sb, sh, sr) of K/V per batch element / kv head / row, (ob, oh, orow) of the outputs.
+struct GatherLayout { long long sb, sh, sr, ob, oh, orow; int Hkv; };
 __global__ void __launch_bounds__(GT) nacl_gather_kernel(const int4* __restrict__ K, const int4* __restrict__ V,
-                                                     const int32_t* __restrict__ idx, int L, int C, int vpr,
+                                                     const int32_t* __restrict__ idx, int C, int vpr, GatherLayout ly,
                                                      size_t n_vec, int4* __restrict__ oK, int4* __restrict__ oV) {
   const size_t stride = (size_t)gridDim.x * GT;
   for (size_t v0 = (size_t)blockIdx.x * GT + threadIdx.x; v0 < n_vec; v0 += stride * GU) {
-    size_t src[GU];
+    size_t src[GU], dst[GU];
     bool ok[GU];
 #pragma unroll
     for (int u = 0; u < GU; ++u) {
@@ -36,22 +38,33 @@ __global__ void __launch_bounds__(GT) nacl_gather_kernel(const int4* __restrict_
         const size_t row = v / (size_t)vpr;          // p * C + c
         const int off = (int)(v - row * (size_t)vpr);
         const size_t p = row / (size_t)C;
+        const int c = (int)(row - p * (size_t)C);
+        const int b = (int)(p / (size_t)ly.Hkv), hk = (int)(p - (size_t)b * ly.Hkv);
         const int j = idx[row];
-        src[u] = (p * (size_t)L + (size_t)j) * (size_t)vpr + off;
+        src[u] = (size_t)(b * ly.sb + hk * ly.sh + (long long)j * ly.sr) + off;
+        dst[u] = (size_t)(b * ly.ob + hk * ly.oh + (long long)c * ly.orow) + off;
       }
     }
-    int4 a[GU], b[GU];
+    int4 a[GU], b4[GU];
 #pragma unroll
     for (int u = 0; u < GU; ++u)
-      if (ok[u]) { a[u] = ld_stream(K + src[u]); b[u] = ld_stream(V + src[u]); }
+      if (ok[u]) { a[u] = ld_stream(K + src[u]); b4[u] = ld_stream(V + src[u]); }
 #pragma unroll
     for (int u = 0; u < GU; ++u)
       if (ok[u]) {
-        const size_t v = v0 + (size_t)u * stride;
-        st_stream(oK + v, a[u]);
-        st_stream(oV + v, b[u]);
+        st_stream(oK + dst[u], a[u]);
+        st_stream(oV + dst[u], b4[u]);
       }
   }
+}
+
+__global__ void __launch_bounds__(256) nacl_compose_positions_kernel(const int32_t* __restrict__ pos_in, long long in_stride,
+                                                                     const int32_t* __restrict__ idx, int C,
+                                                                     int32_t* __restrict__ pos_out, long long out_stride) {
+  const int p = blockIdx.y;
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= C) return;
+  pos_out[(size_t)p * out_stride + c] = pos_in[(size_t)p * in_stride + idx[(size_t)p * C + c]];
 }
 
 // ---- small helpers of the selection variants
@@ -96,15 +109,24 @@ cudaError_t launch_protect(float* imp, int n_prob, int L, const int32_t* protect
   return cudaGetLastError();
 }
 
-cudaError_t launch_gather(const void* K, const void* V, const int32_t* idx, int n_prob, int L, int C, int row_bytes,
+cudaError_t launch_gather(const void* K, const void* V, const int32_t* idx, const Shape& s, int C, int row_bytes,
                           void* out_K, void* out_V, cudaStream_t st) {
   const int vpr = row_bytes / 16;
-  const size_t n_vec = (size_t)n_prob * C * vpr;
+  const size_t n_vec = (size_t)s.batch * s.Hkv * C * vpr;
   if (n_vec == 0) return cudaSuccess;
+  const long long epv = 16 / s.esize;  // elements per 16-byte vector (strides are multiples of it)
+  const GatherLayout ly{s.kv_sb / epv, s.kv_sh / epv, s.kv_sr / epv, s.o_sb / epv, s.o_sh / epv, s.o_sr / epv, s.Hkv};
   size_t want = (n_vec + (size_t)GT * GU - 1) / ((size_t)GT * GU);
   const size_t cap = (size_t)kNumSMs * 8 * 4;  // a few waves of 8 resident CTAs per SM
   int blocks = (int)(want < cap ? want : cap);
-  nacl_gather_kernel<<<blocks, GT, 0, st>>>((const int4*)K, (const int4*)V, idx, L, C, vpr, n_vec, (int4*)out_K, (int4*)out_V);
+  nacl_gather_kernel<<<blocks, GT, 0, st>>>((const int4*)K, (const int4*)V, idx, C, vpr, ly, n_vec, (int4*)out_K, (int4*)out_V);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_compose_positions(const int32_t* pos_in, long long in_stride, const int32_t* idx, int n_prob, int C,
+                                     int32_t* pos_out, long long out_stride, cudaStream_t st) {
+  if (C == 0 || n_prob == 0) return cudaSuccess;
+  nacl_compose_positions_kernel<<<dim3((C + 255) / 256, n_prob), 256, 0, st>>>(pos_in, in_stride, idx, C, pos_out, out_stride);
   return cudaGetLastError();
 }
 

@@ -20,6 +20,8 @@ struct Shape {
   int rows;     // G * P proxy rows per kv head
   int dtype;    // NACL_DTYPE_*
   int esize;    // bytes per element
+  // element strides of K and V (batch, kv head, key row; the d elements of a row are contiguous) and of out_K / out_V
+  long long kv_sb, kv_sh, kv_sr, o_sb, o_sh, o_sr;
 };
 
 // How L is split for the split-L softmax statistics (a pure function of the shape).
@@ -39,6 +41,7 @@ struct Workspace {
   int* sync;           // [sync_ints(heads)]      reserved (counters / flags for future fused variants)
   float* imp_sh;       // [batch, L]              NACL_FLAG_SHARED_HEADS: importance summed over the kv heads
   int32_t* idx_sh;     // [batch, L]              NACL_FLAG_SHARED_HEADS: the shared retained set (C <= L entries per batch element)
+  int32_t* idx_tmp;    // [batch*Hkv, L]          nacl_evict_generation without out_idx: the kept slots
   size_t bytes;
 };
 inline size_t sync_ints(size_t heads) { return 16 + 2 * heads; }
@@ -84,7 +87,7 @@ size_t select_scratch_words(int batch, int Hkv, int L);  // 4-byte words of Work
 cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, int L, int budget_proxy, int budget_random,
                           int n_sink, int n_recent, uint64_t seed, int layer, uint32_t flags, int32_t* out_idx,
                           const void* K, const void* V, void* out_K, void* out_V, int row_bytes, bool* gathered,
-                          int batch_offset, int head_offset, cudaStream_t st);
+                          int batch_offset, int head_offset, const Shape* layout, cudaStream_t st);
 
 // NACL_FLAG_SHARED_HEADS: out[b, j] = sum over the kv heads (in head order, fp32) of imp[b, hk, j]
 cudaError_t launch_head_sum(const float* imp, float* out, int batch, int Hkv, int L, cudaStream_t st);
@@ -94,8 +97,13 @@ cudaError_t launch_replicate_idx(const int32_t* shared, int32_t* idx, int batch,
 cudaError_t launch_protect(float* imp, int n_prob, int L, const int32_t* protect_idx, int n_protect, cudaStream_t st);
 
 // K,V <- K_S,V_S
-cudaError_t launch_gather(const void* K, const void* V, const int32_t* idx, int n_prob, int L, int C,
+// layout: element strides of K/V and of out_K/out_V (Shape::kv_* / o_*), batch x Hkv problems
+cudaError_t launch_gather(const void* K, const void* V, const int32_t* idx, const Shape& layout, int C,
                           int row_bytes, void* out_K, void* out_V, cudaStream_t st);
+// pos_out[p, c] = pos_in[p, idx[p, c]] (int32 rows of length L_in / C_out per problem, row strides given): the
+// position map of a cache that is evicted again (generation phase)
+cudaError_t launch_compose_positions(const int32_t* pos_in, long long in_stride, const int32_t* idx, int n_prob, int C,
+                                     int32_t* pos_out, long long out_stride, cudaStream_t st);
 
 // ------------------------------------------------------------------ small device helpers
 __device__ __forceinline__ float warp_max(float v) {

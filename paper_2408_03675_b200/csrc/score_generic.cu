@@ -21,12 +21,13 @@ __device__ __forceinline__ float to_float(float v) { return v; }
 __device__ __forceinline__ float to_float(__nv_bfloat16 v) { return __bfloat162float(v); }
 
 // rows [row0, row0+n_valid) of a [*, d] matrix -> smem [64][d+1] as fp32, zero rows beyond n_valid
+// (rs = elements between consecutive rows of src)
 template <typename T>
-__device__ __forceinline__ void stage_rows(const T* __restrict__ src, int n_valid, int d, float* dst) {
+__device__ __forceinline__ void stage_rows(const T* __restrict__ src, int n_valid, int d, float* dst, long long rs) {
   const int ld = d + 1;
   for (int e = threadIdx.x; e < 64 * d; e += NT) {
     int r = e / d, t = e - r * d;
-    dst[r * ld + t] = r < n_valid ? to_float(src[(size_t)r * d + t]) : 0.f;
+    dst[r * ld + t] = r < n_valid ? to_float(src[(size_t)r * rs + t]) : 0.f;
   }
 }
 
@@ -53,7 +54,7 @@ __device__ __forceinline__ size_t row_id(int b, int hk, int gr, int G, int P, in
 template <typename T>
 __global__ void __launch_bounds__(NT) nacl_stats_kernel(const T* __restrict__ K, const T* __restrict__ Q, float2* __restrict__ part,
                                                     int L, int Hq, int Hkv, int d, int P, int G, int chunk, int n_chunks,
-                                                    float inv_sqrt_d, int causal) {
+                                                    float inv_sqrt_d, int causal, long long sb, long long sh, long long sr) {
   extern __shared__ float smem[];
   const int ld = d + 1;
   float* Qs = smem;            // [64][d+1]
@@ -62,19 +63,19 @@ __global__ void __launch_bounds__(NT) nacl_stats_kernel(const T* __restrict__ K,
   const int c = blockIdx.x, hk = blockIdx.y, b = blockIdx.z;
   const int rows = G * P;
   const int j_begin = c * chunk, j_end = min(L, j_begin + chunk);
-  const T* Kh = K + ((size_t)b * Hkv + hk) * (size_t)L * d;
+  const T* Kh = K + (size_t)b * sb + (size_t)hk * sh;
   const T* Qh = Q + ((size_t)b * Hq + (size_t)hk * G) * (size_t)P * d;  // the group's G*P rows are contiguous
   const int r = threadIdx.x & 63, sub = threadIdx.x >> 6;
 
   for (int rb = 0; rb < rows; rb += RB) {
     const int nr = min(RB, rows - rb);
     __syncthreads();
-    stage_rows(Qh + (size_t)rb * d, nr, d, Qs);
+    stage_rows(Qh + (size_t)rb * d, nr, d, Qs, d);
     float m = -INFINITY, z = 0.f;
     for (int j0 = j_begin; j0 < j_end; j0 += TK) {
       const int nk = min(TK, j_end - j0);
       __syncthreads();
-      stage_rows(Kh + (size_t)j0 * d, nk, d, Ks);
+      stage_rows(Kh + (size_t)j0 * sr, nk, d, Ks, sr);
       __syncthreads();
       float a[U];
       dots(Qs, r, Ks, sub, d, a);
@@ -117,7 +118,8 @@ __global__ void nacl_combine_kernel(const float2* __restrict__ part, float* __re
 template <typename T>
 __global__ void __launch_bounds__(NT) nacl_colsum_kernel(const T* __restrict__ K, const T* __restrict__ Q, const float* __restrict__ lse,
                                                      float* __restrict__ imp, float* __restrict__ imp_out,
-                                                     int L, int Hq, int Hkv, int d, int P, int G, float inv_sqrt_d, int causal) {
+                                                     int L, int Hq, int Hkv, int d, int P, int G, float inv_sqrt_d, int causal,
+                                                     long long sb, long long sh, long long sr) {
   extern __shared__ float smem[];
   const int ld = d + 1;
   float* Qs = smem;
@@ -128,16 +130,16 @@ __global__ void __launch_bounds__(NT) nacl_colsum_kernel(const T* __restrict__ K
   const int rows = G * P;
   const int j0 = blockIdx.x * TK;
   const int nk = min(TK, L - j0);
-  const T* Kh = K + ((size_t)b * Hkv + hk) * (size_t)L * d;
+  const T* Kh = K + (size_t)b * sb + (size_t)hk * sh;
   const T* Qh = Q + ((size_t)b * Hq + (size_t)hk * G) * (size_t)P * d;
   const int j = threadIdx.x & 63, sub = threadIdx.x >> 6;
 
-  stage_rows(Kh + (size_t)j0 * d, nk, d, Ks);
+  stage_rows(Kh + (size_t)j0 * sr, nk, d, Ks, sr);
   float acc = 0.f;
   for (int rb = 0; rb < rows; rb += RB) {
     const int nr = min(RB, rows - rb);
     __syncthreads();
-    stage_rows(Qh + (size_t)rb * d, nr, d, Qs);
+    stage_rows(Qh + (size_t)rb * d, nr, d, Qs, d);
     if (threadIdx.x < RB) lse_s[threadIdx.x] = threadIdx.x < nr ? lse[row_id(b, hk, rb + threadIdx.x, G, P, Hq)] : 0.f;
     __syncthreads();
     float a[U];
@@ -179,7 +181,7 @@ cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const Spl
   {
     StageScope sc(ST_STATS, st);
     nacl_stats_kernel<T><<<g1, NT, smem, st>>>((const T*)K, (const T*)Q, ws.part, s.L, s.Hq, s.Hkv, s.d, s.P, s.G, sp.chunk,
-                                          sp.n_chunks, inv_sqrt_d, causal ? 1 : 0);
+                                          sp.n_chunks, inv_sqrt_d, causal ? 1 : 0, s.kv_sb, s.kv_sh, s.kv_sr);
   }
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   {
@@ -192,7 +194,7 @@ cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const Spl
   {
     StageScope sc(ST_COLSUM, st);
     nacl_colsum_kernel<T><<<g2, NT, smem, st>>>((const T*)K, (const T*)Q, lse, ws.imp, imp_out, s.L, s.Hq, s.Hkv, s.d, s.P,
-                                           s.G, inv_sqrt_d, causal ? 1 : 0);
+                                           s.G, inv_sqrt_d, causal ? 1 : 0, s.kv_sb, s.kv_sh, s.kv_sr);
   }
   return cudaGetLastError();
 }

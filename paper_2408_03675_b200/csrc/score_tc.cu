@@ -94,6 +94,7 @@ __device__ long long g_tl[2][20][32][8];
 struct TcParams {
   int L, rows, T;          // keys per head, proxy rows per row block (G*P, or 256 when G*P > 256), key tiles per head
   int rows_total, nrb;     // G*P and the number of 256-row blocks (1 unless G*P > 256)
+  int Hkv;                 // kv heads per batch element (K tensor-map coordinates)
   int heads, n_slots;      // n_slots: epilogue warps that share a proxy row in sweep S = partials per (row, piece): 2 if rows > 128, else 4
   int phase;               // 0 = sweep S (statistics), 1 = sweep C (column sums)
   int causal, P;           // NACL_FLAG_CAUSAL: proxy row r (i = r % P, prompt position L-P+i) sees keys j <= L-P+i
@@ -140,9 +141,9 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm,
                ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(bar)
                : "memory");
 }
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar) {
-  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-               ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+               ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar)
                : "memory");
 }
 
@@ -610,14 +611,15 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
         tma_load_2d(qdst + QROWS * 128, &tmQ, 64, sg.head * p.rows_total + sg.rb * 256, q_full(qb));
       }
       ++qrun;
+      const int hb = sg.head / p.Hkv, hk = sg.head - hb * p.Hkv;  // K is addressed as [batch, kv head, key, d] with its own strides
       for (int i = 0; i < sg.n; ++i) {
         TRW(0, mbar_wait(k_empty(stage), kphase ^ 1));
         const uint32_t kdst = sbase + SM::OFF_K + stage * KSTAGE_BYTES;
         const int j0 = (sg.tile + walk.step * i) * TILE;
         if (leader) {
           mbar_expect_tx(k_full(stage), KSTAGE_BYTES);
-          tma_load_3d(kdst, &tmK, 0, j0, sg.head, k_full(stage));
-          tma_load_3d(kdst + BOX_BYTES, &tmK, 64, j0, sg.head, k_full(stage));
+          tma_load_4d(kdst, &tmK, 0, j0, hk, hb, k_full(stage));
+          tma_load_4d(kdst + BOX_BYTES, &tmK, 64, j0, hk, hb, k_full(stage));
         }
         if (++stage == STAGES) { stage = 0; kphase ^= 1; }
       }
@@ -1027,11 +1029,12 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
 
   alignas(64) CUtensorMap tmK, tmQ;
   {
-    const cuuint64_t dims[3] = {(cuuint64_t)HD, (cuuint64_t)s.L, (cuuint64_t)heads};
-    const cuuint64_t strides[2] = {(cuuint64_t)HD * 2, (cuuint64_t)s.L * HD * 2};
-    const cuuint32_t box[3] = {64, (cuuint32_t)TILE, 1};
-    const cuuint32_t es[3] = {1, 1, 1};
-    if (enc(&tmK, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(K), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    // [batch, Hkv, L, d] with the caller's strides (contiguous, a cache with spare capacity, or token-major [B,L,H,d])
+    const cuuint64_t dims[4] = {(cuuint64_t)HD, (cuuint64_t)s.L, (cuuint64_t)s.Hkv, (cuuint64_t)s.batch};
+    const cuuint64_t strides[3] = {(cuuint64_t)s.kv_sr * 2, (cuuint64_t)s.kv_sh * 2, (cuuint64_t)s.kv_sb * 2};
+    const cuuint32_t box[4] = {64, (cuuint32_t)TILE, 1, 1};
+    const cuuint32_t es[4] = {1, 1, 1, 1};
+    if (enc(&tmK, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(K), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
   }
@@ -1048,7 +1051,7 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
   TcParams p;
   p.L = s.L; p.rows = s.rows <= 256 ? s.rows : 256; p.T = (s.L + TILE - 1) / TILE;
   p.rows_total = s.rows; p.nrb = (s.rows + 255) / 256;
-  p.heads = heads;
+  p.heads = heads; p.Hkv = s.Hkv;
   p.n_slots = s.rows <= 128 ? 4 : 2;
   p.phase = 0;
   p.causal = causal ? 1 : 0; p.P = s.P;

@@ -289,6 +289,7 @@ __device__ __forceinline__ long long sel_gtimer() { long long t; asm volatile("m
 // Integer sums: exact and order-independent.  A buffer is rewritten only after a barrier that every reader reaches
 // after its reads, so single buffers suffice.
 constexpr int kMaxRanks = 16;
+struct KvVecLayout { long long sb, sh, sr, ob, oh, orow; };  // strides of K/V and of out_K/out_V in 16-byte vectors
 struct ClShared {
   uint32_t hist[HB];
   uint32_t xsup[kMaxRanks][64];   // [rank][super-bin]: pushed by every rank
@@ -483,7 +484,7 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
                                                                  uint32_t layer, uint32_t flags, int32_t* __restrict__ out_idx,
                                                                  const int4* __restrict__ Kv, const int4* __restrict__ Vv,
                                                                  int4* __restrict__ oKv, int4* __restrict__ oVv, int vpr,
-                                                                 uint32_t b_off, uint32_t h_off) {
+                                                                 uint32_t b_off, uint32_t h_off, KvVecLayout ly) {
   cg::cluster_group cluster = cg::this_cluster();
   extern __shared__ __align__(16) unsigned char dyn_raw[];
   ClShared& sh = *reinterpret_cast<ClShared*>(dyn_raw);
@@ -574,24 +575,26 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
   // consecutive threads on consecutive vectors of the output, four vectors of K and of V in flight per thread
   __syncthreads();
   const int n_vec = min(tot, C - base) * vpr;
-  const size_t src0 = (size_t)p * L * vpr, dst0 = ((size_t)p * C + base) * vpr;
+  // K/V and the outputs have their own strides (in 16-byte vectors); a row's vpr vectors are contiguous
+  const size_t src0 = (size_t)(b * ly.sb + hk * ly.sh), dst0 = (size_t)(b * ly.ob + hk * ly.oh + (long long)base * ly.orow);
   for (int v0 = threadIdx.x; v0 < n_vec; v0 += ST * 4) {
-    size_t src[4];
-    int4 a[4], b[4];
+    size_t src[4], dst[4];
+    int4 a[4], b4[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const int v = v0 + u * ST;
       if (v < n_vec) {
         const int row = v / vpr;
-        src[u] = src0 + (size_t)ib[row] * vpr + (v - row * vpr);
+        src[u] = src0 + (size_t)ib[row] * ly.sr + (v - row * vpr);
+        dst[u] = dst0 + (size_t)row * ly.orow + (v - row * vpr);
       }
     }
 #pragma unroll
     for (int u = 0; u < 4; ++u)
-      if (v0 + u * ST < n_vec) { a[u] = __ldcs(Kv + src[u]); b[u] = __ldcs(Vv + src[u]); }
+      if (v0 + u * ST < n_vec) { a[u] = __ldcs(Kv + src[u]); b4[u] = __ldcs(Vv + src[u]); }
 #pragma unroll
     for (int u = 0; u < 4; ++u)
-      if (v0 + u * ST < n_vec) { __stcs(oKv + dst0 + v0 + u * ST, a[u]); __stcs(oVv + dst0 + v0 + u * ST, b[u]); }
+      if (v0 + u * ST < n_vec) { __stcs(oKv + dst[u], a[u]); __stcs(oVv + dst[u], b4[u]); }
   }
 }
 
@@ -616,7 +619,7 @@ bool select_uses_cluster(int L) { return (L + kMaxRanks - 1) / kMaxRanks <= kMax
 cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, int L, int budget_proxy, int budget_random,
                           int n_sink, int n_recent, uint64_t seed, int layer, uint32_t flags, int32_t* out_idx,
                           const void* K, const void* V, void* out_K, void* out_V, int row_bytes, bool* gathered,
-                          int batch_offset, int head_offset, cudaStream_t st) {
+                          int batch_offset, int head_offset, const Shape* layout, cudaStream_t st) {
   *gathered = false;
   const int C = budget_proxy + budget_random;
   if (C == 0) return cudaSuccess;
@@ -679,10 +682,15 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   cfg.gridDim = dim3((unsigned)(heads * n));
   cfg.dynamicSmemBytes = dyn;
   attr[0].val.clusterDim.x = (unsigned)n;
+  KvVecLayout ly{};
+  if (K != nullptr) {
+    const long long epv = 16 / layout->esize;
+    ly = KvVecLayout{layout->kv_sb / epv, layout->kv_sh / epv, layout->kv_sr / epv, layout->o_sb / epv, layout->o_sh / epv, layout->o_sr / epv};
+  }
   StageScope sc(ST_SELECT, st);
   return cudaLaunchKernelEx(&cfg, nacl_select_cluster_kernel, imp, Hkv, L, Lc, k1, budget_random, n_sink, n_recent, C, sk0, sk1,
                             (uint32_t)layer, flags, out_idx, (const int4*)K, (const int4*)V, (int4*)out_K, (int4*)out_V,
-                            (*gathered = (K != nullptr)) ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset);
+                            (*gathered = (K != nullptr)) ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset, ly);
 }
 
 // 4-byte words of the `key` scratch the select needs (long-row path: the keys)

@@ -392,3 +392,97 @@ def test_log_table_every_interval_at_both_edges_and_the_centre(binding):
     _, keys_ref = oracle.select(imp, 0, 1, 0, 0, seed, layer, 0, return_keys=True)
     a, b = keys_gpu.view(np.int32).astype(np.int64), keys_ref.view(np.int32).astype(np.int64)
     assert int((a != b).sum()) <= 1 and np.abs(a - b).max() <= 1, f"{int((a != b).sum())} of {a.size} keys differ"
+
+
+# ------------------------------------------------------------------ layouts and generation phase (f3)
+@pytest.mark.parametrize("case", [(2, 1500, 8, 2, 128, 16, "bf16"), (2, 333, 4, 2, 64, 5, "f32"), (1, 70000, 4, 2, 128, 16, "bf16")],
+                         ids=["tc", "cuda_core", "long_rows"])
+@pytest.mark.parametrize("layout", ["cache_with_capacity", "token_major"])
+def test_strided_layouts_match_the_contiguous_call(binding, case, layout):
+    """K/V as views of a cache [B,Hkv,cap,d] with spare capacity, or of a token-major [B,L,Hkv,d] tensor (the two KV layouts
+    of FlashAttention-style kernels), and outputs written into a strided destination: bit-identical to the
+    contiguous call (which the oracle checks)."""
+    B, L, Hq, Hkv, d, P, dt = case
+    K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype=dt, seed=L + 23)
+    Kd, Vd, Qd = K.cuda(), V.cuda(), Q.cuda()
+    Bp, Br = L // 6, L // 12
+    C = Bp + Br
+    want = binding.nacl_evict_ex(Kd, Vd, Qd, Bp, Br, 4, P, 5, 1, want_importance=True)
+    if layout == "cache_with_capacity":
+        cap = L + 37 * 8
+        Kb, Vb = torch.zeros(B, Hkv, cap, d, dtype=Kd.dtype, device="cuda"), torch.zeros(B, Hkv, cap, d, dtype=Kd.dtype, device="cuda")
+        Kb[:, :, :L], Vb[:, :, :L] = Kd, Vd
+        Kv, Vv = Kb[:, :, :L], Vb[:, :, :L]
+        oKb, oVb = torch.zeros(B, Hkv, C + 24, d, dtype=Kd.dtype, device="cuda"), torch.zeros(B, Hkv, C + 24, d, dtype=Kd.dtype, device="cuda")
+        oK, oV = oKb[:, :, :C], oVb[:, :, :C]
+    else:
+        Kv, Vv = Kd.permute(0, 2, 1, 3).contiguous().permute(0, 2, 1, 3), Vd.permute(0, 2, 1, 3).contiguous().permute(0, 2, 1, 3)
+        oKb, oVb = torch.zeros(B, C, Hkv, d, dtype=Kd.dtype, device="cuda"), torch.zeros(B, C, Hkv, d, dtype=Kd.dtype, device="cuda")
+        oK, oV = oKb.permute(0, 2, 1, 3), oVb.permute(0, 2, 1, 3)
+    assert not Kv.is_contiguous()
+    got = binding.nacl_evict_ex(Kv, Vv, Qd, Bp, Br, 4, P, 5, 1, out_K=oK, out_V=oV, want_importance=True)
+    torch.cuda.synchronize()
+    assert torch.equal(got["importance"], want["importance"]) and torch.equal(got["out_idx"], want["out_idx"])
+    assert torch.equal(oK, want["out_K"]) and torch.equal(oV, want["out_V"])
+    if layout == "cache_with_capacity":
+        assert oKb[:, :, C:].abs().sum() == 0  # nothing written past the C live rows
+
+
+@pytest.mark.parametrize("case", [(2, 8, 2, 128, "bf16", 256, 4), (1, 4, 4, 64, "f32", 96, 3)], ids=["bf16_gqa", "f32_mha"])
+def test_generation_phase_eviction(binding, case):
+    """PAPER.md:66-70 and Algorithm 1, function Generation: every m steps the cache, grown to C + m
+    entries, is evicted back to C on the attention row of the current token (one proxy row per query head, protected = the
+    first slots and the newest slots).  Twelve decoding steps with appends; at every eviction the full parity protocol runs
+    against the oracle ON THE SAME CACHE STATE (an eviction of the live rows with P = 1 and the step's seed), the caches
+    ping-pong between two buffers with spare capacity, and the position map composes."""
+    from parity import check_e2e_sets, check_scores, check_staged, check_structure
+
+    B, Hq, Hkv, d, dt, C, m = case
+    tdt = torch.bfloat16 if dt == "bf16" else torch.float32
+    g = torch.Generator().manual_seed(C)
+    cap = C + m + 8
+    Bp, Br = (3 * C) // 4, C - (3 * C) // 4
+    ns, nr = 2, 4
+    bufs = [(torch.zeros(B, Hkv, cap, d, dtype=tdt, device="cuda"), torch.zeros(B, Hkv, cap, d, dtype=tdt, device="cuda"),
+             torch.zeros(B, Hkv, cap, dtype=torch.int32, device="cuda")) for _ in range(2)]
+    cur, length = 0, C
+    bufs[0][0][:, :, :C] = torch.randn(B, Hkv, C, d, generator=g).to(tdt).cuda()
+    bufs[0][1][:, :, :C] = torch.randn(B, Hkv, C, d, generator=g).to(tdt).cuda()
+    bufs[0][2][:, :, :C] = torch.arange(C, dtype=torch.int32, device="cuda")
+    n_evictions = 0
+    for t in range(1, 13):
+        Kc, Vc, pos = bufs[cur]
+        Kc[:, :, length] = (1.5 * torch.randn(B, Hkv, d, generator=g)).to(tdt).cuda()  # K_t = [K_{t-1}, z_t W_K]
+        Vc[:, :, length] = torch.randn(B, Hkv, d, generator=g).to(tdt).cuda()
+        pos[:, :, length] = 1000 + t
+        length += 1
+        if t % m != 0:
+            continue
+        q = (2.0 * torch.randn(B, Hq, 1, d, generator=g)).to(tdt).cuda()
+        Ko, Vo, po = bufs[1 - cur]
+        Ko.zero_(); Vo.zero_(); po.zero_()
+        res = binding.nacl_evict_generation(Kc, Vc, q, length, Bp, Br, ns, nr, 77, 5, t, Ko, Vo, pos_in=pos, pos_out=po,
+                                            want_idx=True, want_importance=True, head_offset=1)
+        torch.cuda.synchronize()
+        idx, imp = res["out_idx"].cpu().numpy(), res["importance"].cpu().numpy()
+        Kh, Vh, qh = Kc[:, :, :length].cpu().contiguous(), Vc[:, :, :length].cpu().contiguous(), q.cpu()
+        seed_t = (77 + t * 0x9E3779B97F4A7C15) % (1 << 64)
+        imp_ref = oracle.importance(Kh, qh)
+        check_scores(imp, imp_ref, Hq // Hkv, 1)
+        check_structure(idx, length, C, ns, nr)
+        part = check_staged(idx, imp, Bp, Br, ns, nr, seed_t, 5, head_offset=1)
+        check_e2e_sets(idx, part, imp_ref, Bp, Br, ns, nr, seed_t, 5, head_offset=1)
+        ti = torch.from_numpy(idx.astype(np.int64)).cuda()
+        assert torch.equal(Ko[:, :, :C], torch.gather(Kc, 2, ti[..., None].expand(-1, -1, -1, d)))
+        assert torch.equal(Vo[:, :, :C], torch.gather(Vc, 2, ti[..., None].expand(-1, -1, -1, d)))
+        assert torch.equal(po[:, :, :C].long(), torch.gather(pos.long(), 2, ti))
+        assert Ko[:, :, C:].abs().sum() == 0
+        # without out_idx the call keeps the slots in its workspace and gives the same cache
+        Ko2, Vo2, po2 = torch.zeros_like(Ko), torch.zeros_like(Vo), torch.zeros_like(po)
+        binding.nacl_evict_generation(Kc, Vc, q, length, Bp, Br, ns, nr, 77, 5, t, Ko2, Vo2, pos_in=pos, pos_out=po2, head_offset=1)
+        assert torch.equal(Ko2, Ko) and torch.equal(po2, po)
+        cur, length = 1 - cur, C
+        n_evictions += 1
+    assert n_evictions == 12 // m
+    # the newest tokens (protected recent slots) survive every eviction
+    assert (bufs[cur][2][:, :, C - 1] == 1000 + (12 // m) * m).all()

@@ -51,7 +51,8 @@
  *
  * Supported: 1 <= P <= L <= 2^24; Hq % Hkv == 0; d a multiple of 16, d <= 256; any L (ragged
  * last tile is masked).  The tensor-core path (tcgen05 + TMA) serves bf16, d == 128 and
- * G*P a multiple of 16 up to 256 or a multiple of 256 (blocks of 256 proxy rows); every other shape runs the generic
+ * G*P a multiple of 16 up to 8192 (above 256 in blocks of 256 proxy rows, the last block masked where G*P is off that
+ * grid: the paper's proxy share of 3-20 % of the prompt); every other shape runs the generic
  * CUDA-core kernels of the same library.
  */
 #ifndef NACL_EVICT_H

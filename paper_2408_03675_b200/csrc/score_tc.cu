@@ -244,14 +244,14 @@ __device__ __forceinline__ u64 exp2_mufu2(u64 x) {
   return pack2(fast_exp2(a), fast_exp2(b));
 }
 // acc += (2^x0, 2^x1) on the FMA pipe, for x = s*sc - ref given as the raw logits s and the two constants
-//   scy = sc / 227,  cy = (110 - ref) / 227:
-// y = sat(s*scy + cy) in [0, 1] IS the clamp of x to [-110, 117] (one saturating FMA, no min/max: values below stand
-// for zero -- 2^-110 * 256 rows < the 1e-30 absolute score tolerance -- and values above for "too large", which sweep S
-// turns into a new reference, see s_lazy32); u = 227*y = x + 110 in [0, 227]; n = floor(u) by a round-down FMA onto
-// 1.5*2^23, f = u - n in [0, 1]; 2^f by the degree-3 minimax polynomial (relative error <= 7.5e-5); 2^(n-110) is built
-// in the exponent field (17 + n in [17, 244]) and multiplied in by the FMA that accumulates.  y resolves x to
-// 227 * 2^-24 = 1.4e-5, i.e. 1e-5 relative in 2^x.  8 FMA-pipe instructions and 2 integer ones per pair.
-constexpr float kPolyLo = 110.f, kPolySpan = 227.f;
+//   scy = sc / 227,  cy = (127 - ref) / 227:
+// y = sat(s*scy + cy) in [0, 1] IS the clamp of x to [-127, 100] (one saturating FMA, no min/max); u = 227*y = x + 127 in
+// [0, 227]; n = floor(u) by a round-down FMA onto 1.5*2^23, f = u - n in [0, 1]; 2^f by the degree-3 minimax polynomial
+// (relative error <= 7.5e-5); 2^(n-127) is the float whose exponent FIELD is n -- one shift -- multiplied in by the FMA that
+// accumulates.  n = 0 (x < -126, or cy = -inf for a masked row) gives the scale +0.0: an exact zero, as MUFU.EX2.FTZ gives
+// there.  x > 100 saturates at 2^100, which sweep S turns into a new reference (s_lazy32).  y resolves x to
+// 227 * 2^-24 = 1.4e-5, i.e. 1e-5 relative in 2^x.  8 FMA-pipe instructions and 2 shifts per pair.
+constexpr float kPolyLo = 127.f, kPolySpan = 227.f;
 __device__ __forceinline__ u64 acc_exp2_poly_sat(u64 acc, uint32_t s0, uint32_t s1, float scy, float cy0, float cy1) {
   const u64 y = pack2(fma_sat(__uint_as_float(s0), scy, cy0), fma_sat(__uint_as_float(s1), scy, cy1));
   const u64 span = pack2(kPolySpan, kPolySpan), magic = pack2(12582912.f, 12582912.f);
@@ -262,7 +262,7 @@ __device__ __forceinline__ u64 acc_exp2_poly_sat(u64 acc, uint32_t s0, uint32_t 
   p = fma2(p, f, pack2(0.9999252f, 0.9999252f));
   float t0, t1;
   unpack2(t, t0, t1);
-  const u64 pw = pack2u((__float_as_uint(t0) << 23) + (17u << 23), (__float_as_uint(t1) << 23) + (17u << 23));
+  const u64 pw = pack2u(__float_as_uint(t0) << 23, __float_as_uint(t1) << 23);  // the magic constant's bits shift out: n << 23
   return fma2(p, pw, acc);
 }
 template <uint32_t MASK>
@@ -402,7 +402,7 @@ __device__ __forceinline__ void s_update(const uint32_t (&v)[32], float sc, floa
 }
 // Lazy reference (sweep S, full tiles).  The running sum is a plain fp32 sum of 2^(s*sc - m) for a reference m that
 // stays where it is: fp32 keeps full relative accuracy for any m within ~100 (log2) of the values, so no running max
-// and no rescale are needed per chunk.  Only when the sum leaves [0, 2^100) -- a value far above m, or the first chunk
+// and no rescale are needed per chunk.  Only when the sum leaves [0, 2^99) -- a value far above m, or the first chunk
 // of a segment (m = -inf gives inf/NaN) -- the chunk is redone exactly with a new reference (s_update).  The pair
 // (m, z) is a valid softmax partial for ANY finite m: merge_row never assumes that m is the true maximum.
 __device__ __forceinline__ void s_lazy32(const uint32_t (&v)[32], float sc, float& m, float& z) {
@@ -415,11 +415,11 @@ __device__ __forceinline__ void s_lazy32(const uint32_t (&v)[32], float sc, floa
   float s0, s1;
   unpack2(add2(a0, a1), s0, s1);
   const float zn = z + (s0 + s1);
-  if (zn < 0x1p100f) {  // false for inf and NaN as well
+  if (zn < 0x1p99f) {  // false for inf and NaN as well (the FMA-pipe exp2 saturates just below 2^100)
     z = zn;
   } else {
     s_update(v, sc, m, z);
-    if (!(z < 0x1p100f)) { m += 90.f; z *= 0x1p-90f; }  // many terms just below the limit: move the reference, not the value
+    if (!(z < 0x1p99f)) { m += 90.f; z *= 0x1p-90f; }  // many terms just below the limit: move the reference, not the value
   }
 }
 
@@ -769,7 +769,9 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
     // quad scheme: half and tile parity of this warp's half-buffer; the proxy row it owns in sweep S
     const int q_half = cq & 1, q_par = cq >> 1;
     const int q_row = q_half * 128 + quarter * 32 + lane;
-    const bool q_live = q_half * 128 + quarter * 32 < p.rows;
+    // G*P > 256 off the 256 grid: the last row block is partial.  Its MMA still runs 256 rows wide (the rows past the
+    // head's G*P come from the next head or are zero-filled by the TMA: finite, and ignored below)
+    auto rows_in_block = [&](int rb) { return min(p.rows, p.rows_total - rb * 256); };
     uint32_t ecount = 0;  // tiles seen so far, same sequence as the MMA warp's tcount
     int nseg = 0;
     Walk walk(p);
@@ -791,7 +793,10 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
             const bool ctile = p.causal && (sg.tile + i) * TILE + TILE - 1 > p.L - p.P;
             const uint32_t ta = tbase + q_par * BUF_COLS + q_half * 128;
             const uint32_t ebar = tm_empty(q_par, q_half);
-            TRW(1, if (q_live && !ctile && valid >= TILE) {
+            // warp-uniform (the TMEM loads are warp-wide): does this warp own a live proxy row of this row block?  Threads
+            // past the last row compute on garbage and never store their statistics.
+            const bool row_ok = q_half * 128 + quarter * 32 < rows_in_block(sg.rb);
+            TRW(1, if (row_ok && !ctile && valid >= TILE) {
               uint32_t va[32], vb[32];
               tmem_ld32(ta, va);
               tmem_ld32(ta + 32, vb);
@@ -807,7 +812,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
               s_lazy32(va, sc, m0, z0);
               s_lazy32(vb, sc, m0, z0);
             } else {
-              if (q_live) {
+              if (row_ok) {
                 if (ctile) s_cols_masked(ta, TILE, sc, valid, min(valid, valid - p.P + 1 + (sg.rb * 256 + q_row) % p.P), m0, z0);
                 else s_cols_masked(ta, TILE, sc, valid, valid, m0, z0);
               }
@@ -816,7 +821,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
             TL(2)
             TL_NEXT()
           }
-          if (q_row < p.rows)
+          if (q_row < rows_in_block(sg.rb))
             __stcg(&p.part[(((size_t)blockIdx.x + sg.head) * p.n_slots + q_par) * p.rows_total + sg.rb * 256 + q_row], make_float2(m0, z0));
           ecount += sg.n;
           ++nseg;
@@ -851,7 +856,10 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
         float* nl = nlse_s + ls * 512;
         TRW(2, {
           const int r = threadIdx.x;
-          if (r < p.rows) {
+          if (r < p.rows && r >= rows_in_block(sg.rb)) {
+            nl[r] = -INFINITY;  // a row past the head's G*P: exp2(s - inf) = 0 on both exponential paths
+            nl[kNY + r] = -INFINITY;
+          } else if (r < p.rows) {
             float l2;
             if (p.lse_in) {
               l2 = p.lse_in[(size_t)sg.head * p.rows_total + sg.rb * 256 + r] * 1.4426950408889634f;  // given (natural log) -> log2 domain
@@ -1013,7 +1021,7 @@ cudaError_t launch_cfg(const CUtensorMap& tmK, const CUtensorMap& tmQ, TcParams 
 
 bool score_tc_supported(const Shape& s) {
   return s.dtype == NACL_DTYPE_BF16 && s.d == HD && s.rows % 16 == 0 && s.rows >= 16 &&
-         (s.rows <= 256 || (s.rows % 256 == 0 && s.rows <= 8192));  // larger G*P: blocks of 256 proxy rows
+         s.rows <= 8192;  // G*P > 256: blocks of 256 proxy rows, the last one masked where G*P is off that grid
 }
 
 int score_tc_launch_count(const Shape&) { return 2; }

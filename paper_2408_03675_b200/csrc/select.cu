@@ -577,24 +577,53 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
   const int n_vec = min(tot, C - base) * vpr;
   // K/V and the outputs have their own strides (in 16-byte vectors); a row's vpr vectors are contiguous
   const size_t src0 = (size_t)(b * ly.sb + hk * ly.sh), dst0 = (size_t)(b * ly.ob + hk * ly.oh + (long long)base * ly.orow);
+  const long long dpad = ly.orow - vpr;  // 0 for contiguous output rows: then the output vector index is just v
+  if (dpad == 0) {
+    // four vectors of K and four of V in flight per thread
+    for (int v0 = threadIdx.x; v0 < n_vec; v0 += ST * 4) {
+      size_t src[4];
+      int4 a[4], b4[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int v = v0 + u * ST;
+        if (v < n_vec) {
+          const int row = v / vpr;
+          src[u] = src0 + (size_t)ib[row] * ly.sr + (v - row * vpr);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (v0 + u * ST < n_vec) { a[u] = __ldcs(Kv + src[u]); b4[u] = __ldcs(Vv + src[u]); }
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (v0 + u * ST < n_vec) { __stcs(oKv + dst0 + v0 + u * ST, a[u]); __stcs(oVv + dst0 + v0 + u * ST, b4[u]); }
+    }
+    return;
+  }
+  // output rows with a stride of their own (a cache with spare capacity, a token-major destination): K, then V
   for (int v0 = threadIdx.x; v0 < n_vec; v0 += ST * 4) {
     size_t src[4], dst[4];
-    int4 a[4], b4[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const int v = v0 + u * ST;
       if (v < n_vec) {
         const int row = v / vpr;
         src[u] = src0 + (size_t)ib[row] * ly.sr + (v - row * vpr);
-        dst[u] = dst0 + (size_t)row * ly.orow + (v - row * vpr);
+        dst[u] = dst0 + (size_t)v + (size_t)(row * dpad);
       }
     }
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
-      if (v0 + u * ST < n_vec) { a[u] = __ldcs(Kv + src[u]); b4[u] = __ldcs(Vv + src[u]); }
+    for (int t = 0; t < 2; ++t) {
+      const int4* __restrict__ in = t ? Vv : Kv;
+      int4* __restrict__ out = t ? oVv : oKv;
+      int4 a[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
-      if (v0 + u * ST < n_vec) { __stcs(oKv + dst[u], a[u]); __stcs(oVv + dst[u], b4[u]); }
+      for (int u = 0; u < 4; ++u)
+        if (v0 + u * ST < n_vec) a[u] = __ldcs(in + src[u]);
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (v0 + u * ST < n_vec) __stcs(out + dst[u], a[u]);
+    }
   }
 }
 

@@ -60,6 +60,8 @@ RAGGED = [
     (1, 5000, 16, 16, 128, 48, "bf16", 750, 250, 4, 48),  # G*P = 48
     (1, 1500, 8, 2, 128, 128, "bf16", 300, 75, 4, 128),   # G*P = 512: two 256-row blocks on the tensor-core path
     (2, 900, 6, 2, 128, 256, "bf16", 300, 45, 4, 256),    # G*P = 768: three row blocks, P = 256 proxy rows
+    (1, 1200, 8, 2, 128, 100, "bf16", 300, 60, 4, 100),   # G*P = 400 = 256 + 144: the last row block is partial (masked)
+    (2, 700, 4, 1, 128, 68, "bf16", 200, 30, 4, 68),      # G*P = 272 = 256 + 16
 ]
 
 
@@ -202,8 +204,8 @@ def test_gumbel_keys_bitwise_against_the_oracle(binding, flag_name):
 
 
 @pytest.mark.parametrize("case", [(1, 4100, 32, 8, 128, 64, "bf16"), (2, 1500, 8, 4, 128, 16, "bf16"), (2, 700, 4, 2, 64, 5, "f32"),
-                                  (1, 1100, 8, 2, 128, 128, "bf16")],
-                         ids=["tc_GP256", "tc_GP32", "cuda_core_f32", "tc_GP512_row_blocks"])
+                                  (1, 1100, 8, 2, 128, 128, "bf16"), (1, 1000, 8, 2, 128, 100, "bf16")],
+                         ids=["tc_GP256", "tc_GP32", "cuda_core_f32", "tc_GP512_row_blocks", "tc_GP400_partial_row_block"])
 def test_lse_in_single_sweep(binding, case):
     """SURVEY.md 8(f) f1 / the contract of the paper's Algorithm 2: with the row log-sum-exps
     supplied, one logit sweep gives the same importance (north-star tolerance) and, on it, exactly the oracle's selection."""
@@ -230,8 +232,10 @@ def test_lse_in_single_sweep(binding, case):
 
 
 @pytest.mark.parametrize("case", [(1, 4100, 32, 8, 128, 64, "bf16"), (2, 1000, 8, 2, 128, 48, "bf16"), (1, 300, 4, 4, 128, 16, "bf16"),
-                                  (2, 333, 4, 2, 64, 5, "f32"), (1, 130, 6, 2, 32, 130, "bf16"), (1, 1300, 8, 2, 128, 128, "bf16")],
-                         ids=["tc_GP256_ragged", "tc_GP192", "tc_GP16", "cuda_core_f32", "all_rows_proxy", "tc_GP512_row_blocks"])
+                                  (2, 333, 4, 2, 64, 5, "f32"), (1, 130, 6, 2, 32, 130, "bf16"), (1, 1300, 8, 2, 128, 128, "bf16"),
+                                  (1, 1100, 8, 2, 128, 100, "bf16")],
+                         ids=["tc_GP256_ragged", "tc_GP192", "tc_GP16", "cuda_core_f32", "all_rows_proxy", "tc_GP512_row_blocks",
+                              "tc_GP400_partial_row_block"])
 def test_causal_flag(binding, case):
     """NACL_FLAG_CAUSAL (R1): proxy row i is prompt position L-P+i and attends keys j <= L-P+i only.  The last
     case makes every prompt row a proxy row: accumulated causal attention (the H2O one-shot case)."""

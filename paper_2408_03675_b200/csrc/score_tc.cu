@@ -344,18 +344,19 @@ struct Walk {
 __device__ __forceinline__ int cta_of_tile(long long t, long long N, long long G) { return (int)(((t + 1) * G + N - 1) / N - 1); }
 
 // ------------------------------------------------------------------ shared-memory carve-up
-constexpr int LSE_SLOTS = 2;
-// PH = the sweep the instantiation serves: sweep S needs neither the lse nor the column-sum buffers and spends the
-// space on one more K stage
+// PH = the sweep the instantiation serves.  Sweep C carries two more operand boxes for the NINTH k-step of its MMAs (see
+// "augmented contraction" at the kernel): QA = per proxy row the constant -lse/scale as three bf16 terms, KA = ones.
 template <int QROWS, int NQ, int STAGES, int PH>
 struct Smem {
   static constexpr int Q_BYTES = QROWS * HD * 2;
+  static constexpr int QA_BYTES = QROWS * 128;  // one 128-byte (swizzled) row per proxy row; the first 32 bytes are used
   static constexpr int OFF_Q = 0;
   static constexpr int OFF_K = OFF_Q + NQ * Q_BYTES;
-  static constexpr int OFF_LSE = OFF_K + STAGES * KSTAGE_BYTES;   // float[LSE_SLOTS][2][256]: -lse (log2 domain) of the segment's head, and (110 - lse) / 227
-  static constexpr int OFF_CS = OFF_LSE + (PH ? LSE_SLOTS * 512 * 4 : 0);    // float[N_CS][4][128]: quarter column sums of a C tile
+  static constexpr int OFF_QA = OFF_K + STAGES * KSTAGE_BYTES;
+  static constexpr int OFF_KA = OFF_QA + (PH ? NQ * QA_BYTES : 0);
+  static constexpr int OFF_CS = OFF_KA + (PH ? BOX_BYTES : 0);     // float[N_CS][4][128]: quarter column sums of a C tile
   static constexpr int OFF_BARS = OFF_CS + (PH ? N_CS * 4 * TILE * 4 : 0);
-  static constexpr int N_BARS = 2 * STAGES + 2 * NQ + 4 * N_BUFS + 2 * N_CS;
+  static constexpr int N_BARS = 2 * STAGES + 4 * NQ + 4 * N_BUFS + 2 * N_CS;
   static constexpr int OFF_TMEM = OFF_BARS + N_BARS * 8;
   static constexpr int TOTAL = OFF_TMEM + 8;
 };
@@ -460,13 +461,12 @@ __device__ __forceinline__ void s_cols_masked(uint32_t taddr, int nc, float sc, 
   }
 }
 
-// N4 groups of 4 columns (proxy rows) of a C tile: acc += 2^(s*sc - lse2[row]); nl = -lse2 of those rows and, kNY floats
-// further on, (110 - lse2) / 227 of the same rows (the constant of the FMA-pipe path)
-constexpr int kNY = 256;
+// N4 groups of 4 columns (proxy rows) of a C tile: acc += 2^(v*sc), v = the accumulator, which already holds
+// s - lse/scale (augmented contraction): no per-row constant, no shared-memory traffic in the epilogue
 template <int N4>
-__device__ __forceinline__ void c_update(const uint32_t (&v)[32], float sc, const float* nl, u64& a0, u64& a1) {
-  const u64 sc2 = pack2(sc, sc);
-  const float scy = sc * (1.f / kPolySpan);
+__device__ __forceinline__ void c_update(const uint32_t (&v)[32], float sc, u64& a0, u64& a1) {
+  const u64 sc2 = pack2(sc, sc), zero2 = 0ull;
+  const float scy = sc * (1.f / kPolySpan), cy = kPolyLo * (1.f / kPolySpan);
 #ifdef NACL_EPI_TRIVIAL
 #pragma unroll
   for (int e = 0; e < N4; ++e) {
@@ -477,39 +477,31 @@ __device__ __forceinline__ void c_update(const uint32_t (&v)[32], float sc, cons
 #endif
 #pragma unroll
   for (int e = 0; e < N4; ++e) {
-    if (pair_on_fma_pipe<NACL_POLY_MASK_C>(2 * e)) {
-      const float2 c = *reinterpret_cast<const float2*>(nl + kNY + 4 * e);
-      a0 = acc_exp2_poly_sat(a0, v[4 * e + 0], v[4 * e + 1], scy, c.x, c.y);
-    } else {
-      a0 = add2(a0, exp2_mufu2(fma2(pack2u(v[4 * e + 0], v[4 * e + 1]), sc2, *reinterpret_cast<const u64*>(nl + 4 * e))));
-    }
-    if (pair_on_fma_pipe<NACL_POLY_MASK_C>(2 * e + 1)) {
-      const float2 c = *reinterpret_cast<const float2*>(nl + kNY + 4 * e + 2);
-      a1 = acc_exp2_poly_sat(a1, v[4 * e + 2], v[4 * e + 3], scy, c.x, c.y);
-    } else {
-      a1 = add2(a1, exp2_mufu2(fma2(pack2u(v[4 * e + 2], v[4 * e + 3]), sc2, *reinterpret_cast<const u64*>(nl + 4 * e + 2))));
-    }
+    if (pair_on_fma_pipe<NACL_POLY_MASK_C>(2 * e)) a0 = acc_exp2_poly_sat(a0, v[4 * e + 0], v[4 * e + 1], scy, cy, cy);
+    else a0 = add2(a0, exp2_mufu2(fma2(pack2u(v[4 * e + 0], v[4 * e + 1]), sc2, zero2)));
+    if (pair_on_fma_pipe<NACL_POLY_MASK_C>(2 * e + 1)) a1 = acc_exp2_poly_sat(a1, v[4 * e + 2], v[4 * e + 3], scy, cy, cy);
+    else a1 = add2(a1, exp2_mufu2(fma2(pack2u(v[4 * e + 2], v[4 * e + 3]), sc2, zero2)));
   }
 }
 
 // C tile, this warp's share: the key this thread owns, summed over nc proxy rows (TMEM columns from taddr on;
-// nc a multiple of 4, <= 64) of exp2(s*sc - lse2[row]); nl = -lse2 of those rows
-__device__ __forceinline__ float c_cols(uint32_t taddr, int nc, float sc, const float* nl) {
+// nc a multiple of 4, <= 64) of exp2(v*sc)
+__device__ __forceinline__ float c_cols(uint32_t taddr, int nc, float sc) {
   u64 a0 = 0ull, a1 = 0ull;
   uint32_t va[32], vb[32];
   if (nc == 64) {
     tmem_ld32(taddr, va);
     tmem_ld32(taddr + 32, vb);
     tc_wait_ld(va);
-    c_update<8>(va, sc, nl, a0, a1);
+    c_update<8>(va, sc, a0, a1);
     tc_wait_ld(vb);
-    c_update<8>(vb, sc, nl + 32, a0, a1);
+    c_update<8>(vb, sc, a0, a1);
   } else {
     int c = 0;
-    if (nc & 32) { tmem_ld32(taddr, va); tc_wait_ld(va); c_update<8>(va, sc, nl, a0, a1); c = 32; }
-    if (nc & 16) { tmem_ld16(taddr + c, va); tc_wait_ld(va); c_update<4>(va, sc, nl + c, a0, a1); c += 16; }
-    if (nc & 8) { tmem_ld8(taddr + c, va); tc_wait_ld(va); c_update<2>(va, sc, nl + c, a0, a1); c += 8; }
-    if (nc & 4) { tmem_ld4(taddr + c, va); tc_wait_ld(va); c_update<1>(va, sc, nl + c, a0, a1); }
+    if (nc & 32) { tmem_ld32(taddr, va); tc_wait_ld(va); c_update<8>(va, sc, a0, a1); c = 32; }
+    if (nc & 16) { tmem_ld16(taddr + c, va); tc_wait_ld(va); c_update<4>(va, sc, a0, a1); c += 16; }
+    if (nc & 8) { tmem_ld8(taddr + c, va); tc_wait_ld(va); c_update<2>(va, sc, a0, a1); c += 8; }
+    if (nc & 4) { tmem_ld4(taddr + c, va); tc_wait_ld(va); c_update<1>(va, sc, a0, a1); }
   }
   float s0, s1;
   unpack2(add2(a0, a1), s0, s1);
@@ -518,7 +510,7 @@ __device__ __forceinline__ float c_cols(uint32_t taddr, int nc, float sc, const 
 
 // C tile under NACL_FLAG_CAUSAL (only the tiles that hold the last P keys): proxy rows r with r % P < imin do not see
 // this thread's key and contribute nothing
-__device__ __noinline__ float c_cols_causal(uint32_t taddr, int nc, float sc, const float* nl, int row0, int P, int imin) {
+__device__ __noinline__ float c_cols_causal(uint32_t taddr, int nc, float sc, int row0, int P, int imin) {
   float acc = 0.f;
   uint32_t v[32];
 #pragma unroll 1
@@ -527,7 +519,7 @@ __device__ __noinline__ float c_cols_causal(uint32_t taddr, int nc, float sc, co
     tc_wait_ld(v);
 #pragma unroll
     for (int e = 0; e < 4; ++e)
-      if ((row0 + c + e) % P >= imin) acc += fast_exp2(fmaf(__uint_as_float(v[e]), sc, nl[c + e]));
+      if ((row0 + c + e) % P >= imin) acc += fast_exp2(__uint_as_float(v[e]) * sc);
   }
   return acc;
 }
@@ -542,9 +534,11 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
   if ((sbase & 1023u) != 0) __trap();  // the 128B-swizzled operand tiles need 1024-byte alignment
 
   const uint32_t bars = sbase + SM::OFF_BARS;
-  constexpr int B_KE = STAGES, B_QF = 2 * STAGES, B_QE = B_QF + NQ, B_TF = B_QE + NQ, B_TE = B_TF + 2 * N_BUFS, B_CF = B_TE + 2 * N_BUFS,
-                B_CE = B_CF + N_CS;
+  constexpr int B_KE = STAGES, B_QF = 2 * STAGES, B_QE = B_QF + NQ, B_AF = B_QE + NQ, B_AE = B_AF + NQ, B_TF = B_AE + NQ,
+                B_TE = B_TF + 2 * N_BUFS, B_CF = B_TE + 2 * N_BUFS, B_CE = B_CF + N_CS;
   static_assert(B_CE + N_CS == SM::N_BARS, "barrier count");
+  auto qa_full = [&](int s) { return bars + 8u * (B_AF + s); };   // sweep C: the segment's -lse/scale rows are in shared memory
+  auto qa_empty = [&](int s) { return bars + 8u * (B_AE + s); };  // ... and every MMA that read them has completed
   auto k_full = [&](int s) { return bars + 8u * s; };
   auto k_empty = [&](int s) { return bars + 8u * (B_KE + s); };
   auto q_full = [&](int s) { return bars + 8u * (B_QF + s); };
@@ -556,7 +550,6 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
   auto cs_full = [&](int b) { return bars + 8u * (B_CF + b); };
   auto cs_empty = [&](int b) { return bars + 8u * (B_CE + b); };
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + SM::OFF_TMEM);
-  float* nlse_s = reinterpret_cast<float*>(smem + SM::OFF_LSE);
   float* cs_s = reinterpret_cast<float*>(smem + SM::OFF_CS);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -576,7 +569,10 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
-    for (int s = 0; s < NQ; ++s) { mbar_init(q_full(s), 1); mbar_init(q_empty(s), 2); }  // q_empty: one arrival per MMA issuer
+    for (int s = 0; s < NQ; ++s) {
+      mbar_init(q_full(s), 1); mbar_init(q_empty(s), 2);  // q_empty, qa_empty: one arrival per MMA issuer
+      mbar_init(qa_full(s), 1); mbar_init(qa_empty(s), 2);
+    }
     for (int b = 0; b < N_BUFS; ++b)
       for (int h = 0; h < 2; ++h) {
         mbar_init(tm_full(b, h), 1);
@@ -584,6 +580,17 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
       }
     for (int b = 0; b < N_CS; ++b) { mbar_init(cs_full(b), quad ? N_EPI_WARPS / 2 : N_EPI_WARPS); mbar_init(cs_empty(b), 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if constexpr (PH != 0) {
+    // KA: 128 key rows x 128 bytes in the operand layout (K-major, 128-byte swizzle: 16-byte chunk c of row r sits at chunk
+    // c ^ (r & 7)); the k-step reads chunks 0 and 1 = 16 bf16 per row: {1, 1, 1, 0, ...}
+    if (threadIdx.x < TILE) {
+      const int r = threadIdx.x;
+      uint4* row = reinterpret_cast<uint4*>(smem + SM::OFF_KA + r * 128);
+      row[0 ^ (r & 7)] = make_uint4(0x3F803F80u, 0x00003F80u, 0u, 0u);
+      row[1 ^ (r & 7)] = make_uint4(0u, 0u, 0u, 0u);
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the MMA's async proxy
   }
   if (warp == W_MMA) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(sbase + SM::OFF_TMEM), "r"(TMEM_COLS) : "memory");
@@ -641,17 +648,30 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
     while (walk.next(sg)) {
       const int qb = qrun % NQ;
       TRW(2, mbar_wait(q_full(qb), (qrun / NQ) & 1));
+      if constexpr (PH != 0) {
+        TRW(2, mbar_wait(qa_full(qb), (qrun / NQ) & 1));
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      }
       const uint32_t qsrc = sbase + SM::OFF_Q + qb * SM::Q_BYTES;
+      const uint32_t qasrc = sbase + SM::OFF_QA + qb * SM::QA_BYTES, kasrc = sbase + SM::OFF_KA;
       ++qrun;
       if (sg.n == 1 && (tcount & 1) != mine) {
-        // no tile of this segment is this issuer's: it still owes its arrival on q_empty
-        if (leader) mbar_arrive(q_empty(qb));
+        // no tile of this segment is this issuer's: it still owes its arrival on q_empty (and qa_empty)
+        if (leader) {
+          mbar_arrive(q_empty(qb));
+          if constexpr (PH != 0) mbar_arrive(qa_empty(qb));
+        }
         __syncwarp();
       }
       for (int i = 0; i < sg.n; ++i) {
         const uint32_t buf = tcount & 1, par = (tcount >> 1) & 1;
         if (buf == mine) {
           TL(0)
+          // An issuer sees only every other use of a stage when the ring length is odd, and a parity wait cannot tell
+          // "this use has landed" from "the use before it has not even landed yet".  The consumer of the previous use (the
+          // other issuer) commits k_empty only after that use's MMAs, so once k_empty has completed for it, k_full can
+          // only be in the phase this tile needs.
+          TRW(0, mbar_wait(k_empty(stage), kphase ^ 1));
           TRW(0, mbar_wait(k_full(stage), kphase));
           TL(1)
           const uint32_t ksrc = sbase + SM::OFF_K + stage * KSTAGE_BYTES;
@@ -671,6 +691,8 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
                   if constexpr (PH == 0) tc_mma(dcol + h * 128, umma_desc(qsrc + qo), umma_desc(ksrc + ko), idesc_q, k > 0);
                   else tc_mma(dcol + h * 128, umma_desc(ksrc + ko), umma_desc(qsrc + qo), idesc_q, k > 0);
                 }
+                // ninth k-step (sweep C): + ones x (-lse/scale) -- the row constant of the softmax goes in with the logits
+                if constexpr (PH != 0) tc_mma(dcol + h * 128, umma_desc(kasrc), umma_desc(qasrc + h * BOX_BYTES), idesc_q, 1);
                 tc_commit(tm_full(buf, h));
               }
               __syncwarp();
@@ -678,7 +700,10 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
             TL(2)
             if (leader) {
               tc_commit(k_empty(stage));
-              if (i + 2 >= sg.n) tc_commit(q_empty(qb));
+              if (i + 2 >= sg.n) {
+                tc_commit(q_empty(qb));
+                if constexpr (PH != 0) tc_commit(qa_empty(qb));
+              }
             }
           } else {
           TRW(1, mbar_wait(tm_empty(buf, 0), par ^ 1));
@@ -702,10 +727,14 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
                 const uint32_t qo = (k >> 2) * (QROWS * 128) + (k & 3) * 32;
                 tc_mma(dcol, umma_desc(ksrc + ko), umma_desc(qsrc + qo), idesc, k > 0);
               }
+              tc_mma(dcol, umma_desc(kasrc), umma_desc(qasrc), idesc, 1);  // ninth k-step: the row constants
             }
             tc_commit(tm_full(buf, 0));   // the accumulator buffer is complete
             tc_commit(k_empty(stage));    // the reads of the stage are done once these MMAs complete
-            if (i + 2 >= sg.n) tc_commit(q_empty(qb));  // this issuer's last tile of the segment: its reads of Q are done
+            if (i + 2 >= sg.n) {          // this issuer's last tile of the segment: its reads of Q are done
+              tc_commit(q_empty(qb));
+              if constexpr (PH != 0) tc_commit(qa_empty(qb));
+            }
           }
           }
           __syncwarp();
@@ -851,35 +880,52 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
         if (s_row < p.rows)
           __stcg(&p.part[(((size_t)blockIdx.x + sg.head) * p.n_slots + s_slot) * p.rows_total + sg.rb * 256 + s_row], make_float2(m0, z0));
       } else {
-        // ---------------- C segment: merge the head's partials (ascending piece order) into -lse, then column sums
-        const int ls = nseg % LSE_SLOTS;
-        float* nl = nlse_s + ls * 512;
+        // ---------------- C segment: merge the head's partials (ascending piece order) into lse, hand -lse/scale to the MMA
+        // issuers as the operand of the ninth k-step (augmented contraction: the accumulator then holds s - lse/scale and
+        // the epilogue needs no per-row constant -- in this orientation a thread meets all G*P rows, and fetching their
+        // constants from shared memory cost 10 us per sweep at cfg 4), then column sums
+        const int qs = nseg % NQ;
         TRW(2, {
+          mbar_wait(qa_empty(qs), ((nseg / NQ) & 1) ^ 1);  // the MMAs of the segment that used this slot before are done
           const int r = threadIdx.x;
-          if (r < p.rows && r >= rows_in_block(sg.rb)) {
-            nl[r] = -INFINITY;  // a row past the head's G*P: exp2(s - inf) = 0 on both exponential paths
-            nl[kNY + r] = -INFINITY;
-          } else if (r < p.rows) {
-            float l2;
-            if (p.lse_in) {
-              l2 = p.lse_in[(size_t)sg.head * p.rows_total + sg.rb * 256 + r] * 1.4426950408889634f;  // given (natural log) -> log2 domain
+          if (r < p.rows) {
+            float cf;
+            if (r >= rows_in_block(sg.rb)) {
+              cf = -INFINITY;  // a row past the head's G*P: 2^(-inf) = 0 on both exponential paths
             } else {
-              const int c_first = cta_of_tile((long long)sg.head * p.T, p.N, G);
-              const int c_last = cta_of_tile((long long)(sg.head + 1) * p.T - 1, p.N, G);
-              l2 = merge_row(p.part + ((size_t)(c_first + sg.head) * p.n_slots) * p.rows_total + sg.rb * 256 + r,
-                             (c_last - c_first + 1) * p.n_slots, (size_t)p.rows_total);
+              float l2;
+              if (p.lse_in) {
+                l2 = p.lse_in[(size_t)sg.head * p.rows_total + sg.rb * 256 + r] * 1.4426950408889634f;  // given (natural log) -> log2 domain
+              } else {
+                const int c_first = cta_of_tile((long long)sg.head * p.T, p.N, G);
+                const int c_last = cta_of_tile((long long)(sg.head + 1) * p.T - 1, p.N, G);
+                l2 = merge_row(p.part + ((size_t)(c_first + sg.head) * p.n_slots) * p.rows_total + sg.rb * 256 + r,
+                               (c_last - c_first + 1) * p.n_slots, (size_t)p.rows_total);
+              }
+              // the CTA that owns the head's first tile publishes lse
+              if (p.lse_out && sg.tile - (sg.n - 1) == 0) p.lse_out[(size_t)sg.head * p.rows_total + sg.rb * 256 + r] = l2 * 0.69314718055994530942f;
+              cf = -l2 / sc;  // in units of the raw dot product
             }
-            nl[r] = -l2;
-            nl[kNY + r] = (kPolyLo - l2) * (1.f / kPolySpan);
-            // the CTA that owns the head's first tile publishes lse
-            if (p.lse_out && sg.tile - (sg.n - 1) == 0) p.lse_out[(size_t)sg.head * p.rows_total + sg.rb * 256 + r] = l2 * 0.69314718055994530942f;
+            // three bf16 terms carry cf to 2^-24 relative (the products with 1.0 are exact, the MMA sums them in fp32)
+            const __nv_bfloat16 hi = __float2bfloat16_rn(cf);
+            const bool fin = cf > -INFINITY;
+            const float r1 = fin ? cf - __bfloat162float(hi) : 0.f;
+            const __nv_bfloat16 mid = __float2bfloat16_rn(r1);
+            const __nv_bfloat16 lo = __float2bfloat16_rn(r1 - __bfloat162float(mid));
+            uint4* row = reinterpret_cast<uint4*>(smem + SM::OFF_QA + qs * SM::QA_BYTES + r * 128);
+            row[0 ^ (r & 7)] = make_uint4((uint32_t)__bfloat16_as_ushort(hi) | ((uint32_t)__bfloat16_as_ushort(mid) << 16),
+                                          (uint32_t)__bfloat16_as_ushort(lo), 0u, 0u);
+            row[1 ^ (r & 7)] = make_uint4(0u, 0u, 0u, 0u);
           }
+          // writers' generic-proxy stores -> async proxy (the MMA reads shared memory through it), then the epilogue
+          // warps meet at a named barrier and ONE thread tells the issuers
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory");
+          if (threadIdx.x == 0) mbar_arrive(qa_full(qs));
         })
-        TRW(3, asm volatile("bar.sync 1, %0;" ::"n"(EPI_THREADS) : "memory"));
         if (quad) {
           // this warp: the 32 keys of its lane quarter (one per thread) summed over the 128 proxy rows of half q_half, for
           // the tiles of parity q_par; the combiner adds the two halves of a key
-          const float* nlh = nl + q_half * 128;
           for (int i = 0; i < sg.n; ++i) {
             const uint32_t g = ecount + i;
             if ((int)(g & 1) != q_par) continue;
@@ -893,7 +939,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
             float r;
             if (p.causal && (sg.tile - i) * TILE + TILE - 1 > p.L - p.P) {
               const int jkey = (sg.tile - i) * TILE + quarter * 32 + lane;  // the key this thread owns
-              r = c_cols_causal(ta, 128, sc, nlh, sg.rb * 256 + q_half * 128, p.P, jkey - (p.L - p.P));
+              r = c_cols_causal(ta, 128, sc, sg.rb * 256 + q_half * 128, p.P, jkey - (p.L - p.P));
               release_tmem(ebar);
             } else {
               TRW(1, {
@@ -902,16 +948,16 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
                 tmem_ld32(ta, va);
                 tmem_ld32(ta + 32, vb);
                 tc_wait_ld(va);
-                c_update<8>(va, sc, nlh, a0, a1);
+                c_update<8>(va, sc, a0, a1);
                 tc_wait_ld(vb);
-                c_update<8>(vb, sc, nlh + 32, a0, a1);
+                c_update<8>(vb, sc, a0, a1);
                 tmem_ld32(ta + 64, va);
                 tmem_ld32(ta + 96, vb);
                 tc_wait_ld(va);
                 tc_wait_ld(vb);
                 release_tmem(ebar);
-                c_update<8>(va, sc, nlh + 64, a0, a1);
-                c_update<8>(vb, sc, nlh + 96, a0, a1);
+                c_update<8>(va, sc, a0, a1);
+                c_update<8>(vb, sc, a0, a1);
                 float s0, s1;
                 unpack2(add2(a0, a1), s0, s1);
                 r = s0 + s1;
@@ -937,9 +983,9 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
           float r;
           const int jkey = (sg.tile - i) * TILE + quarter * 32 + lane;  // the key this thread owns
           if (p.causal && (sg.tile - i) * TILE + TILE - 1 > p.L - p.P)
-            r = c_cols_causal(tbase + buf * BUF_COLS + c_col0, c_nc, sc, nl + c_col0, sg.rb * 256 + c_col0, p.P, jkey - (p.L - p.P));
+            r = c_cols_causal(tbase + buf * BUF_COLS + c_col0, c_nc, sc, sg.rb * 256 + c_col0, p.P, jkey - (p.L - p.P));
           else
-            TRW(1, r = c_cols(tbase + buf * BUF_COLS + c_col0, c_nc, sc, nl + c_col0));
+            TRW(1, r = c_cols(tbase + buf * BUF_COLS + c_col0, c_nc, sc));
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(tm_empty(buf, 0));
@@ -1067,8 +1113,8 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
   p.scale_log2 = 1.4426950408889634f / sqrtf((float)s.d);
   p.part = ws.part; p.lse_in = lse_in; p.lse_out = lse_out; p.imp = ws.imp; p.imp_out = imp_out;
 
-  if (qrows == 128) return launch_cfg<128, 2, 5, 4>(tmK, tmQ, p, st);
-  return launch_cfg<256, 1, 5, 4>(tmK, tmQ, p, st);
+  if (qrows == 128) return launch_cfg<128, 2, 5, 3>(tmK, tmQ, p, st);
+  return launch_cfg<256, 1, 5, 3>(tmK, tmQ, p, st);
 }
 
 }  // namespace nacl

@@ -60,12 +60,12 @@ constexpr int N_CS = 4;                        // shared-memory buffers for the 
 constexpr int MAX_GRID = kNumSMs;              // the partial-statistics workspace is sized for this many CTAs
 constexpr uint32_t SPIN_LIMIT = 1u << 26;      // watchdog: a wait that long is a bug -> trap (loud failure)
 // which of every 8 element pairs take the FMA-pipe exp2 instead of MUFU.EX2 (bit e&7), per sweep: measured optimum on
-// B200 (cfg 4, us per layer): sweep S 74.8 / 71.9 / 75.3 and sweep C 82.0 / 82.4 / 86.6 for 2/8, 3/8, 4/8
+// B200 (cfg 4, us per layer): sweep S 74.8 / 71.9 / 75.3 for 2/8, 3/8, 4/8; sweep C 78.2 / 76.2 for 2/8, 3/8
 #ifndef NACL_POLY_MASK_S
 #define NACL_POLY_MASK_S 0x2Au
 #endif
 #ifndef NACL_POLY_MASK_C
-#define NACL_POLY_MASK_C 0x22u
+#define NACL_POLY_MASK_C 0x2Au
 #endif
 
 // Optional wait/compute cycle accounting per warp role (diagnostics build only: -DNACL_TC_TRACE).

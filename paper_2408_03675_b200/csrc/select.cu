@@ -30,8 +30,8 @@ __device__ __forceinline__ uint32_t philox4x32_10_word0(uint32_t c0, uint32_t c1
   constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
 #pragma unroll
   for (int r = 0; r < 10; ++r) {
-    uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
-    uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+    const uint64_t p0 = (uint64_t)M0 * c0, p1 = (uint64_t)M1 * c2;  // one 32x32->64 multiply each (IMAD.WIDE)
+    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0, hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
     c0 = hi1 ^ c1 ^ k0;
     c1 = lo1;
     c2 = hi0 ^ c3 ^ k1;
@@ -58,21 +58,28 @@ __device__ const double kLogTab[92][3] = {
 #include "logtab.inc"
 };
 constexpr double kLn2Hi = 0x1.62e42fefa39efp-1, kLn2Lo = 0x1.abc9e3b39803fp-56;
+// int <-> double without the conversion unit (the sampling keys are issue- and XU-bound): 2^52 + 2^31 + e has e's two's
+// complement in its low word; x + 1.5*2^52 has round-to-nearest-even(x) in its low word.  Both exact.
+__device__ __forceinline__ double small_int_to_double(int e) {
+  return __hiloint2double(0x43300000, (int)(0x80000000u ^ (uint32_t)e)) - 4503601774854144.0;  // 2^52 + 2^31
+}
 __device__ __forceinline__ double log_tab(double x) {
-  const long long bits = __double_as_longlong(x);
-  int e = (int)((bits >> 52) & 0x7FF) - 1023;
-  double m = __longlong_as_double((bits & 0x000FFFFFFFFFFFFFll) | 0x3FF0000000000000ll);  // [1, 2)
+  const int hi = __double2hiint(x);
+  int e = ((hi >> 20) & 0x7FF) - 1023;
+  double m = __hiloint2double((hi & 0x000FFFFF) | 0x3FF00000, __double2loint(x));  // [1, 2)
   if (m > 1.4140625) { m *= 0.5; e += 1; }
-  const int k = __double2int_rn(m * 128.0);  // 90 .. 181
+  const double kt = fma(m, 128.0, 6755399441055744.0);  // 1.5 * 2^52: k = rn(m * 128) = 90 .. 181 in the low word
+  const int k = __double2loint(kt);
+  const double kd = kt - 6755399441055744.0;            // (double)k
   const double* t = kLogTab[k - 90];
-  const double r = (m - (double)k * 0.0078125) * __ldg(&t[0]);
+  const double r = (m - kd * 0.0078125) * __ldg(&t[0]);
   double q = fma(r, 1.0 / 7.0, -1.0 / 6.0);
   q = fma(q, r, 0.2);
   q = fma(q, r, -0.25);
   q = fma(q, r, 1.0 / 3.0);
   q = fma(q, r, -0.5);
   q = q * r * r;
-  const double de = (double)e;
+  const double de = small_int_to_double(e);
   return fma(de, kLn2Hi, __ldg(&t[1]) + (r + (q + fma(de, kLn2Lo, __ldg(&t[2])))));
 }
 
@@ -81,7 +88,8 @@ template <bool ORDERMAP = true>
 __device__ __forceinline__ uint32_t gumbel_key(float imp, uint32_t j, uint32_t hk, uint32_t b, uint32_t layer, uint32_t k0, uint32_t k1,
                                                uint32_t flags) {
   const uint32_t x = philox4x32_10_word0(j, hk, b, layer, k0, k1);
-  const double u = ((double)(x >> 9) + 0.5) * 0x1p-23;  // exact; u in [2^-24, 1-2^-24]
+  // u = ((x >> 9) + 0.5) * 2^-23, exact, in [2^-24, 1 - 2^-24]: 2^52 + n has n in its low word; 2^52 - 0.5 is a double
+  const double u = (__hiloint2double(0x43300000, (int)(x >> 9)) - 4503599627370495.5) * 0x1p-23;
   const double w = (double)imp;
   double ln_w;
   if (flags & NACL_FLAG_SAMPLE_UNIFORM) ln_w = 0.0;

@@ -193,7 +193,7 @@ def run_ours(args) -> dict:
     def step():
         for l, (K, V, Q, oK, oV, oi) in enumerate(data):
             binding.nacl_evict_ex(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l,
-                                  out_K=oK, out_V=oV, out_idx=oi, workspace=ws, stream=stream)
+                                  out_K=oK, out_V=oV, out_idx=oi, workspace=ws, stream=stream, flags=args.nacl_flags)
 
     def timed(n_steps: int) -> float:
         nacl_dist.barrier(dev)
@@ -296,7 +296,7 @@ def run_ours(args) -> dict:
         "hbm_frac_of_nominal_8TBps": round(value / world / 8000.0, 4),
         "clocks": clocks, "e2e": e2e,
         "gpu_launches": args.steps * layers * binding.nacl_launch_count(
-            1 if cfg.dtype == "bf16" else 0, cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P),
+            1 if cfg.dtype == "bf16" else 0, cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P, args.nacl_flags),
         "roofline": roofline, "kernels": stage_rows,
         "ms_per_step_with_kernel_events": round(ms_total_prof / args.steps, 4),
         "lse_in_variant": {"what": "nacl_evict_ex with lse_in (row log-sum-exps supplied, single logit sweep; SURVEY.md 8(f) f1)",
@@ -482,6 +482,8 @@ def main() -> int:
     ap.add_argument("--config", type=int, default=4, choices=sorted(CONFIGS))
     ap.add_argument("--layers", type=int, default=0, help="override the number of layers per step (0 = the workload's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--nacl-flags", type=lambda v: int(v, 0), default=0,
+                    help="NACL_FLAG_* bits for the timed calls (profiling: 0x200 = the two scoring sweeps as two launches)")
     ap.add_argument("--no-other-workloads", action="store_true", help="skip the short runs of the other BASELINE.json configs")
     args = ap.parse_args()
     if args.gpus > 1 and "RANK" not in os.environ:

@@ -89,6 +89,8 @@ extern "C" {
                                                 head's out_idx row holds that set and out_K/out_V are gathered with it */
 #define NACL_FLAG_SCORE_CUDA_CORES 0x100u    /* debugging: run the generic CUDA-core scoring kernels even where
                                                 the tensor-core path applies */
+#define NACL_FLAG_SCORE_TWO_LAUNCHES 0x200u  /* debugging / profiling: the tensor-core path runs its statistics sweep and its
+                                                column-sum sweep as two launches instead of one cooperative launch */
 
 typedef struct nacl_params {
   uint32_t struct_size;            /* = sizeof(nacl_params_t) */

@@ -44,6 +44,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc] + NVCC_FLAGS + ["-I", INCLUDE, "-I", CSRC]
+    cmd += os.environ.get("NACL_NVCC_EXTRA", "").split()  # diagnostics builds: -DNACL_TC_TRACE, -DNACL_TC_STAMPS, -DNACL_SEL_TRACE
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += ["-o", LIB + ".tmp"] + sources()

@@ -73,6 +73,8 @@ Workspace carve_workspace(void* base, int batch, int L, int Hq, int Hkv, int P) 
   size_t off = 0;
   char* b = static_cast<char*>(base);
   Workspace ws;
+  // first, so that its place does not depend on the other sizes: evict_impl keeps track of how much of it is known to be zero
+  ws.sync = reinterpret_cast<int*>(b + off);    off = align_up(off + sync_ints((size_t)batch * Hkv) * sizeof(int), 256);
   size_t n_part = n_rows * sp.n_chunks;  // generic path; the tensor-core path keeps one partial per (CTA + head, warpgroup, row)
   const size_t n_part_tc = score_tc_part_elems(batch * Hkv, (Hq / Hkv) * P);
   if (n_part_tc > n_part) n_part = n_part_tc;
@@ -80,7 +82,6 @@ Workspace carve_workspace(void* base, int batch, int L, int Hq, int Hkv, int P) 
   ws.lse = reinterpret_cast<float*>(b + off);   off = align_up(off + n_rows * sizeof(float), 256);
   ws.imp = reinterpret_cast<float*>(b + off);   off = align_up(off + n_imp * sizeof(float), 256);
   ws.key = reinterpret_cast<uint32_t*>(b + off); off = align_up(off + select_scratch_words(batch, Hkv, L) * sizeof(uint32_t), 256);
-  ws.sync = reinterpret_cast<int*>(b + off);    off = align_up(off + sync_ints((size_t)batch * Hkv) * sizeof(int), 256);
   ws.imp_sh = reinterpret_cast<float*>(b + off); off = align_up(off + (size_t)batch * L * sizeof(float), 256);
   ws.idx_sh = reinterpret_cast<int32_t*>(b + off); off = align_up(off + (size_t)batch * L * sizeof(int32_t), 256);
   ws.idx_tmp = reinterpret_cast<int32_t*>(b + off); off = align_up(off + n_imp * sizeof(int32_t), 256);
@@ -114,7 +115,7 @@ static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 // The internal workspace is keyed by (device, stream): calls on one stream are ordered and may share scratch, calls on
 // different streams may run at the same time and must not.  A buffer that is too small is replaced, but the old one
 // is only freed by nacl_release: a call enqueued earlier on the same stream may still be running out of it.
-struct WsEntry { cudaStream_t stream; void* ptr; size_t bytes; };
+struct WsEntry { cudaStream_t stream; void* ptr; size_t bytes; size_t sync_clean; };  // sync_clean: leading bytes known to be zero
 struct DeviceCache {
   std::vector<WsEntry> ws;
   std::vector<void*> retired;
@@ -142,9 +143,10 @@ static cudaError_t grow(void** p, size_t* have, size_t want) {
 }
 
 // g_mu held
-static cudaError_t stream_workspace(DeviceCache& dc, cudaStream_t st, size_t want, void** out) {
+static cudaError_t stream_workspace(DeviceCache& dc, cudaStream_t st, size_t want, void** out, size_t** sync_clean = nullptr) {
   for (WsEntry& w : dc.ws)
     if (w.stream == st) {
+      if (sync_clean) *sync_clean = &w.sync_clean;
       if (w.bytes < want) {
         dc.retired.push_back(w.ptr);
         const size_t cap = want + want / 8 + 256;
@@ -153,6 +155,7 @@ static cudaError_t stream_workspace(DeviceCache& dc, cudaStream_t st, size_t wan
         if (e != cudaSuccess) { dc.retired.pop_back(); return e; }
         w.ptr = np;
         w.bytes = cap;
+        w.sync_clean = 0;
       }
       *out = w.ptr;
       return cudaSuccess;
@@ -161,7 +164,8 @@ static cudaError_t stream_workspace(DeviceCache& dc, cudaStream_t st, size_t wan
   void* np = nullptr;
   cudaError_t e = cudaMalloc(&np, cap);
   if (e != cudaSuccess) return e;
-  dc.ws.push_back(WsEntry{st, np, cap});
+  dc.ws.push_back(WsEntry{st, np, cap, 0});
+  if (sync_clean) *sync_clean = &dc.ws.back().sync_clean;
   *out = np;
   return cudaSuccess;
 }
@@ -185,7 +189,7 @@ static int evict_impl(const nacl_params_t& p) {
   if (p.n_protect > 0 && !p.protect_idx) return NACL_ERR_NULL;
   if (p.reserved0 != 0) return NACL_ERR_UNSUPPORTED;
   const uint32_t known = NACL_FLAG_CAUSAL | NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE | NACL_FLAG_SAMPLE_UNIFORM | NACL_FLAG_SHARED_HEADS |
-                         NACL_FLAG_SCORE_CUDA_CORES;
+                         NACL_FLAG_SCORE_CUDA_CORES | NACL_FLAG_SCORE_TWO_LAUNCHES;
   if (p.flags & ~known) return NACL_ERR_UNSUPPORTED;
   if ((p.flags & NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE) && (p.flags & NACL_FLAG_SAMPLE_UNIFORM)) return NACL_ERR_UNSUPPORTED;
 
@@ -219,6 +223,13 @@ static int evict_impl(const nacl_params_t& p) {
   cudaStream_t st = static_cast<cudaStream_t>(p.stream);
   cudaError_t e;
   void* wsp = p.workspace;
+  const bool tc = !(p.flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
+  const bool two_launches = (p.flags & NACL_FLAG_SCORE_TWO_LAUNCHES) != 0;
+  // the fused scoring launch hands the softmax partials from CTA to CTA through counters that must be zero at launch;
+  // the kernel leaves them zero again.  A caller's workspace is zeroed every time, the library's own only when the
+  // counters reach into bytes that another shape may have used for something else.
+  const size_t sync_bytes = (tc && !two_launches && !p.lse_in) ? sync_ints((size_t)p.batch * p.Hkv) * sizeof(int) : 0;
+  bool zero_sync = sync_bytes > 0;
   if (wsp) {
     if (p.workspace_bytes < need || (reinterpret_cast<uintptr_t>(wsp) & 255u)) return NACL_ERR_WORKSPACE;
   } else {
@@ -226,16 +237,25 @@ static int evict_impl(const nacl_params_t& p) {
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return fail_cuda(e);
     if (dev < 0 || dev >= 64) return NACL_ERR_UNSUPPORTED;
     std::lock_guard<std::mutex> lk(g_mu);
-    e = stream_workspace(g_cache[dev], st, need, &wsp);
+    size_t* clean = nullptr;
+    e = stream_workspace(g_cache[dev], st, need, &wsp, &clean);
     if (e != cudaSuccess) return fail_cuda(e);
+    // the counters' bytes are reserved for them in every carve-up; what lies behind them is written by this call's other buffers
+    const size_t reserved = sync_ints((size_t)p.batch * p.Hkv) * sizeof(int);
+    if (sync_bytes > 0) {
+      if (*clean >= reserved) zero_sync = false;
+      *clean = reserved;
+    } else if (*clean > reserved) {
+      *clean = reserved;
+    }
   }
   const Workspace ws = carve_workspace(wsp, p.batch, p.L, p.Hq, p.Hkv, p.P);
   const SplitPlan sp = make_split_plan(p.batch, p.L, p.Hkv);
+  if (zero_sync && (e = cudaMemsetAsync(ws.sync, 0, sync_bytes, st)) != cudaSuccess) return fail_cuda(e);
 
-  const bool tc = !(p.flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
   if (p.lse_in && (reinterpret_cast<uintptr_t>(p.lse_in) & 3u)) return NACL_ERR_ALIGN;
   const bool causal = (p.flags & NACL_FLAG_CAUSAL) != 0;
-  if (tc) e = launch_score_tc(s, p.K, p.Qproxy, sp, ws, p.lse_in, causal, p.out_importance, p.out_lse, st);
+  if (tc) e = launch_score_tc(s, p.K, p.Qproxy, sp, ws, p.lse_in, causal, two_launches, p.out_importance, p.out_lse, st);
   else e = launch_score_generic(s, p.K, p.Qproxy, sp, ws, p.lse_in, causal, p.out_importance, p.out_lse, st);
   if (e != cudaSuccess) return fail_cuda(e);
 
@@ -441,7 +461,7 @@ int nacl_launch_count(int dtype, int batch, int L, int Hq, int Hkv, int d, int P
   s.G = Hq / Hkv; s.rows = s.G * P; s.dtype = dtype; s.esize = dtype == NACL_DTYPE_F32 ? 4 : 2;
   const bool tc = !(flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
   // scoring + select (+ a separate keys kernel for very long rows) + gather (budget_random > 0 and C > 0 assumed)
-  return (tc ? score_tc_launch_count(s) : 3) + (select_uses_cluster(L) ? 1 : 3);  // the cluster select also gathers
+  return (tc ? score_tc_launch_count(s, (flags & NACL_FLAG_SCORE_TWO_LAUNCHES) != 0) : 3) + (select_uses_cluster(L) ? 1 : 3);  // the cluster select also gathers
 }
 
 int nacl_profile_enable(int on) {

@@ -38,7 +38,7 @@ struct Workspace {
   float* lse;          // [batch*Hq*P]            natural-log LSE of every proxy row
   float* imp;          // [batch*Hkv, L]          importance F_score
   uint32_t* key;       // select scratch (select_scratch_words): global radix histograms, or [batch*Hkv, L] keys for very long rows
-  int* sync;           // [sync_ints(heads)]      reserved (counters / flags for future fused variants)
+  int* sync;           // [sync_ints(heads)]      fused scoring launch: per-head hand-over counters (score_tc.cu); zero between calls
   float* imp_sh;       // [batch, L]              NACL_FLAG_SHARED_HEADS: importance summed over the kv heads
   int32_t* idx_sh;     // [batch, L]              NACL_FLAG_SHARED_HEADS: the shared retained set (C <= L entries per batch element)
   int32_t* idx_tmp;    // [batch*Hkv, L]          nacl_evict_generation without out_idx: the kept slots
@@ -69,10 +69,11 @@ cudaError_t launch_score_generic(const Shape& s, const void* K, const void* Q, c
 
 // tensor-core scoring (bf16, d == 128, G*P % 16 == 0, G*P <= 256): tcgen05 + TMA
 bool score_tc_supported(const Shape& s);
-int score_tc_launch_count(const Shape& s);
+int score_tc_launch_count(const Shape& s, bool two_launches);
 size_t score_tc_part_elems(int heads, int rows);  // float2 elements of Workspace::part the tensor-core path needs
 cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const SplitPlan& sp,
-                            const Workspace& ws, const float* lse_in, bool causal, float* imp_out, float* lse_out, cudaStream_t st);
+                            const Workspace& ws, const float* lse_in, bool causal, bool two_launches, float* imp_out,
+                            float* lse_out, cudaStream_t st);
 
 // Gumbel-top-k keys: key[p,j] = fl32(ln w(imp) - ln(-ln u)), order-mapped to uint32 (ordermapped) or as float bits
 // batch_offset / head_offset: global indices of the call's first batch element / kv head (Philox counter words)

@@ -91,12 +91,20 @@ __device__ long long g_tl[2][20][32][8];
 #define TL2(k)
 #endif
 
+// Optional globaltimer stamps of every CTA (diagnostics build only: -DNACL_TC_STAMPS): kernel entry, TMEM allocated,
+// sweep S done, sweep C done.
+#ifdef NACL_TC_STAMPS
+__device__ long long g_stamps[160][4];
+#define GSTAMP(k) { if (threadIdx.x == 0 && blockIdx.x < 160) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_stamps[blockIdx.x][k] = t_; } }
+#else
+#define GSTAMP(k)
+#endif
+
 struct TcParams {
   int L, rows, T;          // keys per head, proxy rows per row block (G*P, or 256 when G*P > 256), key tiles per head
   int rows_total, nrb;     // G*P and the number of 256-row blocks (1 unless G*P > 256)
   int Hkv;                 // kv heads per batch element (K tensor-map coordinates)
   int heads, n_slots;      // n_slots: epilogue warps that share a proxy row in sweep S = partials per (row, piece): 2 if rows > 128, else 4
-  int phase;               // 0 = sweep S (statistics), 1 = sweep C (column sums)
   int causal, P;           // NACL_FLAG_CAUSAL: proxy row r (i = r % P, prompt position L-P+i) sees keys j <= L-P+i
   long long N;             // heads * T
   float scale_log2;        // log2(e) / sqrt(d)
@@ -105,6 +113,9 @@ struct TcParams {
   float* lse_out;          // optional [heads*rows], natural log
   float* imp;              // [heads, L]
   float* imp_out;          // optional
+  int* sync;               // fused launch: [2 * heads] zero at launch: per head the number of (CTA, row block) pieces whose
+                           // partials are published, and the number of consumers that have seen them all (the last one
+                           // zeroes both again)
 };
 
 // ------------------------------------------------------------------ PTX wrappers
@@ -311,12 +322,12 @@ struct Walk {
   long long t;
   int remaining, step, T, nrb, rb;
   Seg cur;
-  __device__ Walk(const TcParams& p) {
+  __device__ Walk(const TcParams& p, int phase) {
     const long long G = gridDim.x, c = blockIdx.x;
     const long long t0 = p.N * c / G, t1 = p.N * (c + 1) / G;
     remaining = (int)(t1 - t0);
-    step = p.phase ? -1 : 1;
-    t = p.phase ? t1 - 1 : t0;
+    step = phase ? -1 : 1;
+    t = phase ? t1 - 1 : t0;
     T = p.T;
     nrb = p.nrb;
     rb = nrb;  // "current segment exhausted"
@@ -524,14 +535,46 @@ __device__ __noinline__ float c_cols_causal(uint32_t taddr, int nc, float sc, in
   return acc;
 }
 
+// ------------------------------------------------------------------ inter-CTA hand-over of the partials (fused launch)
+// Called by all epilogue threads after their partial stores (st.cg) of a segment: CTA barrier, then ONE thread makes the
+// stores visible at gpu scope and counts the piece (the pattern of a cooperative-groups grid barrier, per head).
+__device__ __forceinline__ void publish_piece(int* cnt) {
+  asm volatile("bar.sync 2, %0;" ::"n"(EPI_THREADS) : "memory");
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(cnt, 1);
+  }
+}
+// Called by all epilogue threads before they read the partials of a head: one thread polls until all `need` pieces are
+// published; the consumer that completes the head's `need` consumers zeroes both counters for the next launch.
+__device__ __forceinline__ void await_pieces(int* cnt, int* done, int need) {
+  if (threadIdx.x == 0) {
+    uint32_t spins = 0;
+    int v;
+    do {
+      asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(cnt) : "memory");
+      if (++spins > SPIN_LIMIT) __trap();
+    } while (v < need);
+    if (atomicAdd(done, 1) == need - 1) {
+      atomicExch(cnt, 0);
+      atomicExch(done, 0);
+    }
+  }
+  asm volatile("bar.sync 2, %0;" ::"n"(EPI_THREADS) : "memory");
+}
+
 // ------------------------------------------------------------------ the kernel
-template <int QROWS, int NQ, int STAGES, int PH>
-__global__ void __launch_bounds__(NTHREADS, 1)
-nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmQ, const TcParams p) {
+// One sweep (PH = 0: S, PH = 1: C) of the CTA's tile range.  Called once per sweep by the kernel below; TMEM is already
+// allocated (tmem_base), the shared-memory carve-up and every mbarrier are (re)initialised here, and on return every
+// asynchronous arrival on them has landed, so that the next sweep may carve the same bytes differently.
+// FUSED: both sweeps run in one launch.  Sweep C of a head then needs the partials of every CTA whose range touches
+// the head: a per-head counter in global memory (p.sync), incremented by each CTA once its partials of a segment are
+// published and polled by one thread per consumer segment.  Nothing waits in sweep S, so the waits cannot form a cycle;
+// the launch is cooperative, so every CTA is resident.
+template <int QROWS, int NQ, int STAGES, int PH, bool FUSED>
+__device__ __forceinline__ void sweep(const CUtensorMap& tmK, const CUtensorMap& tmQ, const TcParams& p, uint8_t* smem,
+                                      const uint32_t sbase, const uint32_t tmem_base) {
   using SM = Smem<QROWS, NQ, STAGES, PH>;
-  extern __shared__ __align__(1024) uint8_t smem[];
-  const uint32_t sbase = smem_u32(smem);
-  if ((sbase & 1023u) != 0) __trap();  // the 128B-swizzled operand tiles need 1024-byte alignment
 
   const uint32_t bars = sbase + SM::OFF_BARS;
   constexpr int B_KE = STAGES, B_QF = 2 * STAGES, B_QE = B_QF + NQ, B_AF = B_QE + NQ, B_AE = B_AF + NQ, B_TF = B_AE + NQ,
@@ -549,7 +592,6 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
   auto tm_empty = [&](int b, int h) { return bars + 8u * (B_TE + 2 * b + h); };
   auto cs_full = [&](int b) { return bars + 8u * (B_CF + b); };
   auto cs_empty = [&](int b) { return bars + 8u * (B_CE + b); };
-  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + SM::OFF_TMEM);
   float* cs_s = reinterpret_cast<float*>(smem + SM::OFF_CS);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -592,21 +634,16 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the MMA's async proxy
   }
-  if (warp == W_MMA) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(sbase + SM::OFF_TMEM), "r"(TMEM_COLS) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot;
 
   if (warp == W_TMA) {
     // ================================================================ TMA producer
     const bool leader = elect_one();
-    int stage = 0, qrun = 0;
+    int stage = 0, qrun = 0, kuse = 0;
     uint32_t kphase = 0;
-    Walk walk(p);
+    Walk walk(p, PH);
     Seg sg;
     while (walk.next(sg)) {
       const int qb = qrun % NQ;
@@ -622,14 +659,26 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
       for (int i = 0; i < sg.n; ++i) {
         TRW(0, mbar_wait(k_empty(stage), kphase ^ 1));
         const uint32_t kdst = sbase + SM::OFF_K + stage * KSTAGE_BYTES;
+#ifdef NACL_DIAG_SAME_TILE  // diagnostics: every K tile comes from L2 (results are wrong)
+        const int j0 = ((sg.tile + walk.step * i) & 7) * TILE;
+#else
         const int j0 = (sg.tile + walk.step * i) * TILE;
+#endif
         if (leader) {
           mbar_expect_tx(k_full(stage), KSTAGE_BYTES);
           tma_load_4d(kdst, &tmK, 0, j0, hk, hb, k_full(stage));
           tma_load_4d(kdst + BOX_BYTES, &tmK, 64, j0, hk, hb, k_full(stage));
         }
         if (++stage == STAGES) { stage = 0; kphase ^= 1; }
+        ++kuse;
       }
+    }
+    // drain: the tcgen05.commit arrivals on k_empty / q_empty / qa_empty of the last uses are asynchronous and nobody has
+    // waited for them yet; they must have landed before these bytes are re-initialised or carved up differently
+    for (int u = kuse > STAGES ? kuse - STAGES : 0; u < kuse; ++u) mbar_wait(k_empty(u % STAGES), (u / STAGES) & 1);
+    for (int u = qrun > NQ ? qrun - NQ : 0; u < qrun; ++u) {
+      mbar_wait(q_empty(u % NQ), (u / NQ) & 1);
+      if constexpr (PH != 0) mbar_wait(qa_empty(u % NQ), (u / NQ) & 1);
     }
     __syncwarp();
   } else if (warp == W_MMA || warp == W_MMA2) {
@@ -643,7 +692,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
     int stage = 0, qrun = 0;
     uint32_t kphase = 0, tcount = 0;
     const uint32_t idesc = PH == 0 ? umma_idesc(128, TILE) : umma_idesc(128, p.rows);
-    Walk walk(p);
+    Walk walk(p, PH);
     Seg sg;
     while (walk.next(sg)) {
       const int qb = qrun % NQ;
@@ -750,7 +799,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
     // ================================================================ column-sum combiner (sweep C only)
     if constexpr (PH != 0) {
       uint32_t ccount = 0;
-      Walk walk(p);
+      Walk walk(p, PH);
       Seg sg;
       while (walk.next(sg)) {
         for (int i = 0; i < sg.n; ++i, ++ccount) {
@@ -803,7 +852,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
     auto rows_in_block = [&](int rb) { return min(p.rows, p.rows_total - rb * 256); };
     uint32_t ecount = 0;  // tiles seen so far, same sequence as the MMA warp's tcount
     int nseg = 0;
-    Walk walk(p);
+    Walk walk(p, PH);
     Seg sg;
     while (walk.next(sg)) {
       if constexpr (PH == 0) {
@@ -852,6 +901,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
           }
           if (q_row < rows_in_block(sg.rb))
             __stcg(&p.part[(((size_t)blockIdx.x + sg.head) * p.n_slots + q_par) * p.rows_total + sg.rb * 256 + q_row], make_float2(m0, z0));
+          if constexpr (FUSED) publish_piece(p.sync + sg.head);
           ecount += sg.n;
           ++nseg;
           continue;
@@ -879,6 +929,7 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
         // this warp's partial of the piece; (-inf, 0) when it saw no valid key
         if (s_row < p.rows)
           __stcg(&p.part[(((size_t)blockIdx.x + sg.head) * p.n_slots + s_slot) * p.rows_total + sg.rb * 256 + s_row], make_float2(m0, z0));
+        if constexpr (FUSED) publish_piece(p.sync + sg.head);
       } else {
         // ---------------- C segment: merge the head's partials (ascending piece order) into lse, hand -lse/scale to the MMA
         // issuers as the operand of the ninth k-step (augmented contraction: the accumulator then holds s - lse/scale and
@@ -887,6 +938,11 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
         const int qs = nseg % NQ;
         TRW(2, {
           mbar_wait(qa_empty(qs), ((nseg / NQ) & 1) ^ 1);  // the MMAs of the segment that used this slot before are done
+          if constexpr (FUSED) {
+            const int c_first = cta_of_tile((long long)sg.head * p.T, p.N, G);
+            const int c_last = cta_of_tile((long long)(sg.head + 1) * p.T - 1, p.N, G);
+            await_pieces(p.sync + sg.head, p.sync + p.heads + sg.head, (c_last - c_first + 1) * p.nrb);
+          }
           const int r = threadIdx.x;
           if (r < p.rows) {
             float cf;
@@ -1003,6 +1059,31 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
   TR_FLUSH()
   tc_fence_before();
   __syncthreads();
+}
+
+// MODE 0: sweep S, 1: sweep C (two launches, or lse_in given), 2: S then C in one cooperative launch
+template <int QROWS, int NQ, int STAGES_S, int STAGES_C, int MODE>
+__global__ void __launch_bounds__(NTHREADS, 1)
+nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmQ, const TcParams p) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  const uint32_t sbase = smem_u32(smem);
+  if ((sbase & 1023u) != 0) __trap();  // the 128B-swizzled operand tiles need 1024-byte alignment
+  GSTAMP(0)
+  __shared__ uint32_t tmem_slot;
+  const int warp = threadIdx.x >> 5;
+  if (warp == W_MMA) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_slot)), "r"(TMEM_COLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(&tmem_slot);
+  GSTAMP(1)
+  if constexpr (MODE != 1) sweep<QROWS, NQ, STAGES_S, 0, MODE == 2>(tmK, tmQ, p, smem, sbase, tmem_base);
+  GSTAMP(2)
+  if constexpr (MODE != 0) sweep<QROWS, NQ, STAGES_C, 1, MODE == 2>(tmK, tmQ, p, smem, sbase, tmem_base);
+  GSTAMP(3)
   if (warp == W_MMA) {
     tc_fence_after();
     __syncwarp();
@@ -1036,31 +1117,49 @@ int sm_count() {
   return n;
 }
 
+template <class Kern>
+cudaError_t launch_one(Kern kern, int grid, int smem_bytes, bool cooperative, const CUtensorMap& tmK, const CUtensorMap& tmQ,
+                       const TcParams& p, cudaStream_t st) {
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+  if (e != cudaSuccess) return e;
+  cudaLaunchConfig_t cfg = {};
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeCooperative;  // every CTA resident: the fused launch has inter-CTA waits
+  attr[0].val.cooperative = 1;
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3(NTHREADS);
+  cfg.dynamicSmemBytes = (size_t)smem_bytes;
+  cfg.stream = st;
+  cfg.attrs = attr;
+  cfg.numAttrs = cooperative ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, tmK, tmQ, p);
+}
+
 template <int QROWS, int NQ, int STAGES_S, int STAGES_C>
-cudaError_t launch_cfg(const CUtensorMap& tmK, const CUtensorMap& tmQ, TcParams p, cudaStream_t st) {
+cudaError_t launch_cfg(const CUtensorMap& tmK, const CUtensorMap& tmQ, TcParams p, bool two_launches, cudaStream_t st) {
   using SMS = Smem<QROWS, NQ, STAGES_S, 0>;
   using SMC = Smem<QROWS, NQ, STAGES_C, 1>;
-  static_assert(SMS::TOTAL <= 227 * 1024 && SMC::TOTAL <= 227 * 1024, "shared memory budget");
-  auto kern_s = nacl_score_tc_kernel<QROWS, NQ, STAGES_S, 0>;
-  auto kern_c = nacl_score_tc_kernel<QROWS, NQ, STAGES_C, 1>;
-  cudaError_t e = cudaFuncSetAttribute(kern_s, cudaFuncAttributeMaxDynamicSharedMemorySize, SMS::TOTAL);
-  if (e != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(kern_c, cudaFuncAttributeMaxDynamicSharedMemorySize, SMC::TOTAL)) != cudaSuccess) return e;
+  constexpr int kStatic = 1024 + 16;  // the kernel's static shared memory (TMEM slot) and the alignment gap it may cause
+  static_assert(SMS::TOTAL + kStatic <= 227 * 1024 && SMC::TOTAL + kStatic <= 227 * 1024, "shared memory budget");
+  constexpr int kBoth = SMS::TOTAL > SMC::TOTAL ? SMS::TOTAL : SMC::TOTAL;
   long long grid = sm_count() < MAX_GRID ? sm_count() : MAX_GRID;
   if (p.N < grid) grid = p.N;
-  if (!p.lse_in) {
-    StageScope sc(ST_STATS, st);
-    p.phase = 0;
-    kern_s<<<(int)grid, NTHREADS, SMS::TOTAL, st>>>(tmK, tmQ, p);
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  cudaError_t e;
+  if (p.lse_in) {
+    StageScope sc(ST_COLSUM, st);
+    return launch_one(nacl_score_tc_kernel<QROWS, NQ, STAGES_S, STAGES_C, 1>, (int)grid, SMC::TOTAL, false, tmK, tmQ, p, st);
+  }
+  if (!two_launches) {
+    StageScope sc(ST_FUSED, st);
+    return launch_one(nacl_score_tc_kernel<QROWS, NQ, STAGES_S, STAGES_C, 2>, (int)grid, kBoth, true, tmK, tmQ, p, st);
   }
   {
-    StageScope sc(ST_COLSUM, st);
-    p.phase = 1;
-    kern_c<<<(int)grid, NTHREADS, SMC::TOTAL, st>>>(tmK, tmQ, p);
-    e = cudaGetLastError();
+    StageScope sc(ST_STATS, st);
+    e = launch_one(nacl_score_tc_kernel<QROWS, NQ, STAGES_S, STAGES_C, 0>, (int)grid, SMS::TOTAL, false, tmK, tmQ, p, st);
+    if (e != cudaSuccess) return e;
   }
-  return e;
+  StageScope sc(ST_COLSUM, st);
+  return launch_one(nacl_score_tc_kernel<QROWS, NQ, STAGES_S, STAGES_C, 1>, (int)grid, SMC::TOTAL, false, tmK, tmQ, p, st);
 }
 
 }  // namespace
@@ -1070,12 +1169,12 @@ bool score_tc_supported(const Shape& s) {
          s.rows <= 8192;  // G*P > 256: blocks of 256 proxy rows, the last one masked where G*P is off that grid
 }
 
-int score_tc_launch_count(const Shape&) { return 2; }
+int score_tc_launch_count(const Shape&, bool two_launches) { return two_launches ? 2 : 1; }
 
 size_t score_tc_part_elems(int heads, int rows) { return (size_t)(MAX_GRID + heads) * 4 * rows; }
 
 cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const SplitPlan&, const Workspace& ws,
-                            const float* lse_in, bool causal, float* imp_out, float* lse_out, cudaStream_t st) {
+                            const float* lse_in, bool causal, bool two_launches, float* imp_out, float* lse_out, cudaStream_t st) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return cudaErrorNotSupported;  // no silent fallback: the caller reports NACL_ERR_CUDA
   const int heads = s.batch * s.Hkv;
@@ -1107,18 +1206,23 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
   p.rows_total = s.rows; p.nrb = (s.rows + 255) / 256;
   p.heads = heads; p.Hkv = s.Hkv;
   p.n_slots = s.rows <= 128 ? 4 : 2;
-  p.phase = 0;
   p.causal = causal ? 1 : 0; p.P = s.P;
   p.N = (long long)heads * p.T;
   p.scale_log2 = 1.4426950408889634f / sqrtf((float)s.d);
   p.part = ws.part; p.lse_in = lse_in; p.lse_out = lse_out; p.imp = ws.imp; p.imp_out = imp_out;
+  p.sync = ws.sync;
 
-  if (qrows == 128) return launch_cfg<128, 2, 5, 3>(tmK, tmQ, p, st);
-  return launch_cfg<256, 1, 5, 3>(tmK, tmQ, p, st);
+  if (qrows == 128) return launch_cfg<128, 2, 5, 3>(tmK, tmQ, p, two_launches, st);
+  return launch_cfg<256, 1, 5, 3>(tmK, tmQ, p, two_launches, st);
 }
 
 }  // namespace nacl
 
+#ifdef NACL_TC_STAMPS
+extern "C" __attribute__((visibility("default"))) int nacl_debug_stamps_read(long long* host) {
+  return (int)cudaMemcpyFromSymbol(host, nacl::g_stamps, sizeof(nacl::g_stamps));
+}
+#endif
 #ifdef NACL_TC_TRACE
 // diagnostics build only: per-warp wait/compute cycle counters of the last launches
 extern "C" __attribute__((visibility("default"))) int nacl_debug_trace_read(long long* host, size_t bytes) {

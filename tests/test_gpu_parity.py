@@ -78,6 +78,23 @@ def test_cuda_core_flag_matches_default_path(binding, dt, d):
     full_parity(K, V, Q, 120, 40, 4, 16, seed=9, layer=1, flags=binding.FLAG_SCORE_CUDA_CORES, oracle_flags=0)
 
 
+def test_fused_scoring_launch_matches_two_launches(binding):
+    """The tensor-core path runs both sweeps in ONE cooperative launch (per-head hand-over counters between the CTAs);
+    NACL_FLAG_SCORE_TWO_LAUNCHES runs them as two launches.  Same arithmetic in the same order: bit-identical importance,
+    indices and caches.  Shapes alternate so that the self-cleaning counters are reused at different sizes."""
+    shapes = [(1, 4100, 32, 8, 128, 64), (4, 700, 8, 8, 128, 16), (2, 9000, 16, 2, 128, 32), (1, 129, 8, 8, 128, 16),
+              (1, 1200, 8, 2, 128, 100), (4, 700, 8, 8, 128, 16), (1, 4100, 32, 8, 128, 64)]
+    for rep, (B, L, Hq, Hkv, d, P) in enumerate(shapes):
+        K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype="bf16", seed=100 + rep)
+        Kc, Vc, Qc = K.cuda(), V.cuda(), Q.cuda()
+        Bp, Br = L // 5, L // 20
+        a = binding.nacl_evict_ex(Kc, Vc, Qc, Bp, Br, 4, P, 3, rep, want_importance=True)
+        b = binding.nacl_evict_ex(Kc, Vc, Qc, Bp, Br, 4, P, 3, rep, flags=binding.FLAG_SCORE_TWO_LAUNCHES, want_importance=True)
+        for k in ("importance", "out_idx", "out_K", "out_V"):
+            assert torch.equal(a[k], b[k]), f"shape {rep}: {k} differs between the fused and the two-launch scoring"
+    full_parity(K, V, Q, Bp, Br, 4, P, seed=3, layer=1)
+
+
 def test_edge_budgets(binding):
     K, V, Q = make_random_inputs(1, 300, 4, 2, 64, 4, dtype="f32", seed=1)
     L = 300

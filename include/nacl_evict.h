@@ -89,6 +89,8 @@ extern "C" {
                                                 head's out_idx row holds that set and out_K/out_V are gathered with it */
 #define NACL_FLAG_SCORE_CUDA_CORES 0x100u    /* debugging: run the generic CUDA-core scoring kernels even where
                                                 the tensor-core path applies */
+#define NACL_FLAG_SELECT_GENERAL 0x400u      /* debugging / profiling: the selection takes the general three-pass radix path even
+                                                where the one-pass bucket path applies (same result, bit for bit) */
 #define NACL_FLAG_SCORE_TWO_LAUNCHES 0x200u  /* debugging / profiling: the tensor-core path runs its statistics sweep and its
                                                 column-sum sweep as two launches instead of one cooperative launch */
 
@@ -238,6 +240,11 @@ int nacl_launch_count(int dtype, int batch, int L, int Hq, int Hkv, int d, int P
 int nacl_profile_enable(int on);
 int nacl_profile_read(double* ms, int64_t* launches, int reset);
 const char* nacl_stage_name(int stage);
+
+/* Diagnostics: the number of (batch, kv head) selections on the current device that left the one-pass bucket path for the
+ * general three-pass radix path since the last reset (a threshold in a clamped edge bucket, a candidate list that
+ * would overflow; the result is the same either way).  Synchronises the device.  Returns the count or NACL_ERR_CUDA. */
+int nacl_select_fallbacks(int reset);
 
 /* Frees the per-device internal workspaces / staging buffers (optional, e.g. before exit). */
 void nacl_release(void);

@@ -16,11 +16,12 @@ from . import build as _build
 
 NACL_DTYPE_F32, NACL_DTYPE_BF16 = 0, 1
 FLAG_CAUSAL, FLAG_SAMPLE_SOFTMAX_OF_SCORE, FLAG_SAMPLE_UNIFORM, FLAG_SHARED_HEADS, FLAG_SCORE_CUDA_CORES = 1, 2, 4, 8, 0x100
-FLAG_SCORE_TWO_LAUNCHES = 0x200
+FLAG_SCORE_TWO_LAUNCHES, FLAG_SELECT_GENERAL = 0x200, 0x400
 
 EXPORTS = ("nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes",
            "nacl_launch_count", "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version",
-           "nacl_profile_enable", "nacl_profile_read", "nacl_stage_name", "nacl_gumbel_keys", "nacl_evict_generation")
+           "nacl_profile_enable", "nacl_profile_read", "nacl_stage_name", "nacl_gumbel_keys", "nacl_evict_generation",
+           "nacl_select_fallbacks")
 N_STAGES = 7
 
 
@@ -91,6 +92,8 @@ def _load() -> C.CDLL:
     lib.nacl_launch_count.restype = i32
     lib.nacl_release.argtypes = []
     lib.nacl_release.restype = None
+    lib.nacl_select_fallbacks.argtypes = [i32]
+    lib.nacl_select_fallbacks.restype = i32
     lib.nacl_strerror.argtypes = [i32]
     lib.nacl_strerror.restype = C.c_char_p
     lib.nacl_last_cuda_error.argtypes = []
@@ -148,6 +151,13 @@ def nacl_workspace_bytes(batch, L, Hq, Hkv, d, P) -> int:
 
 def nacl_launch_count(dtype, batch, L, Hq, Hkv, d, P, flags=0) -> int:
     return int(_lib.nacl_launch_count(dtype, batch, L, Hq, Hkv, d, P, flags))
+
+
+def nacl_select_fallbacks(reset: bool = True) -> int:
+    rc = int(_lib.nacl_select_fallbacks(1 if reset else 0))
+    if rc < 0:
+        raise NaclError(rc, "nacl_select_fallbacks")
+    return rc
 
 
 def nacl_release() -> None:

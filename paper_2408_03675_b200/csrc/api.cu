@@ -189,7 +189,7 @@ static int evict_impl(const nacl_params_t& p) {
   if (p.n_protect > 0 && !p.protect_idx) return NACL_ERR_NULL;
   if (p.reserved0 != 0) return NACL_ERR_UNSUPPORTED;
   const uint32_t known = NACL_FLAG_CAUSAL | NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE | NACL_FLAG_SAMPLE_UNIFORM | NACL_FLAG_SHARED_HEADS |
-                         NACL_FLAG_SCORE_CUDA_CORES | NACL_FLAG_SCORE_TWO_LAUNCHES;
+                         NACL_FLAG_SCORE_CUDA_CORES | NACL_FLAG_SCORE_TWO_LAUNCHES | NACL_FLAG_SELECT_GENERAL;
   if (p.flags & ~known) return NACL_ERR_UNSUPPORTED;
   if ((p.flags & NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE) && (p.flags & NACL_FLAG_SAMPLE_UNIFORM)) return NACL_ERR_UNSUPPORTED;
 
@@ -266,12 +266,14 @@ static int evict_impl(const nacl_params_t& p) {
     if ((e = launch_head_sum(ws.imp, ws.imp_sh, p.batch, p.Hkv, p.L, st)) != cudaSuccess) return fail_cuda(e);
     if ((e = launch_protect(ws.imp_sh, p.batch, p.L, p.protect_idx, p.n_protect, st)) != cudaSuccess) return fail_cuda(e);
     e = launch_select(ws.imp_sh, ws.key, p.batch, 1, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
-                      p.flags, ws.idx_sh, nullptr, nullptr, nullptr, nullptr, row_bytes, &gathered, p.batch_offset, p.head_offset, &s, st);
+                      p.flags, ws.idx_sh, nullptr, nullptr, nullptr, nullptr, row_bytes, &gathered, p.batch_offset, p.head_offset, &s,
+                      (float)p.Hkv * (float)s.rows / (float)p.L, st);
     if (e == cudaSuccess) e = launch_replicate_idx(ws.idx_sh, p.out_idx, p.batch, p.Hkv, C, st);
   } else {
     if ((e = launch_protect(ws.imp, p.batch * p.Hkv, p.L, p.protect_idx, p.n_protect, st)) != cudaSuccess) return fail_cuda(e);
     e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
-                      p.flags, p.out_idx, p.K, p.V, p.out_K, p.out_V, row_bytes, &gathered, p.batch_offset, p.head_offset, &s, st);
+                      p.flags, p.out_idx, p.K, p.V, p.out_K, p.out_V, row_bytes, &gathered, p.batch_offset, p.head_offset, &s,
+                      (float)s.rows / (float)p.L, st);
   }
   if (e != cudaSuccess) return fail_cuda(e);
   if (!gathered) {

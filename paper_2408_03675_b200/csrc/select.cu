@@ -15,6 +15,8 @@
 //                  candidates that survive the top-k.  Used whenever the slices fit; 8x more CTAs than heads.
 // Integer work only after the keys: results are bit-exact functions of (imp, key).
 #include <cooperative_groups.h>
+#include <math.h>
+#include <string.h>
 
 #include "nacl_internal.cuh"
 
@@ -101,6 +103,34 @@ __device__ __forceinline__ uint32_t gumbel_key(float imp, uint32_t j, uint32_t h
   return ORDERMAP ? ordermap(__float_as_uint(f)) : __float_as_uint(f);
 }
 
+
+// fp32 estimate of the same key (not order-mapped), |estimate - key| < 1e-3 whenever the key is finite and its weight
+// is a normal float (a subnormal or zero weight gives -inf; the exact key is then below -80 or -inf).  Used by the
+// fast selection path to put the candidates into buckets; every decision near the threshold is re-taken on the exact key.
+//   -ln u: for u > 63/64 from the series of -log1p(-(1-u)) (1-u is exact), else from lg2.approx (absolute error 2^-22 on
+//   (0.5, 2), relative 2^-22 elsewhere): relative error < 4e-5;  -ln(-ln u) and ln w the same way: absolute error < 2e-4.
+__device__ __forceinline__ float lg2_approx(float x) {
+  float y;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float gumbel_key_estimate(float imp, uint32_t j, uint32_t hk, uint32_t b, uint32_t layer, uint32_t k0,
+                                                      uint32_t k1, uint32_t flags) {
+  const uint32_t x = philox4x32_10_word0(j, hk, b, layer, k0, k1);
+  const float n = __uint_as_float(0x4B000000u | (x >> 9)) - 8388608.0f;  // (float)(x >> 9), exact
+  const float u = (n + 0.5f) * 0x1p-23f;                                  // exact (24 significant bits)
+  const float v = 1.0f - u;                                               // exact for u >= 0.5
+  float a;                                                                // -ln u
+  if (v < 0.015625f) a = v * fmaf(v, fmaf(v, fmaf(v, 0.25f, 0.33333334f), 0.5f), 1.0f);
+  else a = -0.69314718f * lg2_approx(u);
+  const float g = -0.69314718f * lg2_approx(a);
+  float ln_w;
+  if (flags & NACL_FLAG_SAMPLE_UNIFORM) ln_w = 0.0f;
+  else if (flags & NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE) ln_w = imp;
+  else ln_w = 0.69314718f * lg2_approx(imp);  // imp == 0 (or subnormal: flushed) -> -inf
+  return ln_w + g;
+}
+
 template <bool ORDERMAP>
 __global__ void __launch_bounds__(256) nacl_keys_kernel(const float* __restrict__ imp, uint32_t* __restrict__ key,
                                                     int Hkv, int L, uint32_t k0, uint32_t k1, uint32_t layer, uint32_t flags,
@@ -121,11 +151,12 @@ struct SelShared {
   uint32_t hist[HB];
   int warp_tot[32];
   int total;
-  int bin, krem, cut;
+  int bin, krem, lcut;
 };
 
 // exclusive prefix sum of v over the block in thread order; total in `tot` (uniform)
-__device__ __forceinline__ int block_excl_scan(int v, SelShared& sh, int& tot) {
+template <class SH>
+__device__ __forceinline__ int block_excl_scan(int v, SH& sh, int& tot) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   int inc = v;
 #pragma unroll
@@ -164,8 +195,8 @@ __device__ __forceinline__ void hist_add_aggregated(uint32_t* hist, bool take, u
 // The K largest values of {val(j) : lo <= j < hi, valid(j)}, ties to the lower index, described as
 //   member(j)  <=>  val(j) > thr  ||  (val(j) == thr && j <= cut).
 // Requires 0 <= K <= #valid.  All threads of the block call it with uniform arguments.
-template <class F>
-__device__ void block_radix_select(F getval, int lo, int hi, int K, SelShared& sh, uint32_t& thr, int& cut) {
+template <class SH, class F>
+__device__ void block_radix_select(F getval, int lo, int hi, int K, SH& sh, uint32_t& thr, int& cut) {
   if (K <= 0) { thr = 0xFFFFFFFFu; cut = -1; return; }
   uint32_t prefix = 0, mask = 0;
   int krem = K;
@@ -197,7 +228,7 @@ __device__ void block_radix_select(F getval, int lo, int hi, int K, SelShared& s
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         if (q < w) {
-          if (above < krem && krem <= above + cnt[q]) { sh.bin = top - q; sh.krem = krem - above; sh.cut = cnt[q]; }
+          if (above < krem && krem <= above + cnt[q]) { sh.bin = top - q; sh.krem = krem - above; sh.lcut = cnt[q]; }
           above += cnt[q];
         }
       }
@@ -206,7 +237,7 @@ __device__ void block_radix_select(F getval, int lo, int hi, int K, SelShared& s
     prefix |= (uint32_t)sh.bin << shift;
     mask |= (uint32_t)(nb - 1) << shift;
     krem = sh.krem;
-    n_eq = sh.cut;
+    n_eq = sh.lcut;
     __syncthreads();
   }
   thr = prefix;
@@ -222,9 +253,9 @@ __device__ void block_radix_select(F getval, int lo, int hi, int K, SelShared& s
     int tot;
     const int excl = block_excl_scan(flag, sh, tot);
     if (running + tot >= krem) {
-      if (flag && running + excl + 1 == krem) sh.cut = j;
+      if (flag && running + excl + 1 == krem) sh.lcut = j;
       __syncthreads();
-      result = sh.cut;
+      result = sh.lcut;
       __syncthreads();
       break;
     }
@@ -297,24 +328,30 @@ __device__ __forceinline__ long long sel_gtimer() { long long t; asm volatile("m
 // Integer sums: exact and order-independent.  A buffer is rewritten only after a barrier that every reader reaches
 // after its reads, so single buffers suffice.
 constexpr int kMaxRanks = 16;
+constexpr int kFineW = 68;  // row width of the fine exchange buffer: 64 bins, one neighbour on either side, padding
 struct KvVecLayout { long long sb, sh, sr, ob, oh, orow; };  // strides of K/V and of out_K/out_V in 16-byte vectors
 struct ClShared {
   uint32_t hist[HB];
   uint32_t xsup[kMaxRanks][64];   // [rank][super-bin]: pushed by every rank
-  uint32_t xfine[kMaxRanks][64];  // [rank][bin of the chosen super-bin]
+  uint32_t xfine[kMaxRanks][kFineW];  // [rank][bin of the chosen super-bin] (fast path: one more bin on either side)
   int warp_tot[32];
   int total;
   int sup, bin, krem, neq;        // result of the two steps of a radix pass
   int cnt[3][kMaxRanks];          // per-rank counts: ties of select 0 / select 1, kept positions
   int cut[2];                     // index of the last tie taken, select 0 / select 1
-  int pad[1];                     // sizeof % 16 == 0
+  int lcut;                       // block_radix_select on a candidate list
+  int rc[kMaxRanks][4];           // fast path: per-rank counts of the bins threshold-1, threshold, threshold+1
+  uint32_t lthr;                  // fast path: threshold value found on a candidate list
+  int above;                      // fast path: elements in bins above the threshold bin
+  int pad[2];                     // sizeof % 16 == 0
 };
 static_assert(sizeof(ClShared) % 16 == 0, "the slices behind ClShared stay 16-byte aligned");
 
 // Warp 0: x[r][i], r < nrank, i < n (n = 16 or 64) are per-rank counts of n bins in ascending bin order.  Finds the
 // bin that holds the krem-th element counted from the TOP bin; returns (in every lane) its index, the number of
 // elements in higher bins and its own count.
-__device__ __forceinline__ void warp_find_from_top(const uint32_t (*x)[64], int nrank, int n, int krem, int& idx, int& above,
+template <int W>
+__device__ __forceinline__ void warp_find_from_top(const uint32_t (*x)[W], int nrank, int n, int krem, int& idx, int& above,
                                                    int& count) {
   const int lane = threadIdx.x & 31;
   int lo = 0, hi = 0;
@@ -485,6 +522,331 @@ __device__ void cluster_radix_select(F getval, int nloc, int j0, int K, ClShared
   cut = sh.cut[which];
 }
 
+
+// ------------------------------------------------------------------ fast selection path (one bucket pass per select)
+// The general path above refines a 32-bit radix key in three cluster-wide passes per select (two cluster barriers each).
+// Here every select takes ONE cluster-wide histogram pass over buckets that are fine where the threshold is expected:
+//   top-k:   bucket = the importance's float bits >> 14 (512 buckets per binade) in a 4096-bucket window around the row
+//            mean G*P/L (the importance of a head sums to G*P);  the elements of the threshold bucket (a few hundred of
+//            32k) are pushed, in index order, into a list that every CTA of the cluster holds, and every CTA finishes the
+//            select on that list by itself (no further cluster barrier);
+//   sample:  bucket = floor((k~ - lo) * 64) of the fp32 ESTIMATE k~ of the Gumbel key (|k~ - key| < 1e-3, bucket width
+//            1/64).  With b the bucket that holds the Br-th largest estimate, the Br-th largest EXACT key lies in
+//            [edge(b) - eps, edge(b+1) + eps): every candidate in a bucket >= b+2 is taken, none in a bucket <= b-2 is, and
+//            only the candidates of buckets b-1, b, b+1 (some tens) get the exact fp64 key (gumbel_key) and are decided on
+//            it -- the same decisions as the general path, bit for bit, at a third of the arithmetic per candidate.
+// The path gives up (cluster-uniformly, before it has written anything) whenever a threshold falls into a clamped
+// edge bucket or a list would overflow; the general path then runs from the start.
+#ifdef NACL_SEL_TRACE
+__device__ long long g_sel_trace2[1024][10];
+#define FSTAMP(k) { if (blockIdx.x == 0 && threadIdx.x == 0) g_sel_trace[8 + (k)] = clock64(); \
+  if (threadIdx.x == 0 && blockIdx.x < 1024) g_sel_trace2[blockIdx.x][k] = sel_gtimer(); }
+#else
+#define FSTAMP(k)
+#endif
+__device__ int g_select_fallbacks = 0;  // selections that gave up the fast path (nacl_select_fallbacks)
+constexpr int kFastMaxE = 16;   // consecutive positions per thread (instantiations for 8 and 16): slices of at most 16 * ST positions
+constexpr int kListCap = 4096;  // candidate-list entries (value, position) per select
+constexpr int kImpShift = 14;   // float bits dropped by the top-k bucket: 512 buckets per binade
+constexpr float kKeyBucketsPerUnit = 64.f, kKeyBelow = 24.f;  // sample buckets: [ln mean - 24, ln mean + 40)
+
+// CODE SIZE matters here: every phase of the selection runs once, so straight-line code is fetched cold (the first
+// version of this path spent a third of its time in instruction-fetch stalls).  The helpers are __noinline__ and hand
+// their results over in shared memory; loops over ranks and list entries are not unrolled.
+
+// The cluster: the bucket that holds the krem-th element counted from the top bucket of a 4096-bin histogram (sh.hist,
+// this CTA's slice), by the two small exchanges of cluster_radix_select; the second one also carries the two bins next
+// to the chosen super-bin.  Result in shared memory (valid until the next call): sh.bin, sh.krem = rank inside the bin
+// counted from its top, sh.above = elements in higher bins, and for every rank r the counts of bins bin-1, bin, bin+1 of
+// ITS slice in sh.rc[r][0..2].
+__device__ __noinline__ void fast_hist_find(ClShared& sh, int krem) {
+  cg::cluster_group cluster = cg::this_cluster();
+  const unsigned rank = cluster.block_rank(), nrank = cluster.num_blocks();
+  const int lane = threadIdx.x & 31;
+  {
+    const uint4 h = *reinterpret_cast<const uint4*>(&sh.hist[threadIdx.x * 4]);
+    int s4 = (int)(h.x + h.y + h.z + h.w);
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) s4 += __shfl_xor_sync(0xffffffffu, s4, o);
+    const int sb = (int)threadIdx.x >> 4;
+    if ((lane & 15) == 0) {
+#pragma unroll 1
+      for (unsigned r = 0; r < nrank; ++r) cluster.map_shared_rank(&sh, r)->xsup[rank][sb] = (uint32_t)s4;
+    }
+  }
+  cluster.sync();
+  if (threadIdx.x < 32) {
+    int idx, above, count;
+    warp_find_from_top(sh.xsup, (int)nrank, 64, krem, idx, above, count);
+    if (lane == 0) { sh.sup = idx; sh.krem = krem - above; sh.above = above; }
+  }
+  __syncthreads();
+  const int sup = sh.sup;
+  const int krem1 = sh.krem, above1 = sh.above;
+  if (threadIdx.x < 66) {
+    const int bq = sup * 64 - 1 + (int)threadIdx.x;  // the 64 bins of the super-bin and one on either side
+    const uint32_t h = (bq >= 0 && bq < HB) ? sh.hist[bq] : 0u;
+#pragma unroll 1
+    for (unsigned r = 0; r < nrank; ++r) cluster.map_shared_rank(&sh, r)->xfine[rank][threadIdx.x] = h;
+  }
+  cluster.sync();
+  if (threadIdx.x < 32) {
+    int idx, above, count;
+    // (xfine rows are 66 wide here; warp_find_from_top reads columns 1..64 through the shifted base)
+    warp_find_from_top(reinterpret_cast<const uint32_t(*)[kFineW]>(&sh.xfine[0][1]), (int)nrank, 64, krem1, idx, above, count);
+    if (lane == 0) { sh.bin = sup * 64 + idx; sh.krem = krem1 - above; sh.above = above1 + above; }
+    if (lane < (int)nrank) {
+      const int q = idx + 1;  // column of the threshold bin
+      sh.rc[lane][0] = (int)sh.xfine[lane][q - 1];
+      sh.rc[lane][1] = (int)sh.xfine[lane][q];
+      sh.rc[lane][2] = (int)sh.xfine[lane][q + 1];
+    }
+  }
+  __syncthreads();
+}
+
+// The K-th largest value of list[0..n) (.x = value, ties: the lower list position first), 1 <= K <= n <= kListCap; the
+// list is identical in every CTA, every CTA computes the same.  Result in shared memory: sh.lthr = that value, sh.lcut =
+// the position of the last tie taken (0x7FFFFFFF: all of them).
+__device__ __noinline__ void list_select(const uint2* list, int n, int K, ClShared& sh) {
+  if (n <= 256) {
+    // rank by counting: the element that exactly K-1 elements precede in (value desc, position asc) order
+    if ((int)threadIdx.x < n) {
+      const uint32_t me = list[threadIdx.x].x;
+      int before = 0;
+#pragma unroll 4
+      for (int q = 0; q < n; ++q) {
+        const uint32_t o = list[q].x;
+        before += (o > me || (o == me && q < (int)threadIdx.x)) ? 1 : 0;
+      }
+      if (before == K - 1) { sh.lthr = me; sh.lcut = (int)threadIdx.x; }
+    }
+    __syncthreads();
+    return;
+  }
+  uint32_t thr;
+  int cutpos;
+  block_radix_select([&](int q, uint32_t& v) { v = list[q].x; return true; }, 0, n, K, sh, thr, cutpos);
+  if (threadIdx.x == 0) { sh.lthr = thr; sh.lcut = cutpos; }
+  __syncthreads();
+}
+
+__device__ __noinline__ int fast_scan(int v, ClShared& sh) {
+  int tot;
+  return block_excl_scan(v, sh, tot);  // (the total stays in sh.total)
+}
+__device__ __noinline__ float key_estimate_call(float imp, uint32_t j, uint32_t hk, uint32_t b, uint32_t layer, uint32_t k0, uint32_t k1,
+                                                uint32_t flags) {
+  return gumbel_key_estimate(imp, j, hk, b, layer, k0, k1, flags);
+}
+// this CTA's entries [off, off + cnt) of the candidate list, already in its own copy, go to the other CTAs' copies
+__device__ __noinline__ void list_publish(uint2* list, int off, int cnt) {
+  cg::cluster_group cluster = cg::this_cluster();
+  const unsigned rank = cluster.block_rank(), nrank = cluster.num_blocks();
+  __syncthreads();
+#pragma unroll 1
+  for (int q = threadIdx.x; q < cnt; q += ST) {
+    const uint2 c = list[off + q];
+#pragma unroll 1
+    for (unsigned r = 0; r < nrank; ++r)
+      if (r != rank) cluster.map_shared_rank(list, r)[off + q] = c;
+  }
+  cluster.sync();
+}
+
+// Fast path of the cluster kernel (see above).  Returns false (cluster-uniform) when it gives up; otherwise the kept
+// positions are in out[] and ib[0..tot) (this CTA's part, output rows base .. base+tot).
+template <int FE>
+__device__ bool select_fast(const float* __restrict__ row, int nloc, int E, int j0, int lo, int hi, int k1, int Br, int C,
+                            int imp_base, float key_lo, uint32_t hk_g, uint32_t b_g, uint32_t layer, uint32_t sk0, uint32_t sk1,
+                            uint32_t flags, ClShared& sh, uint32_t* ib, uint32_t* kb, uint2* list, cg::cluster_group& cluster,
+                            int32_t* __restrict__ out, int& tot_out, int& base_out) {
+  const unsigned rank = cluster.block_rank(), nrank = cluster.num_blocks();
+  // thread t owns the E = ceil(Lc / ST) <= FE consecutive positions from i0 = t * E on (short slices spread over all threads)
+  const int t = (int)threadIdx.x, i0 = t * E;
+  auto free_pos = [&](int i) { const int j = j0 + i; return j >= lo && j < hi; };
+
+  // coalesced load through shared memory, then the thread's consecutive positions in registers
+  for (int i = t; i < nloc; i += ST) ib[i] = ordermap(__float_as_uint(row[i]));
+  __syncthreads();
+  uint32_t v[FE];
+  uint32_t livem = 0, freem = 0;  // bit e: position i0+e is this thread's and exists / and is not protected
+#pragma unroll
+  for (int e = 0; e < FE; ++e) {
+    const bool live = e < E && i0 + e < nloc;
+    v[e] = live ? ib[i0 + e] : 0u;
+    livem |= (live ? 1u : 0u) << e;
+    freem |= (live && free_pos(i0 + e) ? 1u : 0u) << e;
+  }
+  cluster.sync();  // every CTA of the cluster is running: its shared memory may be written
+  STAMP(1)
+
+  // ---- a4: top-k1 of the importance outside the protected set
+  uint32_t thr_p = 0xFFFFFFFFu;
+  int cut_p = -1;
+  if (k1 > 0) {
+    for (int i = t; i < HB; i += ST) sh.hist[i] = 0;
+    __syncthreads();
+    uint32_t inb = 0;  // bit e: in the threshold bucket (after the find)
+    int dg[FE];
+#pragma unroll
+    for (int e = 0; e < FE; ++e) {
+      dg[e] = min(max((int)(v[e] >> kImpShift) - imp_base, 0), HB - 1);
+      // (plain shared-memory atomics: the buckets are fine where the values are, lanes rarely meet in one)
+      if ((freem >> e) & 1u) atomicAdd(&sh.hist[dg[e]], 1u);
+    }
+    __syncthreads();
+    FSTAMP(0)
+    fast_hist_find(sh, k1);
+    FSTAMP(1)
+    const int bin = sh.bin, krem = sh.krem;
+    int n_eq = 0, before = 0;
+#pragma unroll 1
+    for (unsigned r = 0; r < nrank; ++r) { before += r < rank ? sh.rc[r][1] : 0; n_eq += sh.rc[r][1]; }
+    if (bin == 0 || bin == HB - 1 || n_eq > kListCap) return false;  // clamped bucket / list overflow (cluster-uniform)
+    if (krem == n_eq) {
+      thr_p = (uint32_t)(bin + imp_base) << kImpShift;  // the whole bucket is taken: its lower edge is a threshold
+      cut_p = 0x7FFFFFFF;
+    } else {
+      int mine = 0;
+#pragma unroll
+      for (int e = 0; e < FE; ++e) {
+        const bool b = ((freem >> e) & 1u) && dg[e] == bin;
+        inb |= (b ? 1u : 0u) << e;
+        mine += b ? 1 : 0;
+      }
+      int pos = before + fast_scan(mine, sh);
+#pragma unroll
+      for (int e = 0; e < FE; ++e)
+        if ((inb >> e) & 1u) list[pos++] = make_uint2(v[e], (uint32_t)(j0 + i0 + e));
+      list_publish(list, before, (int)sh.rc[rank][1]);
+      FSTAMP(2)
+      list_select(list, n_eq, krem, sh);
+      thr_p = sh.lthr;
+      cut_p = sh.lcut == 0x7FFFFFFF ? 0x7FFFFFFF : (int)list[sh.lcut].y;
+      FSTAMP(3)
+    }
+  }
+  auto in_topk = [&](uint32_t val, int j) { return val > thr_p || (val == thr_p && j <= cut_p); };
+  STAMP(2)
+
+  // ---- a5: Gumbel-top-Br over the remaining candidates
+  int kbin = -1;                 // bucket of the Br-th largest key estimate
+  uint32_t thr_r = 0xFFFFFFFFu;  // exact threshold among the candidates of buckets kbin-1 .. kbin+1
+  int cut_r = -1;
+  int kd[FE];                    // bucket of the key estimate; -1: not a candidate
+#pragma unroll
+  for (int e = 0; e < FE; ++e) kd[e] = -1;
+  if (Br > 0) {
+    // (no barrier needed here: a CTA writes another CTA's exchange buffers or list again only after the cluster barriers of
+    // the next fast_hist_find, which that CTA reaches after its last read of them)
+    for (int i = t; i < HB; i += ST) sh.hist[i] = 0;
+    __syncthreads();
+#pragma unroll
+    for (int e = 0; e < FE; ++e) {
+      const int i = i0 + e;
+      if (((freem >> e) & 1u) && !in_topk(v[e], j0 + i)) {
+        const float w = __uint_as_float(v[e] & 0x80000000u ? v[e] & 0x7FFFFFFFu : ~v[e]);  // ordermap^-1
+        const float ke = key_estimate_call(w, (uint32_t)(j0 + i), hk_g, b_g, layer, sk0, sk1, flags);
+        // (-inf, and anything below the window, lands in bucket 0; NaN cannot occur: the weight is >= 0 or +inf)
+        kd[e] = (int)fminf(fmaxf((ke - key_lo) * kKeyBucketsPerUnit, 0.f), (float)(HB - 1));
+        atomicAdd(&sh.hist[kd[e]], 1u);
+      }
+    }
+    STAMP(3)
+    __syncthreads();
+    FSTAMP(4)
+    fast_hist_find(sh, Br);
+    FSTAMP(5)
+    kbin = sh.bin;
+    const int above = sh.above;
+    int n_mid = 0, n_up = 0, before = 0;
+#pragma unroll 1
+    for (unsigned r = 0; r < nrank; ++r) {
+      const int c3 = sh.rc[r][0] + sh.rc[r][1] + sh.rc[r][2];
+      before += r < rank ? c3 : 0;
+      n_mid += c3;
+      n_up += sh.rc[r][2];
+    }
+    if (kbin < 2 || kbin > HB - 3 || n_mid > kListCap) return false;  // too close to a clamped bucket / list overflow
+    const int m = Br - (above - n_up);  // to be taken from buckets kbin-1 .. kbin+1: all of the buckets >= kbin+2 are in
+    uint32_t midm = 0;
+    int mine = 0;
+#pragma unroll
+    for (int e = 0; e < FE; ++e) {
+      const bool b = kd[e] >= kbin - 1 && kd[e] <= kbin + 1;
+      midm |= (b ? 1u : 0u) << e;
+      mine += b ? 1 : 0;
+    }
+    // the candidates of the three buckets go out as (importance, position); every CTA then evaluates the exact keys of the
+    // WHOLE list, one per thread in converged warps (a few tens of keys: cheaper than each owner evaluating its own in
+    // divergent code), and the owners read theirs back from their list slot
+    const int pos0 = before + fast_scan(mine, sh);
+    {
+      int pos = pos0;
+#pragma unroll
+      for (int e = 0; e < FE; ++e)
+        if ((midm >> e) & 1u) list[pos++] = make_uint2(v[e], (uint32_t)(j0 + i0 + e));
+    }
+    list_publish(list, before, sh.rc[rank][0] + sh.rc[rank][1] + sh.rc[rank][2]);
+    FSTAMP(6)
+#pragma unroll 1
+    for (int q = t; q < n_mid; q += ST) {
+      const uint2 c = list[q];
+      const float w = __uint_as_float(c.x & 0x80000000u ? c.x & 0x7FFFFFFFu : ~c.x);  // ordermap^-1
+      list[q].x = gumbel_key<true>(w, c.y, hk_g, b_g, layer, sk0, sk1, flags);       // exact, order-mapped
+    }
+    __syncthreads();
+    FSTAMP(7)
+    list_select(list, n_mid, m, sh);
+    thr_r = sh.lthr;
+    cut_r = sh.lcut == 0x7FFFFFFF ? 0x7FFFFFFF : (int)list[sh.lcut].y;
+    // the owners decide their candidates of the three buckets on the exact key in their list slot
+    {
+      int q = pos0;
+#pragma unroll
+      for (int e = 0; e < FE; ++e)
+        if ((midm >> e) & 1u) {
+          const uint32_t kx = list[q++].x;
+          kd[e] = (kx > thr_r || (kx == thr_r && j0 + i0 + e <= cut_r)) ? HB : -1;  // HB: "above the threshold"
+        }
+    }
+  }
+
+  STAMP(4)
+  // ---- a6: ascending kept-position list
+  uint32_t keep = 0;
+  int mine = 0;
+#pragma unroll
+  for (int e = 0; e < FE; ++e) {
+    const int i = i0 + e;
+    bool k = false;
+    if ((livem >> e) & 1u) k = !((freem >> e) & 1u) || in_topk(v[e], j0 + i) || kd[e] >= kbin + 2;
+    keep |= (k ? 1u : 0u) << e;
+    mine += k ? 1 : 0;
+  }
+  const int excl = fast_scan(mine, sh);
+  const int tot = sh.total;
+  __syncthreads();  // (ib is rewritten below; its last reads lie before the scan)
+  if (t < (int)nrank) cluster.map_shared_rank(&sh, t)->cnt[2][rank] = tot;
+  FSTAMP(8)
+  cluster.sync();  // the last access to another CTA's shared memory lies before this barrier
+  FSTAMP(9)
+  int base = 0;
+#pragma unroll 1
+  for (unsigned r = 0; r < rank; ++r) base += sh.cnt[2][r];
+  int pos = base + excl;
+#pragma unroll
+  for (int e = 0; e < FE; ++e)
+    if ((keep >> e) & 1u) {
+      if (pos < C) { out[pos] = j0 + i0 + e; ib[pos - base] = (uint32_t)(j0 + i0 + e); }
+      ++pos;
+    }
+  tot_out = tot;
+  base_out = base;
+  return true;
+}
+
 // One cluster per (batch, kv head); CTA `rank` owns positions [rank*Lc, min(L, (rank+1)*Lc)).
 // Dynamic shared memory: ClShared, uint32 ib[Lc] (order-mapped importance), uint32 kb[Lc] (order-mapped keys, later keep flags).
 __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __restrict__ imp, int Hkv, int L, int Lc, int k1, int Br,
@@ -492,7 +854,8 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
                                                                  uint32_t layer, uint32_t flags, int32_t* __restrict__ out_idx,
                                                                  const int4* __restrict__ Kv, const int4* __restrict__ Vv,
                                                                  int4* __restrict__ oKv, int4* __restrict__ oVv, int vpr,
-                                                                 uint32_t b_off, uint32_t h_off, KvVecLayout ly) {
+                                                                 uint32_t b_off, uint32_t h_off, KvVecLayout ly, int fast,
+                                                                 int imp_base, float key_lo) {
   cg::cluster_group cluster = cg::this_cluster();
   extern __shared__ __align__(16) unsigned char dyn_raw[];
   ClShared& sh = *reinterpret_cast<ClShared*>(dyn_raw);
@@ -507,7 +870,22 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
   const int lo = n_sink, hi = L - n_recent;  // non-protected positions [lo, hi)
   const float* row = imp + (size_t)p * L + j0;
 
+  int tot = 0, base = 0;
+  int32_t* out = out_idx + (size_t)p * C;
   STAMP(0)
+  bool done = false;
+  if (fast) {
+    uint2* list = reinterpret_cast<uint2*>(dyn + 2 * (size_t)Lc);
+    const int E = (Lc + ST - 1) / ST;
+    if (E <= 8)
+      done = select_fast<8>(row, nloc, E, j0, lo, hi, k1, Br, C, imp_base, key_lo, (uint32_t)hk + h_off, (uint32_t)b + b_off, layer, sk0,
+                            sk1, flags, sh, ib, kb, list, cluster, out, tot, base);
+    else
+      done = select_fast<16>(row, nloc, E, j0, lo, hi, k1, Br, C, imp_base, key_lo, (uint32_t)hk + h_off, (uint32_t)b + b_off, layer, sk0,
+                             sk1, flags, sh, ib, kb, list, cluster, out, tot, base);
+  }
+  if (!done) {
+  if (fast && rank == 0 && threadIdx.x == 0) atomicAdd(&g_select_fallbacks, 1);
   for (int i = threadIdx.x; i < nloc; i += ST) ib[i] = ordermap(__float_as_uint(row[i]));
   cluster.sync();  // every CTA of the cluster is running: its shared memory may be written
   STAMP(1)
@@ -562,14 +940,11 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
   const int i0 = (int)threadIdx.x * E;
   int mine = 0;
   for (int e = 0; e < E; ++e) mine += (i0 + e < nloc) ? (int)kb[i0 + e] : 0;
-  int tot;
   const int excl = cl_block_excl_scan(mine, sh, tot);
   if (threadIdx.x < nrank) cluster.map_shared_rank(&sh, threadIdx.x)->cnt[2][rank] = tot;
   cluster.sync();  // the last access to another CTA's shared memory lies before this barrier
-  int base = 0;  // kept positions of the lower ranks
-  for (unsigned r = 0; r < rank; ++r) base += sh.cnt[2][r];
+  for (unsigned r = 0; r < rank; ++r) base += sh.cnt[2][r];  // kept positions of the lower ranks
   int pos = base + excl;
-  int32_t* out = out_idx + (size_t)p * C;
   for (int e = 0; e < E; ++e) {
     const int i = i0 + e;
     if (i < nloc && kb[i]) {
@@ -577,6 +952,7 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
       ++pos;
     }
   }
+  }  // general path
   STAMP(5)
   if (vpr == 0) return;
   // a7, fused: this CTA moves the K and V rows of the positions IT kept (out rows base .. base+tot), 16-byte vectors,
@@ -656,7 +1032,7 @@ bool select_uses_cluster(int L) { return (L + kMaxRanks - 1) / kMaxRanks <= kMax
 cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, int L, int budget_proxy, int budget_random,
                           int n_sink, int n_recent, uint64_t seed, int layer, uint32_t flags, int32_t* out_idx,
                           const void* K, const void* V, void* out_K, void* out_V, int row_bytes, bool* gathered,
-                          int batch_offset, int head_offset, const Shape* layout, cudaStream_t st) {
+                          int batch_offset, int head_offset, const Shape* layout, float imp_mean, cudaStream_t st) {
   *gathered = false;
   const int C = budget_proxy + budget_random;
   if (C == 0) return cudaSuccess;
@@ -688,6 +1064,10 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   int n = 0, Lc = 0;
   size_t dyn = 0;
   double best = 0.0;
+  // the fast path (slices of at most kFastMaxE * ST positions) keeps a candidate list behind the two slice arrays
+  auto dyn_bytes = [](int lc) {
+    return sizeof(ClShared) + (size_t)lc * 2 * sizeof(uint32_t) + (lc <= kFastMaxE * ST ? (size_t)kListCap * sizeof(uint2) : 0);
+  };
   cudaError_t e = cudaFuncSetAttribute(nacl_select_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)(sizeof(ClShared) + (size_t)kMaxSlice * 2 * sizeof(uint32_t)));
   if (e != cudaSuccess) return e;
@@ -697,7 +1077,7 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
     const int lc = ((L + c - 1) / c + 3) / 4 * 4;
     if (lc > kMaxSlice) continue;
     if (c > 1 && L / c < ST / 2) break;  // slices below half a block of positions are not worth a barrier per pass
-    const size_t d = sizeof(ClShared) + (size_t)lc * 2 * sizeof(uint32_t);
+    const size_t d = dyn_bytes(lc);
     static int active_cache[5][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}, {0, 0}};  // [log2 c][smem class]: co-resident clusters
     const int ci = c == 1 ? 0 : (c == 2 ? 1 : (c == 4 ? 2 : (c == 8 ? 3 : 4))), si = d > 100 * 1024 ? 1 : 0;
     int active = active_cache[ci][si];
@@ -712,7 +1092,9 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
       active_cache[ci][si] = active;
     }
     const double waves = (double)((heads + active - 1) / active);
-    const double cost = waves * (37000.0 + 6.0 * lc);
+    // cycles per wave, measured at cfg 4 (profiles/): the one-pass bucket path where the slice allows it, else the general one
+    const bool fast_ok = lc <= kFastMaxE * ST && !(flags & NACL_FLAG_SELECT_GENERAL);
+    const double cost = waves * (fast_ok ? 20000.0 + 4.0 * lc : 37000.0 + 6.0 * lc);
     if (n == 0 || cost < best) { n = c; Lc = lc; dyn = d; best = cost; }
   }
   if (n == 0) return cudaErrorInvalidConfiguration;
@@ -724,10 +1106,23 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
     const long long epv = 16 / layout->esize;
     ly = KvVecLayout{layout->kv_sb / epv, layout->kv_sh / epv, layout->kv_sr / epv, layout->o_sb / epv, layout->o_sh / epv, layout->o_sr / epv};
   }
+  // fast path: bucket windows around the row mean of the importance (its sum over a row is known: G*P) and around the
+  // logarithm of that mean for the sampling keys (uniform weights: ln w = 0; weight exp(imp): ln w = imp)
+  int fast = (Lc <= kFastMaxE * ST && !(flags & NACL_FLAG_SELECT_GENERAL) && imp_mean > 0.f && imp_mean < 1e30f) ? 1 : 0;
+  int imp_base = 0;
+  float key_lo = 0.f;
+  if (fast) {
+    uint32_t mb;
+    memcpy(&mb, &imp_mean, sizeof(mb));
+    imp_base = (int)((mb | 0x80000000u) >> kImpShift) - HB / 2;
+    const float centre = (flags & NACL_FLAG_SAMPLE_UNIFORM) ? 0.f : ((flags & NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE) ? imp_mean : logf(imp_mean));
+    key_lo = centre - kKeyBelow;
+  }
   StageScope sc(ST_SELECT, st);
   return cudaLaunchKernelEx(&cfg, nacl_select_cluster_kernel, imp, Hkv, L, Lc, k1, budget_random, n_sink, n_recent, C, sk0, sk1,
                             (uint32_t)layer, flags, out_idx, (const int4*)K, (const int4*)V, (int4*)out_K, (int4*)out_V,
-                            (*gathered = (K != nullptr)) ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset, ly);
+                            (*gathered = (K != nullptr)) ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset, ly,
+                            fast, imp_base, key_lo);
 }
 
 // 4-byte words of the `key` scratch the select needs (long-row path: the keys)
@@ -738,7 +1133,24 @@ size_t select_scratch_words(int batch, int Hkv, int L) {
 
 }  // namespace nacl
 
+extern "C" __attribute__((visibility("default"))) int nacl_select_fallbacks(int reset) {
+  int v = 0;
+  if (cudaMemcpyFromSymbol(&v, nacl::g_select_fallbacks, sizeof(v)) != cudaSuccess) { cudaGetLastError(); return NACL_ERR_CUDA; }
+  if (reset) {
+    const int zero = 0;
+    if (cudaMemcpyToSymbol(nacl::g_select_fallbacks, &zero, sizeof(zero)) != cudaSuccess) { cudaGetLastError(); return NACL_ERR_CUDA; }
+  }
+  return v;
+}
+
 #ifdef NACL_SEL_TRACE
+extern "C" __attribute__((visibility("default"))) int nacl_debug_sel_trace_reset() {
+  static long long zeros[16 + 2 * 1024] = {};
+  return (int)cudaMemcpyToSymbol(nacl::g_sel_trace, zeros, sizeof(zeros));
+}
+extern "C" __attribute__((visibility("default"))) int nacl_debug_sel_trace2_read(long long* host) {
+  return (int)cudaMemcpyFromSymbol(host, nacl::g_sel_trace2, sizeof(nacl::g_sel_trace2));
+}
 extern "C" __attribute__((visibility("default"))) int nacl_debug_sel_trace_read(long long* host) {
   return (int)cudaMemcpyFromSymbol(host, nacl::g_sel_trace, sizeof(nacl::g_sel_trace));
 }

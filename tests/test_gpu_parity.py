@@ -95,6 +95,56 @@ def test_fused_scoring_launch_matches_two_launches(binding):
     full_parity(K, V, Q, Bp, Br, 4, P, seed=3, layer=1)
 
 
+FAST_CASES = [
+    # B, L, Hq, Hkv, d, P, dtype, Bp, Br, n_sink, n_recent, flags
+    (1, 32768, 8, 2, 128, 64, "bf16", 4915, 1638, 4, 64, 0),        # a cfg-4 head shape: clusters of 4, 8192 positions per CTA
+    (2, 16384, 4, 4, 128, 32, "bf16", 2457, 819, 4, 32, 0),
+    (1, 4096, 8, 8, 128, 32, "bf16", 614, 205, 4, 32, 0),
+    (1, 9000, 8, 2, 128, 16, "bf16", 1800, 450, 4, 16, 2),           # weight exp(importance)
+    (1, 9000, 8, 2, 128, 16, "bf16", 1800, 450, 4, 16, 4),           # uniform weights
+    (2, 3001, 4, 2, 64, 8, "f32", 500, 333, 3, 8, 0),                # CUDA-core scoring, ragged slices
+    (1, 5000, 4, 4, 128, 16, "bf16", 4000, 900, 4, 16, 0),           # almost everything kept
+    (1, 5000, 4, 4, 128, 16, "bf16", 21, 1, 4, 16, 0),               # one top-k element, one sample
+    (1, 5000, 4, 4, 128, 16, "bf16", 20, 300, 4, 16, 0),             # no top-k at all
+    (1, 131072, 4, 1, 128, 64, "bf16", 10485, 2622, 4, 64, 0),       # a cfg-5 head: cluster of 16
+    (1, 131072, 8, 8, 128, 8, "bf16", 10485, 2622, 4, 64, 0),        # cfg-5 rows on 8 heads: 16 positions per thread
+    (1, 70000, 6, 6, 128, 16, "bf16", 9000, 3000, 4, 16, 0),
+]
+
+
+@pytest.mark.parametrize("case", FAST_CASES, ids=lambda c: f"B{c[0]}_L{c[1]}_H{c[2]}-{c[3]}_P{c[5]}_{c[6]}_Bp{c[7]}_Br{c[8]}_f{c[11]}")
+def test_fast_selection_matches_general_path(binding, case):
+    """The one-pass bucket selection (windowed buckets for the top-k, fp32 key estimates + exact keys next to the
+    threshold for the sample) takes the same decisions as the three-pass radix path on exact keys, bit for bit, and as
+    the oracle's steps 4-7 on the same importance; on these shapes it must not fall back."""
+    B, L, Hq, Hkv, d, P, dt, Bp, Br, ns, nr, flags = case
+    K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype=dt, seed=L + Bp)
+    Kc, Vc, Qc = K.cuda(), V.cuda(), Q.cuda()
+    binding.nacl_select_fallbacks(reset=True)
+    a = binding.nacl_evict_ex(Kc, Vc, Qc, Bp, Br, ns, nr, 77, 5, flags=flags, want_importance=True)
+    torch.cuda.synchronize()
+    assert binding.nacl_select_fallbacks(reset=True) == 0, "the fast selection path fell back to the general one"
+    b = binding.nacl_evict_ex(Kc, Vc, Qc, Bp, Br, ns, nr, 77, 5, flags=flags | binding.FLAG_SELECT_GENERAL, want_importance=True)
+    for k in ("importance", "out_idx", "out_K", "out_V"):
+        assert torch.equal(a[k], b[k]), f"{k} differs between the fast and the general selection"
+    ref = oracle.select(a["importance"].cpu().numpy(), Bp, Br, ns, nr, 77, 5, flags=flags)
+    np.testing.assert_array_equal(a["out_idx"].cpu().numpy(), ref)
+
+
+def test_fast_selection_falls_back_on_degenerate_rows(binding):
+    """All-equal importance (every top-k decision is a tie: the threshold bucket holds the whole row), rows that are mostly
+    zero importance (keys of -inf), and protected positions marked +inf: the fast path must give up or handle them, with
+    the oracle's result either way."""
+    K, V, Q = make_random_inputs(1, 20000, 4, 2, 128, 8, dtype="bf16", seed=3)
+    K[:] = K[:, :, :1, :]
+    full_parity(K, V, Q, 3000, 1000, 2, 8, seed=1, layer=0)
+    K2, V2, Q2 = make_random_inputs(1, 6000, 2, 2, 128, 16, dtype="bf16", seed=11)
+    Q2[:] = Q2[:, :, :1, :]
+    K2[0, :, 100:130] = (300.0 * Q2[0, :, :1] / Q2[0, :, :1].float().norm(dim=-1, keepdim=True)).to(K2.dtype)
+    r = full_parity(K2, V2, Q2, 500, 400, 2, 16, seed=1, layer=0)
+    assert (r["imp_gpu"] == 0).sum() > 0
+
+
 def test_edge_budgets(binding):
     K, V, Q = make_random_inputs(1, 300, 4, 2, 64, 4, dtype="f32", seed=1)
     L = 300

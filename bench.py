@@ -295,8 +295,8 @@ def run_ours(args) -> dict:
         "hbm_frac_of_measured": round(value / world / peaks["hbm_gbs"], 4),
         "hbm_frac_of_nominal_8TBps": round(value / world / 8000.0, 4),
         "clocks": clocks, "e2e": e2e,
-        "gpu_launches": args.steps * layers * binding.nacl_launch_count(
-            1 if cfg.dtype == "bf16" else 0, cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P, args.nacl_flags),
+        # counted by the library itself: kernel launches recorded by the per-stage events over the same args.steps steps
+        "gpu_launches": int(sum(n for _, n in stages.values())),
         "roofline": roofline, "kernels": stage_rows,
         "ms_per_step_with_kernel_events": round(ms_total_prof / args.steps, 4),
         "lse_in_variant": {"what": "nacl_evict_ex with lse_in (row log-sum-exps supplied, single logit sweep; SURVEY.md 8(f) f1)",

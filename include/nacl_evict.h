@@ -91,6 +91,7 @@ extern "C" {
                                                 the tensor-core path applies */
 #define NACL_FLAG_SELECT_GENERAL 0x400u      /* debugging / profiling: the selection takes the general three-pass radix path even
                                                 where the one-pass bucket path applies (same result, bit for bit) */
+#define NACL_FLAG_GATHER_SEPARATE 0x800u     /* debugging / profiling: the K/V gather always runs as a kernel of its own */
 #define NACL_FLAG_SCORE_TWO_LAUNCHES 0x200u  /* debugging / profiling: the tensor-core path runs its statistics sweep and its
                                                 column-sum sweep as two launches instead of one cooperative launch */
 

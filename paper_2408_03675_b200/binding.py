@@ -16,7 +16,7 @@ from . import build as _build
 
 NACL_DTYPE_F32, NACL_DTYPE_BF16 = 0, 1
 FLAG_CAUSAL, FLAG_SAMPLE_SOFTMAX_OF_SCORE, FLAG_SAMPLE_UNIFORM, FLAG_SHARED_HEADS, FLAG_SCORE_CUDA_CORES = 1, 2, 4, 8, 0x100
-FLAG_SCORE_TWO_LAUNCHES, FLAG_SELECT_GENERAL = 0x200, 0x400
+FLAG_SCORE_TWO_LAUNCHES, FLAG_SELECT_GENERAL, FLAG_GATHER_SEPARATE = 0x200, 0x400, 0x800
 
 EXPORTS = ("nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes",
            "nacl_launch_count", "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version",

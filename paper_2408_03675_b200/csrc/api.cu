@@ -189,7 +189,7 @@ static int evict_impl(const nacl_params_t& p) {
   if (p.n_protect > 0 && !p.protect_idx) return NACL_ERR_NULL;
   if (p.reserved0 != 0) return NACL_ERR_UNSUPPORTED;
   const uint32_t known = NACL_FLAG_CAUSAL | NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE | NACL_FLAG_SAMPLE_UNIFORM | NACL_FLAG_SHARED_HEADS |
-                         NACL_FLAG_SCORE_CUDA_CORES | NACL_FLAG_SCORE_TWO_LAUNCHES | NACL_FLAG_SELECT_GENERAL;
+                         NACL_FLAG_SCORE_CUDA_CORES | NACL_FLAG_SCORE_TWO_LAUNCHES | NACL_FLAG_SELECT_GENERAL | NACL_FLAG_GATHER_SEPARATE;
   if (p.flags & ~known) return NACL_ERR_UNSUPPORTED;
   if ((p.flags & NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE) && (p.flags & NACL_FLAG_SAMPLE_UNIFORM)) return NACL_ERR_UNSUPPORTED;
 

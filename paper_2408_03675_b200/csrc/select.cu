@@ -1118,10 +1118,13 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
     const float centre = (flags & NACL_FLAG_SAMPLE_UNIFORM) ? 0.f : ((flags & NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE) ? imp_mean : logf(imp_mean));
     key_lo = centre - kKeyBelow;
   }
+  // the kernel also moves the kept rows when its grid covers most of the GPU; a grid of few CTAs (few heads, short rows)
+  // would leave the gather to a fraction of the SMs: the stand-alone gather kernel (all SMs) follows instead
+  *gathered = K != nullptr && !(flags & NACL_FLAG_GATHER_SEPARATE) && heads * n * 5 >= (long)kNumSMs * 4;
   StageScope sc(ST_SELECT, st);
   return cudaLaunchKernelEx(&cfg, nacl_select_cluster_kernel, imp, Hkv, L, Lc, k1, budget_random, n_sink, n_recent, C, sk0, sk1,
                             (uint32_t)layer, flags, out_idx, (const int4*)K, (const int4*)V, (int4*)out_K, (int4*)out_V,
-                            (*gathered = (K != nullptr)) ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset, ly,
+                            *gathered ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset, ly,
                             fast, imp_base, key_lo);
 }
 

@@ -209,10 +209,33 @@ def run_ours(args) -> dict:
 
     for _ in range(max(args.warmup, 3)):
         step()
+    # The timed step is ONE CUDA-graph launch of the step's calls (the library only enqueues: every call is capturable with
+    # a caller workspace); the same calls launched one by one from Python are timed beside it (ms_per_step_eager).
+    eager_step = step
+    graph = None
+    if not args.no_graph:
+        cap = torch.cuda.Stream(dev)
+        cap.wait_stream(stream)
+        with torch.cuda.stream(cap):
+            graph = torch.cuda.CUDAGraph()
+            outer_stream, stream = stream, cap
+            with torch.cuda.graph(graph, stream=cap):
+                eager_step()
+            stream = outer_stream
+        stream.wait_stream(cap)
+        torch.cuda.synchronize(dev)
+
+        def step():
+            graph.replay()
+
+        for _ in range(max(args.warmup, 3)):
+            step()
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
     ms_total = timed(args.steps)
+    step = eager_step
+    ms_total_eager = timed(args.steps) if graph is not None else ms_total
     # the same region again with per-kernel events (include/nacl_evict.h nacl_profile_*), for the roofline
     binding.nacl_profile_enable(True)
     binding.nacl_profile_read(reset=True)
@@ -298,6 +321,7 @@ def run_ours(args) -> dict:
         # counted by the library itself: kernel launches recorded by the per-stage events over the same args.steps steps
         "gpu_launches": int(sum(n for _, n in stages.values())),
         "roofline": roofline, "kernels": stage_rows,
+        "ms_per_step_eager": round(ms_total_eager / args.steps, 4),
         "ms_per_step_with_kernel_events": round(ms_total_prof / args.steps, 4),
         "lse_in_variant": {"what": "nacl_evict_ex with lse_in (row log-sum-exps supplied, single logit sweep; SURVEY.md 8(f) f1)",
                            "ms_per_step": round(ms_lse, 4), "us_per_layer": round(ms_lse * 1e3 / layers, 2),
@@ -305,6 +329,7 @@ def run_ours(args) -> dict:
                            "hbm_frac_of_measured": round(alg_bytes_step / world / (ms_lse * 1e-3) / 1e9 / peaks["hbm_gbs"], 4)},
         "library": os.path.relpath(binding.library_path(), ROOT),
     }
+    out["config"]["launch"] = "one CUDA-graph launch per step" if graph is not None else "one C-ABI call per layer from Python"
     if rank == 0 and world == 1 and not args.no_other_workloads:
         del data, lses
         torch.cuda.empty_cache()
@@ -482,6 +507,7 @@ def main() -> int:
     ap.add_argument("--config", type=int, default=4, choices=sorted(CONFIGS))
     ap.add_argument("--layers", type=int, default=0, help="override the number of layers per step (0 = the workload's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="time the step's calls launched one by one instead of one CUDA-graph launch")
     ap.add_argument("--nacl-flags", type=lambda v: int(v, 0), default=0,
                     help="NACL_FLAG_* bits for the timed calls (profiling: 0x200 = the two scoring sweeps as two launches)")
     ap.add_argument("--no-other-workloads", action="store_true", help="skip the short runs of the other BASELINE.json configs")

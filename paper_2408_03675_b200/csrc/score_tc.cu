@@ -1187,8 +1187,11 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
     const cuuint64_t strides[3] = {(cuuint64_t)s.kv_sr * 2, (cuuint64_t)s.kv_sh * 2, (cuuint64_t)s.kv_sb * 2};
     const cuuint32_t box[4] = {64, (cuuint32_t)TILE, 1, 1};
     const cuuint32_t es[4] = {1, 1, 1, 1};
+#ifndef NACL_K_L2PROMO
+#define NACL_K_L2PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+#endif
     if (enc(&tmK, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(K), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            CU_TENSOR_MAP_SWIZZLE_128B, NACL_K_L2PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
   }
   {
@@ -1212,8 +1215,11 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
   p.part = ws.part; p.lse_in = lse_in; p.lse_out = lse_out; p.imp = ws.imp; p.imp_out = imp_out;
   p.sync = ws.sync;
 
-  if (qrows == 128) return launch_cfg<128, 2, 5, 3>(tmK, tmQ, p, two_launches, st);
-  return launch_cfg<256, 1, 5, 3>(tmK, tmQ, p, two_launches, st);
+#ifndef NACL_STAGES_S
+#define NACL_STAGES_S 5
+#endif
+  if (qrows == 128) return launch_cfg<128, 2, NACL_STAGES_S, 3>(tmK, tmQ, p, two_launches, st);
+  return launch_cfg<256, 1, NACL_STAGES_S, 3>(tmK, tmQ, p, two_launches, st);
 }
 
 }  // namespace nacl

@@ -15,6 +15,7 @@
 //                  candidates that survive the top-k.  Used whenever the slices fit; 8x more CTAs than heads.
 // Integer work only after the keys: results are bit-exact functions of (imp, key).
 #include <cooperative_groups.h>
+#include <mutex>
 #include <math.h>
 #include <string.h>
 
@@ -660,7 +661,8 @@ template <int FE>
 __device__ bool select_fast(const float* __restrict__ row, int nloc, int E, int j0, int lo, int hi, int k1, int Br, int C,
                             int imp_base, float key_lo, uint32_t hk_g, uint32_t b_g, uint32_t layer, uint32_t sk0, uint32_t sk1,
                             uint32_t flags, ClShared& sh, uint32_t* ib, uint32_t* kb, uint2* list, cg::cluster_group& cluster,
-                            int32_t* __restrict__ out, int& tot_out, int& base_out) {
+                            int32_t* __restrict__ out, int& tot_out, int& base_out, const int4* pf_K, const int4* pf_V,
+                            size_t pf_src0, long long pf_sr, uint32_t pf_bytes) {
   const unsigned rank = cluster.block_rank(), nrank = cluster.num_blocks();
   // thread t owns the E = ceil(Lc / ST) <= FE consecutive positions from i0 = t * E on (short slices spread over all threads)
   const int t = (int)threadIdx.x, i0 = t * E;
@@ -729,6 +731,18 @@ __device__ bool select_fast(const float* __restrict__ row, int nloc, int E, int 
   }
   auto in_topk = [&](uint32_t val, int j) { return val > thr_p || (val == thr_p && j <= cut_p); };
   STAMP(2)
+  // Three quarters of the rows that will be gathered are known now (protected + top-k): their K and V rows are prefetched
+  // into L2 (one bulk prefetch per row) while the SMs work on the sampling keys and HBM would otherwise sit idle; the
+  // gather at the end of the kernel then reads them from L2.
+  if (pf_bytes > 0) {
+#pragma unroll
+    for (int e = 0; e < FE; ++e)
+      if (((livem >> e) & 1u) && (!((freem >> e) & 1u) || in_topk(v[e], j0 + i0 + e))) {
+        const size_t off = pf_src0 + (size_t)(j0 + i0 + e) * (size_t)pf_sr;
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(pf_K + off), "r"(pf_bytes) : "memory");
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(pf_V + off), "r"(pf_bytes) : "memory");
+      }
+  }
 
   // ---- a5: Gumbel-top-Br over the remaining candidates
   int kbin = -1;                 // bucket of the Br-th largest key estimate
@@ -877,12 +891,15 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
   if (fast) {
     uint2* list = reinterpret_cast<uint2*>(dyn + 2 * (size_t)Lc);
     const int E = (Lc + ST - 1) / ST;
+    // rows to prefetch for the fused gather (16-byte vectors; nothing when the gather is not fused)
+    const size_t pf0 = (size_t)(b * ly.sb + hk * ly.sh);
+    const uint32_t pfb = (uint32_t)vpr * 16u;
     if (E <= 8)
       done = select_fast<8>(row, nloc, E, j0, lo, hi, k1, Br, C, imp_base, key_lo, (uint32_t)hk + h_off, (uint32_t)b + b_off, layer, sk0,
-                            sk1, flags, sh, ib, kb, list, cluster, out, tot, base);
+                            sk1, flags, sh, ib, kb, list, cluster, out, tot, base, Kv, Vv, pf0, ly.sr, pfb);
     else
       done = select_fast<16>(row, nloc, E, j0, lo, hi, k1, Br, C, imp_base, key_lo, (uint32_t)hk + h_off, (uint32_t)b + b_off, layer, sk0,
-                             sk1, flags, sh, ib, kb, list, cluster, out, tot, base);
+                             sk1, flags, sh, ib, kb, list, cluster, out, tot, base, Kv, Vv, pf0, ly.sr, pfb);
   }
   if (!done) {
   if (fast && rank == 0 && threadIdx.x == 0) atomicAdd(&g_select_fallbacks, 1);
@@ -1038,8 +1055,9 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   if (C == 0) return cudaSuccess;
   const int k1 = budget_proxy - n_sink - n_recent;
   const uint32_t sk0 = (uint32_t)(seed & 0xFFFFFFFFu), sk1 = (uint32_t)(seed >> 32);
-  if (!select_uses_cluster(L)) {
-    // very long rows: sampling keys in a kernel of their own, one CTA per head working out of global memory
+  // very long rows, or no cluster size that this device can co-schedule: sampling keys in a kernel of their own, one CTA
+  // per head working out of global memory (the caller then runs the stand-alone gather)
+  auto long_row_path = [&]() -> cudaError_t {
     if (budget_random > 0) {
       StageScope sc(ST_KEYS, st);
       cudaError_t e = launch_keys(imp, key, batch, Hkv, L, seed, layer, flags, true, batch_offset, head_offset, st);
@@ -1048,7 +1066,8 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
     StageScope sc(ST_SELECT, st);
     nacl_select_kernel<<<batch * Hkv, ST, 0, st>>>(imp, key, L, k1, budget_random, n_sink, n_recent, C, out_idx);
     return cudaGetLastError();
-  }
+  };
+  if (!select_uses_cluster(L)) return long_row_path();
   // cluster size n: the n that minimises (waves of co-resident clusters) x (per-CTA cost ~ fixed + per-position),
   // with the co-residency limit asked from the runtime (clusters need n free SMs inside one GPC)
   cudaLaunchConfig_t cfg = {};
@@ -1061,6 +1080,8 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   const long heads = (long)batch * Hkv;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); dev = 0; }
   int n = 0, Lc = 0;
   size_t dyn = 0;
   double best = 0.0;
@@ -1078,26 +1099,34 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
     if (lc > kMaxSlice) continue;
     if (c > 1 && L / c < ST / 2) break;  // slices below half a block of positions are not worth a barrier per pass
     const size_t d = dyn_bytes(lc);
-    static int active_cache[5][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}, {0, 0}};  // [log2 c][smem class]: co-resident clusters
+    // co-resident clusters of this size, per device and shared-memory class; -1: the device cannot schedule one (a MIG
+    // slice, another SKU): the size is skipped
+    static std::mutex cache_mu;
+    static int active_cache[64][5][2] = {};
     const int ci = c == 1 ? 0 : (c == 2 ? 1 : (c == 4 ? 2 : (c == 8 ? 3 : 4))), si = d > 100 * 1024 ? 1 : 0;
-    int active = active_cache[ci][si];
-    if (active == 0) {
-      cfg.gridDim = dim3((unsigned)(c * 64));
-      cfg.dynamicSmemBytes = si ? sizeof(ClShared) + (size_t)kMaxSlice * 2 * sizeof(uint32_t) : 100 * 1024;
-      attr[0].val.clusterDim.x = (unsigned)c;
-      if (cudaOccupancyMaxActiveClusters(&active, nacl_select_cluster_kernel, &cfg) != cudaSuccess || active < 1) {
-        cudaGetLastError();
-        active = kNumSMs / c / 2;  // conservative guess
+    int active;
+    {
+      std::lock_guard<std::mutex> lk(cache_mu);
+      active = active_cache[dev][ci][si];
+      if (active == 0) {
+        cfg.gridDim = dim3((unsigned)(c * 64));
+        cfg.dynamicSmemBytes = si ? sizeof(ClShared) + (size_t)kMaxSlice * 2 * sizeof(uint32_t) : 100 * 1024;
+        attr[0].val.clusterDim.x = (unsigned)c;
+        if (cudaOccupancyMaxActiveClusters(&active, nacl_select_cluster_kernel, &cfg) != cudaSuccess || active < 1) {
+          cudaGetLastError();
+          active = -1;
+        }
+        active_cache[dev][ci][si] = active;
       }
-      active_cache[ci][si] = active;
     }
+    if (active < 1) continue;
     const double waves = (double)((heads + active - 1) / active);
     // cycles per wave, measured at cfg 4 (profiles/): the one-pass bucket path where the slice allows it, else the general one
     const bool fast_ok = lc <= kFastMaxE * ST && !(flags & NACL_FLAG_SELECT_GENERAL);
     const double cost = waves * (fast_ok ? 20000.0 + 4.0 * lc : 37000.0 + 6.0 * lc);
     if (n == 0 || cost < best) { n = c; Lc = lc; dyn = d; best = cost; }
   }
-  if (n == 0) return cudaErrorInvalidConfiguration;
+  if (n == 0) return long_row_path();
   cfg.gridDim = dim3((unsigned)(heads * n));
   cfg.dynamicSmemBytes = dyn;
   attr[0].val.clusterDim.x = (unsigned)n;
@@ -1121,17 +1150,24 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   // the kernel also moves the kept rows when its grid covers most of the GPU; a grid of few CTAs (few heads, short rows)
   // would leave the gather to a fraction of the SMs: the stand-alone gather kernel (all SMs) follows instead
   *gathered = K != nullptr && !(flags & NACL_FLAG_GATHER_SEPARATE) && heads * n * 5 >= (long)kNumSMs * 4;
-  StageScope sc(ST_SELECT, st);
-  return cudaLaunchKernelEx(&cfg, nacl_select_cluster_kernel, imp, Hkv, L, Lc, k1, budget_random, n_sink, n_recent, C, sk0, sk1,
-                            (uint32_t)layer, flags, out_idx, (const int4*)K, (const int4*)V, (int4*)out_K, (int4*)out_V,
-                            *gathered ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset, ly,
-                            fast, imp_base, key_lo);
+  {
+    StageScope sc(ST_SELECT, st);
+    e = cudaLaunchKernelEx(&cfg, nacl_select_cluster_kernel, imp, Hkv, L, Lc, k1, budget_random, n_sink, n_recent, C, sk0, sk1,
+                           (uint32_t)layer, flags, out_idx, (const int4*)K, (const int4*)V, (int4*)out_K, (int4*)out_V,
+                           *gathered ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset, ly, fast, imp_base, key_lo);
+  }
+  if (e == cudaSuccess) return e;
+  // the launch itself was refused (cluster resources): nothing ran; take the path without clusters
+  cudaGetLastError();
+  *gathered = false;
+  return long_row_path();
 }
 
 // 4-byte words of the `key` scratch the select needs (long-row path: the keys)
 size_t select_scratch_words(int batch, int Hkv, int L) {
-  if (!select_uses_cluster(L)) return (size_t)batch * Hkv * L;
-  return 64;  // the cluster path keeps everything in shared memory
+  // the keys of the path without clusters (very long rows, or a device that cannot co-schedule a cluster); the cluster
+  // path keeps everything in shared memory
+  return (size_t)batch * Hkv * L + 64;
 }
 
 }  // namespace nacl

@@ -661,8 +661,7 @@ template <int FE>
 __device__ bool select_fast(const float* __restrict__ row, int nloc, int E, int j0, int lo, int hi, int k1, int Br, int C,
                             int imp_base, float key_lo, uint32_t hk_g, uint32_t b_g, uint32_t layer, uint32_t sk0, uint32_t sk1,
                             uint32_t flags, ClShared& sh, uint32_t* ib, uint32_t* kb, uint2* list, cg::cluster_group& cluster,
-                            int32_t* __restrict__ out, int& tot_out, int& base_out, const int4* pf_K, const int4* pf_V,
-                            size_t pf_src0, long long pf_sr, uint32_t pf_bytes) {
+                            int32_t* __restrict__ out, int& tot_out, int& base_out) {
   const unsigned rank = cluster.block_rank(), nrank = cluster.num_blocks();
   // thread t owns the E = ceil(Lc / ST) <= FE consecutive positions from i0 = t * E on (short slices spread over all threads)
   const int t = (int)threadIdx.x, i0 = t * E;
@@ -731,19 +730,6 @@ __device__ bool select_fast(const float* __restrict__ row, int nloc, int E, int 
   }
   auto in_topk = [&](uint32_t val, int j) { return val > thr_p || (val == thr_p && j <= cut_p); };
   STAMP(2)
-  // Three quarters of the rows that will be gathered are known now (protected + top-k): their K and V rows are prefetched
-  // into L2 (one bulk prefetch per row) while the SMs work on the sampling keys and HBM would otherwise sit idle; the
-  // gather at the end of the kernel then reads them from L2.
-  if (pf_bytes > 0) {
-#pragma unroll
-    for (int e = 0; e < FE; ++e)
-      if (((livem >> e) & 1u) && (!((freem >> e) & 1u) || in_topk(v[e], j0 + i0 + e))) {
-        const size_t off = pf_src0 + (size_t)(j0 + i0 + e) * (size_t)pf_sr;
-        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(pf_K + off), "r"(pf_bytes) : "memory");
-        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(pf_V + off), "r"(pf_bytes) : "memory");
-      }
-  }
-
   // ---- a5: Gumbel-top-Br over the remaining candidates
   int kbin = -1;                 // bucket of the Br-th largest key estimate
   uint32_t thr_r = 0xFFFFFFFFu;  // exact threshold among the candidates of buckets kbin-1 .. kbin+1
@@ -891,15 +877,12 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
   if (fast) {
     uint2* list = reinterpret_cast<uint2*>(dyn + 2 * (size_t)Lc);
     const int E = (Lc + ST - 1) / ST;
-    // rows to prefetch for the fused gather (16-byte vectors; nothing when the gather is not fused)
-    const size_t pf0 = (size_t)(b * ly.sb + hk * ly.sh);
-    const uint32_t pfb = (uint32_t)vpr * 16u;
     if (E <= 8)
       done = select_fast<8>(row, nloc, E, j0, lo, hi, k1, Br, C, imp_base, key_lo, (uint32_t)hk + h_off, (uint32_t)b + b_off, layer, sk0,
-                            sk1, flags, sh, ib, kb, list, cluster, out, tot, base, Kv, Vv, pf0, ly.sr, pfb);
+                            sk1, flags, sh, ib, kb, list, cluster, out, tot, base);
     else
       done = select_fast<16>(row, nloc, E, j0, lo, hi, k1, Br, C, imp_base, key_lo, (uint32_t)hk + h_off, (uint32_t)b + b_off, layer, sk0,
-                             sk1, flags, sh, ib, kb, list, cluster, out, tot, base, Kv, Vv, pf0, ly.sr, pfb);
+                             sk1, flags, sh, ib, kb, list, cluster, out, tot, base);
   }
   if (!done) {
   if (fast && rank == 0 && threadIdx.x == 0) atomicAdd(&g_select_fallbacks, 1);

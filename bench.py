@@ -151,15 +151,16 @@ def load_traffic(cfg_name: str, kernel: str):
     """dram bytes (read + write) per launch of `kernel` from the committed ncu --set full summary
     (profiles/traffic.csv: workload,kernel,dram_bytes_per_launch,source), if one exists."""
     path = os.path.join(ROOT, "profiles", "traffic.csv")
+    found = None
     try:
         with open(path) as f:
             for line in f:
                 c = [x.strip() for x in line.split(",")]
                 if len(c) >= 3 and c[0] == cfg_name and c[1] == kernel:
-                    return int(float(c[2]))
+                    found = int(float(c[2]))  # later lines are later captures
     except (OSError, ValueError):
         pass
-    return None
+    return found
 
 
 def run_ours(args) -> dict:
@@ -241,6 +242,14 @@ def run_ours(args) -> dict:
     binding.nacl_profile_read(reset=True)
     ms_total_prof = timed(args.steps)
     stages = binding.nacl_profile_read(reset=True)
+    # the two scoring sweeps as two launches (NACL_FLAG_SCORE_TWO_LAUNCHES), for the per-sweep times of the fused launch
+    fused_flags = args.nacl_flags
+    args.nacl_flags = fused_flags | 0x200
+    step()
+    binding.nacl_profile_read(reset=True)
+    timed(max(1, args.steps // 4))
+    stages_two = binding.nacl_profile_read(reset=True)
+    args.nacl_flags = fused_flags
     binding.nacl_profile_enable(False)
     clocks = sampler.stop() if rank == 0 else None
 
@@ -321,6 +330,9 @@ def run_ours(args) -> dict:
         # counted by the library itself: kernel launches recorded by the per-stage events over the same args.steps steps
         "gpu_launches": int(sum(n for _, n in stages.values())),
         "roofline": roofline, "kernels": stage_rows,
+        "kernels_two_scoring_launches": {name: {"launches": n, "avg_us": round(ms / n * 1e3, 2),
+                                                "alg_GBps": round(sab.get(name, 0) / (ms / n * 1e-3) / 1e9, 1)}
+                                         for name, (ms, n) in stages_two.items() if n},
         "ms_per_step_eager": round(ms_total_eager / args.steps, 4),
         "ms_per_step_with_kernel_events": round(ms_total_prof / args.steps, 4),
         "lse_in_variant": {"what": "nacl_evict_ex with lse_in (row log-sum-exps supplied, single logit sweep; SURVEY.md 8(f) f1)",

@@ -679,17 +679,16 @@ __device__ bool select_fast(const float* __restrict__ row, int nloc, int E, int 
     livem |= (live ? 1u : 0u) << e;
     freem |= (live && free_pos(i0 + e) ? 1u : 0u) << e;
   }
-  cluster.sync();  // every CTA of the cluster is running: its shared memory may be written
   STAMP(1)
 
   // ---- a4: top-k1 of the importance outside the protected set
   uint32_t thr_p = 0xFFFFFFFFu;
   int cut_p = -1;
+  uint32_t inb = 0;  // bit e: in the threshold bucket (after the find)
+  int dg[FE];
   if (k1 > 0) {
     for (int i = t; i < HB; i += ST) sh.hist[i] = 0;
     __syncthreads();
-    uint32_t inb = 0;  // bit e: in the threshold bucket (after the find)
-    int dg[FE];
 #pragma unroll
     for (int e = 0; e < FE; ++e) {
       dg[e] = min(max((int)(v[e] >> kImpShift) - imp_base, 0), HB - 1);
@@ -698,6 +697,14 @@ __device__ bool select_fast(const float* __restrict__ row, int nloc, int E, int 
     }
     __syncthreads();
     FSTAMP(0)
+  }
+  // every CTA of the cluster is running (the barrier it arrived at when it started): its shared memory may be written
+#ifndef NACL_SEL_NO_SPLIT_BARRIER
+  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+#else
+  cluster.sync();
+#endif
+  if (k1 > 0) {
     fast_hist_find(sh, k1);
     FSTAMP(1)
     const int bin = sh.bin, krem = sh.krem;
@@ -875,6 +882,10 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
   STAMP(0)
   bool done = false;
   if (fast) {
+    // split cluster barrier: arrive now, wait right before the first write into another CTA's shared memory (select_fast)
+#ifndef NACL_SEL_NO_SPLIT_BARRIER
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+#endif
     uint2* list = reinterpret_cast<uint2*>(dyn + 2 * (size_t)Lc);
     const int E = (Lc + ST - 1) / ST;
     if (E <= 8)

@@ -367,7 +367,7 @@ struct Smem {
   static constexpr int OFF_KA = OFF_QA + (PH ? NQ * QA_BYTES : 0);
   static constexpr int OFF_CS = OFF_KA + (PH ? BOX_BYTES : 0);     // float[N_CS][4][128]: quarter column sums of a C tile
   static constexpr int OFF_BARS = OFF_CS + (PH ? N_CS * 4 * TILE * 4 : 0);
-  static constexpr int N_BARS = 2 * STAGES + 4 * NQ + 4 * N_BUFS + 2 * N_CS;
+  static constexpr int N_BARS = 2 * STAGES + 4 * NQ + 4 * N_BUFS + 2 * N_CS + 2;  // (+2: partials of a segment stored / counted)
   static constexpr int OFF_TMEM = OFF_BARS + N_BARS * 8;
   static constexpr int TOTAL = OFF_TMEM + 8;
 };
@@ -536,15 +536,7 @@ __device__ __noinline__ float c_cols_causal(uint32_t taddr, int nc, float sc, in
 }
 
 // ------------------------------------------------------------------ inter-CTA hand-over of the partials (fused launch)
-// Called by all epilogue threads after their partial stores (st.cg) of a segment: CTA barrier, then ONE thread makes the
-// stores visible at gpu scope and counts the piece (the pattern of a cooperative-groups grid barrier, per head).
-__device__ __forceinline__ void publish_piece(int* cnt) {
-  asm volatile("bar.sync 2, %0;" ::"n"(EPI_THREADS) : "memory");
-  if (threadIdx.x == 0) {
-    __threadfence();
-    atomicAdd(cnt, 1);
-  }
-}
+// Producer side (sweep S): see the publisher role in the kernel.
 // Called by all epilogue threads before they read the partials of a head: one thread polls until all `need` pieces are
 // published; the consumer that completes the head's `need` consumers zeroes both counters for the next launch.
 __device__ __forceinline__ void await_pieces(int* cnt, int* done, int need) {
@@ -579,7 +571,10 @@ __device__ __forceinline__ void sweep(const CUtensorMap& tmK, const CUtensorMap&
   const uint32_t bars = sbase + SM::OFF_BARS;
   constexpr int B_KE = STAGES, B_QF = 2 * STAGES, B_QE = B_QF + NQ, B_AF = B_QE + NQ, B_AE = B_AF + NQ, B_TF = B_AE + NQ,
                 B_TE = B_TF + 2 * N_BUFS, B_CF = B_TE + 2 * N_BUFS, B_CE = B_CF + N_CS;
-  static_assert(B_CE + N_CS == SM::N_BARS, "barrier count");
+  constexpr int B_PUB = B_CE + N_CS;
+  static_assert(B_PUB + 2 == SM::N_BARS, "barrier count");
+  // fused launch, sweep S: all epilogue warps have stored their partials of a segment / the publisher has taken note of it
+  const uint32_t pub_bar = bars + 8u * B_PUB, pub_done = bars + 8u * (B_PUB + 1);
   auto qa_full = [&](int s) { return bars + 8u * (B_AF + s); };   // sweep C: the segment's -lse/scale rows are in shared memory
   auto qa_empty = [&](int s) { return bars + 8u * (B_AE + s); };  // ... and every MMA that read them has completed
   auto k_full = [&](int s) { return bars + 8u * s; };
@@ -621,6 +616,8 @@ __device__ __forceinline__ void sweep(const CUtensorMap& tmK, const CUtensorMap&
         mbar_init(tm_empty(b, h), quad ? 4 : N_EPI_WARPS);  // epilogue warps that drain it
       }
     for (int b = 0; b < N_CS; ++b) { mbar_init(cs_full(b), quad ? N_EPI_WARPS / 2 : N_EPI_WARPS); mbar_init(cs_empty(b), 1); }
+    mbar_init(pub_bar, N_EPI_WARPS);
+    mbar_init(pub_done, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if constexpr (PH != 0) {
@@ -796,6 +793,26 @@ __device__ __forceinline__ void sweep(const CUtensorMap& tmK, const CUtensorMap&
     }
     __syncwarp();
   } else if (warp == W_CMB) {
+    // ================================================================ sweep S of the fused launch: publisher of the partials
+    // The epilogue warps only ARRIVE (mbarrier, release at CTA scope) once their partials of a segment are stored and go
+    // on with the next segment; this otherwise idle warp waits for the 16 arrivals (acquire), makes the stores visible at
+    // gpu scope and counts the piece.  (A __threadfence inside an epilogue warp stalled the accumulator hand-over for
+    // 3-9 k cycles at every head boundary under a saturated memory system: profiles/r2b_final_kernels.md.)
+    if constexpr (PH == 0 && FUSED) {
+      uint32_t nseg = 0;
+      Walk walk(p, PH);
+      Seg sg;
+      while (walk.next(sg)) {
+        mbar_wait(pub_bar, nseg & 1);
+        if (lane == 0) {
+          mbar_arrive(pub_done);
+          __threadfence();
+          atomicAdd(p.sync + sg.head, 1);
+        }
+        __syncwarp();
+        ++nseg;
+      }
+    }
     // ================================================================ column-sum combiner (sweep C only)
     if constexpr (PH != 0) {
       uint32_t ccount = 0;
@@ -901,7 +918,15 @@ __device__ __forceinline__ void sweep(const CUtensorMap& tmK, const CUtensorMap&
           }
           if (q_row < rows_in_block(sg.rb))
             __stcg(&p.part[(((size_t)blockIdx.x + sg.head) * p.n_slots + q_par) * p.rows_total + sg.rb * 256 + q_row], make_float2(m0, z0));
-          if constexpr (FUSED) publish_piece(p.sync + sg.head);
+          if constexpr (FUSED) {
+          // (a warp arrives for a segment only after the publisher has consumed the arrivals of the segment before it: the
+          // publisher can never be two phases behind, however short the segments are)
+          __syncwarp();
+          if (lane == 0) {
+            if (nseg > 0) mbar_wait(pub_done, (uint32_t)(nseg - 1) & 1u);
+            mbar_arrive(pub_bar);
+          }
+        }
           ecount += sg.n;
           ++nseg;
           continue;
@@ -929,7 +954,15 @@ __device__ __forceinline__ void sweep(const CUtensorMap& tmK, const CUtensorMap&
         // this warp's partial of the piece; (-inf, 0) when it saw no valid key
         if (s_row < p.rows)
           __stcg(&p.part[(((size_t)blockIdx.x + sg.head) * p.n_slots + s_slot) * p.rows_total + sg.rb * 256 + s_row], make_float2(m0, z0));
-        if constexpr (FUSED) publish_piece(p.sync + sg.head);
+        if constexpr (FUSED) {
+          // (a warp arrives for a segment only after the publisher has consumed the arrivals of the segment before it: the
+          // publisher can never be two phases behind, however short the segments are)
+          __syncwarp();
+          if (lane == 0) {
+            if (nseg > 0) mbar_wait(pub_done, (uint32_t)(nseg - 1) & 1u);
+            mbar_arrive(pub_bar);
+          }
+        }
       } else {
         // ---------------- C segment: merge the head's partials (ascending piece order) into lse, hand -lse/scale to the MMA
         // issuers as the operand of the ninth k-step (augmented contraction: the accumulator then holds s - lse/scale and

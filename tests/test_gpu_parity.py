@@ -145,6 +145,30 @@ def test_fast_selection_falls_back_on_degenerate_rows(binding):
     assert (r["imp_gpu"] == 0).sum() > 0
 
 
+def test_concurrent_streams_keep_their_results_apart(binding):
+    """Two streams evict different problems at the same time through the library's own (device, stream) workspaces: the
+    cooperative scoring launches serialise instead of deadlocking, the hand-over counters of one call never meet the other's."""
+    shapes = [(2, 6000, 16, 4, 128, 16), (1, 9000, 8, 8, 128, 32)]
+    data = []
+    for rep, (B, L, Hq, Hkv, d, P) in enumerate(shapes):
+        K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype="bf16", seed=40 + rep)
+        data.append((K.cuda(), V.cuda(), Q.cuda(), L // 5, L // 20, P))
+    want = [binding.nacl_evict_ex(K, V, Q, Bp, Br, 4, P, 9, 1) for K, V, Q, Bp, Br, P in data]
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    got = [[], []]
+    for it in range(6):
+        for si, st in enumerate(streams):
+            K, V, Q, Bp, Br, P = data[si]
+            with torch.cuda.stream(st):
+                got[si].append(binding.nacl_evict_ex(K, V, Q, Bp, Br, 4, P, 9, 1, stream=st))
+    torch.cuda.synchronize()
+    for si in range(2):
+        for r in got[si]:
+            for k in ("out_idx", "out_K", "out_V"):
+                assert torch.equal(r[k], want[si][k]), f"stream {si}: {k} differs from the single-stream result"
+
+
 def test_edge_budgets(binding):
     K, V, Q = make_random_inputs(1, 300, 4, 2, 64, 4, dtype="f32", seed=1)
     L = 300

@@ -205,6 +205,18 @@ typedef struct nacl_gen_params {
 } nacl_gen_params_t;
 int nacl_evict_generation(const nacl_gen_params_t* g);
 
+/* Variable-length batches ("compatible with FlashAttention": padded / varlen prompt batches).
+ * Batch element b holds seq_len[b] <= p->L live keys in the padded K/V [batch, Hkv, p->L, d] (or the strided layout p
+ * describes), its proxy queries Qproxy[b] are the last P positions of ITS prompt, and it keeps budget_proxy[b] +
+ * budget_random[b] <= C_max positions: rows 0 .. C_b-1 of its slices of out_K / out_V [batch, Hkv, C_max, d] (or the strided
+ * output layout of p; rows past C_b are left untouched) and, PACKED as [Hkv, C_b], the first Hkv*C_b entries of its slice
+ * out_idx[b*Hkv*C_max ...].  seq_len, budget_proxy, budget_random: HOST arrays of `batch` ints (read before the call
+ * returns); p->budget_proxy / p->budget_random are ignored.  Every element is evicted exactly as a batch-1 nacl_evict_ex call
+ * with batch_offset = p->batch_offset + b would evict it (same Philox streams), one after the other on p->stream.
+ * lse_in, out_importance, out_lse and protect_idx must be NULL.  Returns the first error, NACL_OK otherwise. */
+int nacl_evict_varlen(const nacl_params_t* p, const int32_t* seq_len, const int32_t* budget_proxy,
+                      const int32_t* budget_random, int C_max);
+
 /* Same operation with every tensor in HOST memory (pinned memory makes the copies
  * asynchronous).  Copies K, V, Qproxy to grow-only device staging buffers, runs steps 1-7
  * and copies out_K, out_V, out_idx back; returns after the results are in host memory.

@@ -21,7 +21,7 @@ FLAG_SCORE_TWO_LAUNCHES, FLAG_SELECT_GENERAL, FLAG_GATHER_SEPARATE = 0x200, 0x40
 EXPORTS = ("nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes",
            "nacl_launch_count", "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version",
            "nacl_profile_enable", "nacl_profile_read", "nacl_stage_name", "nacl_gumbel_keys", "nacl_evict_generation",
-           "nacl_select_fallbacks")
+           "nacl_select_fallbacks", "nacl_evict_varlen")
 N_STAGES = 7
 
 
@@ -94,6 +94,8 @@ def _load() -> C.CDLL:
     lib.nacl_release.restype = None
     lib.nacl_select_fallbacks.argtypes = [i32]
     lib.nacl_select_fallbacks.restype = i32
+    lib.nacl_evict_varlen.argtypes = [C.POINTER(NaclParams), C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32), i32]
+    lib.nacl_evict_varlen.restype = i32
     lib.nacl_strerror.argtypes = [i32]
     lib.nacl_strerror.restype = C.c_char_p
     lib.nacl_last_cuda_error.argtypes = []
@@ -273,6 +275,43 @@ def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, s
     if lse is not None:
         out["lse"] = lse
     return out
+
+
+def nacl_evict_varlen(K, V, Qproxy, seq_len, budget_proxy, budget_random, n_sink, n_recent, seed, layer, flags=0,
+                      workspace=None, stream=None, batch_offset=0, head_offset=0):
+    """include/nacl_evict.h `nacl_evict_varlen`: padded K/V [B,Hkv,L_max,d], Qproxy [B,Hq,P,d] (the last P positions of
+    every prompt), per-element lengths and budgets (Python ints).  Returns out_K / out_V [B,Hkv,C_max,d] (rows past an
+    element's own C untouched: zero here) and per element its packed index rows out_idx[b] [Hkv, C_b]."""
+    B, Hkv, L, d, Hq, P = _shapes(K, V, Qproxy)
+    if not K.is_cuda:
+        raise ValueError("nacl_evict_varlen takes CUDA tensors")
+    dev = K.device
+    Cs = [int(a) + int(b) for a, b in zip(budget_proxy, budget_random)]
+    C_max = max(Cs) if Cs else 0
+    out_K = torch.zeros((B, Hkv, C_max, d), dtype=K.dtype, device=dev)
+    out_V = torch.zeros_like(out_K)
+    idx_flat = torch.zeros((B, Hkv * C_max), dtype=torch.int32, device=dev)
+    p = NaclParams()
+    p.struct_size = C.sizeof(NaclParams)
+    p.dtype = _dtype_tag(K)
+    p.K, p.V, p.Qproxy = K.data_ptr(), V.data_ptr(), Qproxy.data_ptr()
+    p.batch, p.L, p.Hq, p.Hkv, p.d, p.P = B, L, Hq, Hkv, d, P
+    p.n_sink, p.n_recent = n_sink, n_recent
+    p.seed, p.layer, p.flags = seed, layer, flags
+    p.batch_offset, p.head_offset = batch_offset, head_offset
+    p.kv_stride_batch, p.kv_stride_head, p.kv_stride_row = _kv_strides(K)
+    p.out_K, p.out_V, p.out_idx = out_K.data_ptr(), out_V.data_ptr(), idx_flat.data_ptr()
+    if workspace is not None:
+        p.workspace, p.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
+    p.stream = (stream or torch.cuda.current_stream(dev)).cuda_stream
+    arr = C.c_int32 * B
+    with torch.cuda.device(dev):
+        rc = _lib.nacl_evict_varlen(C.byref(p), arr(*[int(v) for v in seq_len]), arr(*[int(v) for v in budget_proxy]),
+                                    arr(*[int(v) for v in budget_random]), C_max)
+    if rc != 0:
+        raise NaclError(rc, "nacl_evict_varlen")
+    out_idx = [idx_flat[b, :Hkv * Cs[b]].view(Hkv, Cs[b]) for b in range(B)]
+    return {"out_K": out_K, "out_V": out_V, "out_idx": out_idx, "C": Cs}
 
 
 def nacl_evict_generation(K_cache, V_cache, q, length, budget_proxy, budget_random, n_sink, n_recent, seed, layer, step,

@@ -378,6 +378,45 @@ int nacl_evict_generation(const nacl_gen_params_t* g) {
   return e == cudaSuccess ? NACL_OK : fail_cuda(e);
 }
 
+int nacl_evict_varlen(const nacl_params_t* p, const int32_t* seq_len, const int32_t* budget_proxy, const int32_t* budget_random,
+                      int C_max) {
+  if (!p || !seq_len || !budget_proxy || !budget_random) return NACL_ERR_NULL;
+  if (p->struct_size != sizeof(nacl_params_t)) return NACL_ERR_UNSUPPORTED;
+  if (p->lse_in || p->out_importance || p->out_lse || p->protect_idx || p->n_protect != 0) return NACL_ERR_UNSUPPORTED;
+  if (p->batch < 1 || p->L < 1 || p->Hkv < 1 || p->Hq < 1 || p->d < 1 || p->P < 1 || C_max < 0) return NACL_ERR_SHAPE;
+  const size_t esz = p->dtype == NACL_DTYPE_F32 ? 4 : 2;
+  // element strides of the padded tensors (all-zero = contiguous [batch, Hkv, L, d] / [batch, Hkv, C_max, d])
+  const bool kv0 = p->kv_stride_batch == 0 && p->kv_stride_head == 0 && p->kv_stride_row == 0;
+  const bool o0 = p->out_stride_batch == 0 && p->out_stride_head == 0 && p->out_stride_row == 0;
+  const int64_t kv_sr = kv0 ? p->d : p->kv_stride_row, kv_sh = kv0 ? (int64_t)p->L * p->d : p->kv_stride_head;
+  const int64_t kv_sb = kv0 ? (int64_t)p->Hkv * p->L * p->d : p->kv_stride_batch;
+  const int64_t o_sr = o0 ? p->d : p->out_stride_row, o_sh = o0 ? (int64_t)C_max * p->d : p->out_stride_head;
+  const int64_t o_sb = o0 ? (int64_t)p->Hkv * C_max * p->d : p->out_stride_batch;
+  for (int b = 0; b < p->batch; ++b) {
+    if (seq_len[b] < 1 || seq_len[b] > p->L) return NACL_ERR_SHAPE;
+    if (budget_proxy[b] < 0 || budget_random[b] < 0 || (long)budget_proxy[b] + budget_random[b] > C_max) return NACL_ERR_BUDGET;
+  }
+  for (int b = 0; b < p->batch; ++b) {
+    nacl_params_t q = *p;
+    q.batch = 1;
+    q.L = seq_len[b];
+    q.budget_proxy = budget_proxy[b];
+    q.budget_random = budget_random[b];
+    q.batch_offset = p->batch_offset + b;
+    q.K = static_cast<const char*>(p->K) + (size_t)b * kv_sb * esz;
+    q.V = static_cast<const char*>(p->V) + (size_t)b * kv_sb * esz;
+    q.Qproxy = static_cast<const char*>(p->Qproxy) + (size_t)b * p->Hq * p->P * p->d * esz;
+    q.out_K = p->out_K ? static_cast<char*>(p->out_K) + (size_t)b * o_sb * esz : nullptr;
+    q.out_V = p->out_V ? static_cast<char*>(p->out_V) + (size_t)b * o_sb * esz : nullptr;
+    q.out_idx = p->out_idx ? p->out_idx + (size_t)b * p->Hkv * C_max : nullptr;
+    q.kv_stride_row = kv_sr; q.kv_stride_head = kv_sh; q.kv_stride_batch = kv_sb;
+    q.out_stride_row = o_sr; q.out_stride_head = o_sh; q.out_stride_batch = o_sb;
+    const int rc = evict_impl(q);
+    if (rc != NACL_OK) return rc;
+  }
+  return NACL_OK;
+}
+
 int nacl_evict_host(const void* K, const void* V, const void* Qproxy, int dtype, int batch, int L, int Hq, int Hkv, int d,
                     int P, int budget_proxy, int budget_random, int n_sink, int n_recent, uint64_t seed, int layer,
                     void* out_K, void* out_V, int32_t* out_idx, int device) {

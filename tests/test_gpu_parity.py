@@ -169,6 +169,35 @@ def test_concurrent_streams_keep_their_results_apart(binding):
                 assert torch.equal(r[k], want[si][k]), f"stream {si}: {k} differs from the single-stream result"
 
 
+@pytest.mark.parametrize("case", [(3, 5000, 8, 2, 128, 16, "bf16"), (2, 700, 4, 4, 64, 4, "f32")], ids=["tc", "cuda_core"])
+def test_varlen_batch_matches_one_call_per_prompt(binding, case):
+    """nacl_evict_varlen: a padded batch whose prompts have different lengths and budgets.  Every
+    element must come out exactly as a batch-1 call on its own live rows with batch_offset = b (same Philox streams), and
+    that call's index list must be the oracle's on the same importance; nothing is written past an element's own C rows."""
+    B, Lmax, Hq, Hkv, d, P, dt = case
+    K, V, Q = make_random_inputs(B, Lmax, Hq, Hkv, d, P, dtype=dt, seed=77)
+    lens = [Lmax, Lmax * 3 // 5 + 1, Lmax // 4 + 3][:B]
+    bps = [l // 6 for l in lens]
+    brs = [l // 17 for l in lens]
+    ns, nr = 4, P
+    # element b's proxy queries are the last P positions of ITS prompt: Q as given stands for them
+    Kc, Vc, Qc = K.cuda(), V.cuda(), Q.cuda()
+    res = binding.nacl_evict_varlen(Kc, Vc, Qc, lens, bps, brs, ns, nr, 11, 2)
+    torch.cuda.synchronize()
+    for b in range(B):
+        Kb, Vb, Qb = K[b:b + 1, :, :lens[b]].contiguous(), V[b:b + 1, :, :lens[b]].contiguous(), Q[b:b + 1].contiguous()
+        one = binding.nacl_evict_ex(Kb.cuda(), Vb.cuda(), Qb.cuda(), bps[b], brs[b], ns, nr, 11, 2, batch_offset=b, want_importance=True)
+        Cb = bps[b] + brs[b]
+        assert torch.equal(res["out_idx"][b], one["out_idx"][0])
+        assert torch.equal(res["out_K"][b, :, :Cb], one["out_K"][0]) and torch.equal(res["out_V"][b, :, :Cb], one["out_V"][0])
+        assert (res["out_K"][b, :, Cb:] == 0).all() and (res["out_V"][b, :, Cb:] == 0).all()
+        ref = oracle.select(one["importance"].cpu().numpy(), bps[b], brs[b], ns, nr, 11, 2, batch_offset=b)
+        np.testing.assert_array_equal(one["out_idx"].cpu().numpy(), ref)
+        imp_ref = oracle.importance(Kb, Qb)
+        rel = np.abs(one["importance"].cpu().numpy() - imp_ref) / (np.abs(imp_ref) + 1e-30)
+        assert rel.max() <= 2e-3
+
+
 def test_edge_budgets(binding):
     K, V, Q = make_random_inputs(1, 300, 4, 2, 64, 4, dtype="f32", seed=1)
     L = 300

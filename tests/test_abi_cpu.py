@@ -99,6 +99,30 @@ def test_ex_rejects_wrong_struct_and_unknown_flags(lib):
     assert lib.nacl_evict_ex(C.byref(p)) == -5
 
 
+def test_varlen_validation_without_touching_the_device(lib):
+    from paper_2408_03675_b200.binding import NaclParams
+
+    i32x2 = C.c_int32 * 2
+    lib.nacl_evict_varlen.argtypes = [C.POINTER(NaclParams), C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.c_int]
+    p = NaclParams()
+    p.struct_size = C.sizeof(NaclParams)
+    p.dtype = 1
+    p.K, p.V, p.Qproxy, p.out_K, p.out_V, p.out_idx = 0x1000, 0x2000, 0x3000, 0x4000, 0x5000, 0x6000
+    p.batch, p.L, p.Hq, p.Hkv, p.d, p.P = 2, 512, 4, 4, 64, 16
+    p.n_sink, p.n_recent = 4, 16
+    lens, bp, br = i32x2(512, 300), i32x2(76, 40), i32x2(26, 10)
+    assert lib.nacl_evict_varlen(None, lens, bp, br, 102) == -1
+    assert lib.nacl_evict_varlen(C.byref(p), None, bp, br, 102) == -1
+    assert lib.nacl_evict_varlen(C.byref(p), i32x2(512, 513), bp, br, 102) == -2  # longer than the padded length
+    assert lib.nacl_evict_varlen(C.byref(p), i32x2(512, 0), bp, br, 102) == -2
+    assert lib.nacl_evict_varlen(C.byref(p), lens, bp, br, 101) == -3             # an element's budget exceeds C_max
+    p.lse_in = 0x7000
+    assert lib.nacl_evict_varlen(C.byref(p), lens, bp, br, 102) == -7             # not offered for variable-length batches
+    p.lse_in = None
+    p.struct_size = 8
+    assert lib.nacl_evict_varlen(C.byref(p), lens, bp, br, 102) == -7
+
+
 def test_product_does_not_import_the_oracle():
     pkg = os.path.join(ROOT, "paper_2408_03675_b200")
     for dirpath, _, files in os.walk(pkg):

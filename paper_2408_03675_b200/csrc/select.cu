@@ -548,7 +548,7 @@ __device__ long long g_sel_trace2[1024][10];
 __device__ int g_select_fallbacks = 0;  // selections that gave up the fast path (nacl_select_fallbacks)
 constexpr int kFastMaxE = 16;   // consecutive positions per thread (instantiations for 8 and 16): slices of at most 16 * ST positions
 constexpr int kListCap = 4096;  // candidate-list entries (value, position) per select
-constexpr int kImpShift = 14;   // float bits dropped by the top-k bucket: 512 buckets per binade
+// (the top-k bucket drops imp_shift = 12..14 float bits: 512 buckets per binade for rows up to 40k, more for longer rows)
 constexpr float kKeyBucketsPerUnit = 64.f, kKeyBelow = 24.f;  // sample buckets: [ln mean - 24, ln mean + 40)
 
 // CODE SIZE matters here: every phase of the selection runs once, so straight-line code is fetched cold (the first
@@ -659,7 +659,7 @@ __device__ __noinline__ void list_publish(uint2* list, int off, int cnt) {
 // positions are in out[] and ib[0..tot) (this CTA's part, output rows base .. base+tot).
 template <int FE>
 __device__ bool select_fast(const float* __restrict__ row, int nloc, int E, int j0, int lo, int hi, int k1, int Br, int C,
-                            int imp_base, float key_lo, uint32_t hk_g, uint32_t b_g, uint32_t layer, uint32_t sk0, uint32_t sk1,
+                            int imp_base, int imp_shift, float key_lo, uint32_t hk_g, uint32_t b_g, uint32_t layer, uint32_t sk0, uint32_t sk1,
                             uint32_t flags, ClShared& sh, uint32_t* ib, uint32_t* kb, uint2* list, cg::cluster_group& cluster,
                             int32_t* __restrict__ out, int& tot_out, int& base_out) {
   const unsigned rank = cluster.block_rank(), nrank = cluster.num_blocks();
@@ -691,7 +691,7 @@ __device__ bool select_fast(const float* __restrict__ row, int nloc, int E, int 
     __syncthreads();
 #pragma unroll
     for (int e = 0; e < FE; ++e) {
-      dg[e] = min(max((int)(v[e] >> kImpShift) - imp_base, 0), HB - 1);
+      dg[e] = min(max((int)(v[e] >> imp_shift) - imp_base, 0), HB - 1);
       // (plain shared-memory atomics: the buckets are fine where the values are, lanes rarely meet in one)
       if ((freem >> e) & 1u) atomicAdd(&sh.hist[dg[e]], 1u);
     }
@@ -713,7 +713,7 @@ __device__ bool select_fast(const float* __restrict__ row, int nloc, int E, int 
     for (unsigned r = 0; r < nrank; ++r) { before += r < rank ? sh.rc[r][1] : 0; n_eq += sh.rc[r][1]; }
     if (bin == 0 || bin == HB - 1 || n_eq > kListCap) return false;  // clamped bucket / list overflow (cluster-uniform)
     if (krem == n_eq) {
-      thr_p = (uint32_t)(bin + imp_base) << kImpShift;  // the whole bucket is taken: its lower edge is a threshold
+      thr_p = (uint32_t)(bin + imp_base) << imp_shift;  // the whole bucket is taken: its lower edge is a threshold
       cut_p = 0x7FFFFFFF;
     } else {
       int mine = 0;
@@ -862,7 +862,7 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
                                                                  const int4* __restrict__ Kv, const int4* __restrict__ Vv,
                                                                  int4* __restrict__ oKv, int4* __restrict__ oVv, int vpr,
                                                                  uint32_t b_off, uint32_t h_off, KvVecLayout ly, int fast,
-                                                                 int imp_base, float key_lo) {
+                                                                 int imp_base, int imp_shift, float key_lo) {
   cg::cluster_group cluster = cg::this_cluster();
   extern __shared__ __align__(16) unsigned char dyn_raw[];
   ClShared& sh = *reinterpret_cast<ClShared*>(dyn_raw);
@@ -889,10 +889,10 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
     uint2* list = reinterpret_cast<uint2*>(dyn + 2 * (size_t)Lc);
     const int E = (Lc + ST - 1) / ST;
     if (E <= 8)
-      done = select_fast<8>(row, nloc, E, j0, lo, hi, k1, Br, C, imp_base, key_lo, (uint32_t)hk + h_off, (uint32_t)b + b_off, layer, sk0,
+      done = select_fast<8>(row, nloc, E, j0, lo, hi, k1, Br, C, imp_base, imp_shift, key_lo, (uint32_t)hk + h_off, (uint32_t)b + b_off, layer, sk0,
                             sk1, flags, sh, ib, kb, list, cluster, out, tot, base);
     else
-      done = select_fast<16>(row, nloc, E, j0, lo, hi, k1, Br, C, imp_base, key_lo, (uint32_t)hk + h_off, (uint32_t)b + b_off, layer, sk0,
+      done = select_fast<16>(row, nloc, E, j0, lo, hi, k1, Br, C, imp_base, imp_shift, key_lo, (uint32_t)hk + h_off, (uint32_t)b + b_off, layer, sk0,
                              sk1, flags, sh, ib, kb, list, cluster, out, tot, base);
   }
   if (!done) {
@@ -1132,12 +1132,15 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   // fast path: bucket windows around the row mean of the importance (its sum over a row is known: G*P) and around the
   // logarithm of that mean for the sampling keys (uniform weights: ln w = 0; weight exp(imp): ln w = imp)
   int fast = (Lc <= kFastMaxE * ST && !(flags & NACL_FLAG_SELECT_GENERAL) && imp_mean > 0.f && imp_mean < 1e30f) ? 1 : 0;
-  int imp_base = 0;
+  int imp_base = 0, imp_shift = 14;
   float key_lo = 0.f;
   if (fast) {
     uint32_t mb;
     memcpy(&mb, &imp_mean, sizeof(mb));
-    imp_base = (int)((mb | 0x80000000u) >> kImpShift) - HB / 2;
+    // finer buckets for longer rows (the threshold bucket should hold a few hundred elements at most); the window is
+    // centred on the mean: a skewed row (few heavy hitters carry the mass) has its top-k threshold well BELOW the mean
+    imp_shift = L <= 40000 ? 14 : (L <= 80000 ? 13 : 12);
+    imp_base = (int)((mb | 0x80000000u) >> imp_shift) - HB / 2;
     const float centre = (flags & NACL_FLAG_SAMPLE_UNIFORM) ? 0.f : ((flags & NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE) ? imp_mean : logf(imp_mean));
     key_lo = centre - kKeyBelow;
   }
@@ -1148,7 +1151,7 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
     StageScope sc(ST_SELECT, st);
     e = cudaLaunchKernelEx(&cfg, nacl_select_cluster_kernel, imp, Hkv, L, Lc, k1, budget_random, n_sink, n_recent, C, sk0, sk1,
                            (uint32_t)layer, flags, out_idx, (const int4*)K, (const int4*)V, (int4*)out_K, (int4*)out_V,
-                           *gathered ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset, ly, fast, imp_base, key_lo);
+                           *gathered ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset, ly, fast, imp_base, imp_shift, key_lo);
   }
   if (e == cudaSuccess) return e;
   // the launch itself was refused (cluster resources): nothing ran; take the path without clusters

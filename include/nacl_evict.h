@@ -65,7 +65,7 @@
 extern "C" {
 #endif
 
-#define NACL_VERSION 200 /* major*10000 + minor*100 + patch */
+#define NACL_VERSION 210 /* major*10000 + minor*100 + patch */
 
 #define NACL_DTYPE_F32 0
 #define NACL_DTYPE_BF16 1
@@ -146,6 +146,20 @@ typedef struct nacl_params {
   int64_t out_stride_batch;        /* the same for out_K / out_V; all three 0 = contiguous [batch,Hkv,C,d]                  */
   int64_t out_stride_head;
   int64_t out_stride_row;
+  /* Paged K/V (the block-table caches of paged-attention servers): with block_table != NULL, K and V
+     are page POOLS and position j of batch element b lives in page block_table[b*table_stride + j/page_size], row
+     j % page_size of that page.  kv_stride_page / kv_stride_head / kv_stride_row are the ELEMENT strides between pages,
+     between the kv heads of a page and between the rows of a page (all three 0 = a contiguous pool
+     [n_pages, Hkv, page_size, d]; kv_stride_batch is ignored).  page_size: 8, 16, 32, 64 or 128.  table_stride >=
+     ceil(L / page_size); the entries of the pages that hold positions < L must lie in [0, n_pages) (device memory: not
+     validated).  Served by the tensor-core scoring path only (bf16, d = 128, G*P a multiple of 16):
+     NACL_ERR_UNSUPPORTED otherwise.  out_K / out_V stay dense. */
+  const int32_t* block_table;      /* DEVICE [batch, table_stride] int32, or NULL */
+  int32_t page_size;
+  int32_t table_stride;
+  int32_t n_pages;
+  int32_t reserved1;               /* 0 */
+  int64_t kv_stride_page;
 } nacl_params_t;
 
 /* bf16 K/V/Q.  Steps 1-7 above on `stream`. */

@@ -40,6 +40,8 @@ class NaclParams(C.Structure):
         ("protect_idx", C.c_void_p), ("n_protect", C.c_int32), ("reserved0", C.c_int32),
         ("kv_stride_batch", C.c_int64), ("kv_stride_head", C.c_int64), ("kv_stride_row", C.c_int64),
         ("out_stride_batch", C.c_int64), ("out_stride_head", C.c_int64), ("out_stride_row", C.c_int64),
+        ("block_table", C.c_void_p), ("page_size", C.c_int32), ("table_stride", C.c_int32), ("n_pages", C.c_int32),
+        ("reserved1", C.c_int32), ("kv_stride_page", C.c_int64),
     ]
 
 
@@ -274,6 +276,52 @@ def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, s
         out["importance"] = imp
     if lse is not None:
         out["lse"] = lse
+    return out
+
+
+def nacl_evict_paged(K_pool, V_pool, block_table, L, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer,
+                     flags=0, pool_layout="HND", want_importance=False, workspace=None, stream=None, batch_offset=0, head_offset=0):
+    """include/nacl_evict.h `nacl_evict_ex` with a block table: K_pool / V_pool are page pools [n_pages, Hkv, page, d]
+    ("HND") or [n_pages, page, Hkv, d] ("NHD"), block_table [B, pages_per_seq] int32 (device), L live keys per batch
+    element.  Outputs are dense, as for nacl_evict_ex."""
+    if pool_layout == "HND":
+        n_pages, Hkv, ps, d = K_pool.shape
+        st_page, st_head, st_row = K_pool.stride(0), K_pool.stride(1), K_pool.stride(2)
+    else:
+        n_pages, ps, Hkv, d = K_pool.shape
+        st_page, st_row, st_head = K_pool.stride(0), K_pool.stride(1), K_pool.stride(2)
+    if not (K_pool.is_cuda and V_pool.is_cuda and K_pool.stride() == V_pool.stride() and K_pool.stride(3) == 1):
+        raise ValueError("nacl_evict_paged takes CUDA pools that share their strides and have contiguous rows")
+    assert block_table.is_cuda and block_table.dtype == torch.int32 and block_table.dim() == 2 and block_table.stride(1) == 1
+    B, Hq, P, _ = Qproxy.shape
+    dev = K_pool.device
+    Cn = budget_proxy + budget_random
+    out_K = torch.empty((B, Hkv, max(Cn, 0), d), dtype=K_pool.dtype, device=dev)
+    out_V = torch.empty_like(out_K)
+    out_idx = torch.empty((B, Hkv, max(Cn, 0)), dtype=torch.int32, device=dev)
+    imp = torch.empty((B, Hkv, L), dtype=torch.float32, device=dev) if want_importance else None
+    p = NaclParams()
+    p.struct_size = C.sizeof(NaclParams)
+    p.dtype = _dtype_tag(K_pool)
+    p.K, p.V, p.Qproxy = K_pool.data_ptr(), V_pool.data_ptr(), Qproxy.data_ptr()
+    p.batch, p.L, p.Hq, p.Hkv, p.d, p.P = B, L, Hq, Hkv, d, P
+    p.budget_proxy, p.budget_random, p.n_sink, p.n_recent = budget_proxy, budget_random, n_sink, n_recent
+    p.seed, p.layer, p.flags = seed, layer, flags
+    p.batch_offset, p.head_offset = batch_offset, head_offset
+    p.kv_stride_head, p.kv_stride_row, p.kv_stride_page = st_head, st_row, st_page
+    p.block_table, p.page_size, p.table_stride, p.n_pages = block_table.data_ptr(), ps, block_table.stride(0), n_pages
+    p.out_K, p.out_V, p.out_idx = out_K.data_ptr(), out_V.data_ptr(), out_idx.data_ptr()
+    p.out_importance = imp.data_ptr() if imp is not None else None
+    if workspace is not None:
+        p.workspace, p.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
+    p.stream = (stream or torch.cuda.current_stream(dev)).cuda_stream
+    with torch.cuda.device(dev):
+        rc = _lib.nacl_evict_ex(C.byref(p))
+    if rc != 0:
+        raise NaclError(rc, "nacl_evict_ex (paged)")
+    out = {"out_K": out_K, "out_V": out_V, "out_idx": out_idx}
+    if imp is not None:
+        out["importance"] = imp
     return out
 
 

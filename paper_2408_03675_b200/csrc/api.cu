@@ -203,7 +203,7 @@ static int evict_impl(const nacl_params_t& p) {
   {
     const bool kv0 = p.kv_stride_batch == 0 && p.kv_stride_head == 0 && p.kv_stride_row == 0;
     const bool o0 = p.out_stride_batch == 0 && p.out_stride_head == 0 && p.out_stride_row == 0;
-    if (!kv0 && (p.kv_stride_batch <= 0 || p.kv_stride_head <= 0 || p.kv_stride_row < p.d)) return NACL_ERR_SHAPE;
+    if (!kv0 && !p.block_table && (p.kv_stride_batch <= 0 || p.kv_stride_head <= 0 || p.kv_stride_row < p.d)) return NACL_ERR_SHAPE;
     if (!o0 && (p.out_stride_batch <= 0 || p.out_stride_head <= 0 || p.out_stride_row < p.d)) return NACL_ERR_SHAPE;
     s.kv_sr = kv0 ? p.d : p.kv_stride_row;
     s.kv_sh = kv0 ? (long long)p.L * p.d : p.kv_stride_head;
@@ -213,6 +213,26 @@ static int evict_impl(const nacl_params_t& p) {
     s.o_sb = o0 ? (long long)p.Hkv * C * p.d : p.out_stride_batch;
     const long long epv = 16 / s.esize;
     if (s.kv_sr % epv || s.kv_sh % epv || s.kv_sb % epv || s.o_sr % epv || s.o_sh % epv || s.o_sb % epv) return NACL_ERR_ALIGN;
+  }
+  if (p.block_table) {
+    if (p.reserved1 != 0) return NACL_ERR_UNSUPPORTED;
+    const int ps = p.page_size;
+    if (!(ps == 8 || ps == 16 || ps == 32 || ps == 64 || ps == 128) || p.n_pages < 1) return NACL_ERR_SHAPE;
+    if ((long long)p.table_stride * ps < p.L) return NACL_ERR_SHAPE;
+    if (reinterpret_cast<uintptr_t>(p.block_table) & 3u) return NACL_ERR_ALIGN;
+    const bool pg0 = p.kv_stride_page == 0 && p.kv_stride_head == 0 && p.kv_stride_row == 0;
+    if (!pg0 && (p.kv_stride_page <= 0 || p.kv_stride_head <= 0 || p.kv_stride_row < p.d)) return NACL_ERR_SHAPE;
+    s.table = p.block_table; s.ps = ps; s.tstride = p.table_stride; s.n_pages = p.n_pages;
+    s.kv_sr = pg0 ? p.d : p.kv_stride_row;
+    s.kv_sh = pg0 ? (long long)ps * p.d : p.kv_stride_head;
+    s.kv_sp = pg0 ? (long long)p.Hkv * ps * p.d : p.kv_stride_page;
+    s.kv_sb = 0;
+    const long long epv = 16 / s.esize;
+    if (s.kv_sr % epv || s.kv_sh % epv || s.kv_sp % epv) return NACL_ERR_ALIGN;
+    // only the tensor-core scoring kernel walks a block table
+    if ((p.flags & NACL_FLAG_SCORE_CUDA_CORES) || !score_tc_supported(s)) return NACL_ERR_UNSUPPORTED;
+  } else if (p.page_size != 0 || p.table_stride != 0 || p.n_pages != 0 || p.kv_stride_page != 0 || p.reserved1 != 0) {
+    return NACL_ERR_UNSUPPORTED;
   }
   if (!aligned16(p.K) || !aligned16(p.V) || !aligned16(p.Qproxy) || !aligned16(p.out_K) || !aligned16(p.out_V) ||
       (reinterpret_cast<uintptr_t>(p.out_idx) & 3u))
@@ -382,7 +402,7 @@ int nacl_evict_varlen(const nacl_params_t* p, const int32_t* seq_len, const int3
                       int C_max) {
   if (!p || !seq_len || !budget_proxy || !budget_random) return NACL_ERR_NULL;
   if (p->struct_size != sizeof(nacl_params_t)) return NACL_ERR_UNSUPPORTED;
-  if (p->lse_in || p->out_importance || p->out_lse || p->protect_idx || p->n_protect != 0) return NACL_ERR_UNSUPPORTED;
+  if (p->lse_in || p->out_importance || p->out_lse || p->protect_idx || p->n_protect != 0 || p->block_table) return NACL_ERR_UNSUPPORTED;
   if (p->batch < 1 || p->L < 1 || p->Hkv < 1 || p->Hq < 1 || p->d < 1 || p->P < 1 || C_max < 0) return NACL_ERR_SHAPE;
   const size_t esz = p->dtype == NACL_DTYPE_F32 ? 4 : 2;
   // element strides of the padded tensors (all-zero = contiguous [batch, Hkv, L, d] / [batch, Hkv, C_max, d])

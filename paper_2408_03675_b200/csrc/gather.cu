@@ -22,7 +22,8 @@ constexpr int GU = 4;    // vectors of K and of V in flight per thread
 
 // vpr = 16-byte vectors per row; n_vec = n_prob * C * vpr output vectors per tensor.  Strides in 16-byte vectors:
 // (sb, sh, sr) of K/V per batch element / kv head / row, (ob, oh, orow) of the outputs.
-struct GatherLayout { long long sb, sh, sr, ob, oh, orow; int Hkv; };
+// Paged source (table != nullptr): row j of batch element b = row j % ps of page table[b * tstride + j / ps], page stride sp.
+struct GatherLayout { long long sb, sh, sr, ob, oh, orow; int Hkv; const int32_t* table; int ps, tstride; long long sp; };
 __global__ void __launch_bounds__(GT) nacl_gather_kernel(const int4* __restrict__ K, const int4* __restrict__ V,
                                                      const int32_t* __restrict__ idx, int C, int vpr, GatherLayout ly,
                                                      size_t n_vec, int4* __restrict__ oK, int4* __restrict__ oV) {
@@ -41,7 +42,12 @@ __global__ void __launch_bounds__(GT) nacl_gather_kernel(const int4* __restrict_
         const int c = (int)(row - p * (size_t)C);
         const int b = (int)(p / (size_t)ly.Hkv), hk = (int)(p - (size_t)b * ly.Hkv);
         const int j = idx[row];
-        src[u] = (size_t)(b * ly.sb + hk * ly.sh + (long long)j * ly.sr) + off;
+        if (ly.table) {
+          const long long pg = __ldg(&ly.table[(size_t)b * ly.tstride + j / ly.ps]);
+          src[u] = (size_t)(pg * ly.sp + hk * ly.sh + (long long)(j % ly.ps) * ly.sr) + off;
+        } else {
+          src[u] = (size_t)(b * ly.sb + hk * ly.sh + (long long)j * ly.sr) + off;
+        }
         dst[u] = (size_t)(b * ly.ob + hk * ly.oh + (long long)c * ly.orow) + off;
       }
     }
@@ -115,7 +121,8 @@ cudaError_t launch_gather(const void* K, const void* V, const int32_t* idx, cons
   const size_t n_vec = (size_t)s.batch * s.Hkv * C * vpr;
   if (n_vec == 0) return cudaSuccess;
   const long long epv = 16 / s.esize;  // elements per 16-byte vector (strides are multiples of it)
-  const GatherLayout ly{s.kv_sb / epv, s.kv_sh / epv, s.kv_sr / epv, s.o_sb / epv, s.o_sh / epv, s.o_sr / epv, s.Hkv};
+  const GatherLayout ly{s.kv_sb / epv, s.kv_sh / epv, s.kv_sr / epv, s.o_sb / epv, s.o_sh / epv, s.o_sr / epv, s.Hkv,
+                        s.table, s.ps, s.tstride, s.kv_sp / epv};
   size_t want = (n_vec + (size_t)GT * GU - 1) / ((size_t)GT * GU);
   const size_t cap = (size_t)kNumSMs * 8 * 4;  // a few waves of 8 resident CTAs per SM
   int blocks = (int)(want < cap ? want : cap);

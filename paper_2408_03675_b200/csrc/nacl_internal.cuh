@@ -22,6 +22,11 @@ struct Shape {
   int esize;    // bytes per element
   // element strides of K and V (batch, kv head, key row; the d elements of a row are contiguous) and of out_K / out_V
   long long kv_sb, kv_sh, kv_sr, o_sb, o_sh, o_sr;
+  // paged K/V (table != nullptr): position j of batch element b = row j % ps of page table[b * tstride + j / ps];
+  // kv_sp = element stride between pages (kv_sb unused)
+  const int32_t* table = nullptr;
+  int ps = 0, tstride = 0, n_pages = 0;
+  long long kv_sp = 0;
 };
 
 // How L is split for the split-L softmax statistics (a pure function of the shape).

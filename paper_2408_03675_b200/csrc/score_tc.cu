@@ -113,6 +113,8 @@ struct TcParams {
   float* lse_out;          // optional [heads*rows], natural log
   float* imp;              // [heads, L]
   float* imp_out;          // optional
+  const int* table;        // paged K (or nullptr): page of position j of batch element hb = table[hb * tstride + j / ps]
+  int ps, tstride;
   int* sync;               // fused launch: [2 * heads] zero at launch: per head the number of (CTA, row block) pieces whose
                            // partials are published, and the number of consumers that have seen them all (the last one
                            // zeroes both again)
@@ -661,7 +663,24 @@ __device__ __forceinline__ void sweep(const CUtensorMap& tmK, const CUtensorMap&
 #else
         const int j0 = (sg.tile + walk.step * i) * TILE;
 #endif
-        if (leader) {
+        if (p.table) {
+          // paged K: the tile's 128 / ps pages are looked up by one lane each and loaded page by page into their rows of the
+          // stage (ps rows x 128 B per box and page: a multiple of the 1024-byte swizzle atom).  Pages past the last key are
+          // not loaded: their rows hold stale bytes, the keys past L are masked in both sweeps.
+          const int nsub = TILE / p.ps;
+          const int jb = j0 + lane * p.ps;
+          int pg = 0;
+          if (lane < nsub && jb < p.L) pg = __ldg(&p.table[(size_t)hb * p.tstride + jb / p.ps]);
+          const int nload = min(nsub, (p.L - j0 + p.ps - 1) / p.ps);
+          if (leader) mbar_expect_tx(k_full(stage), (uint32_t)(nload * p.ps * 256));
+          for (int sb = 0; sb < nload; ++sb) {
+            const int page = __shfl_sync(0xffffffffu, pg, sb);
+            if (leader) {
+              tma_load_4d(kdst + sb * p.ps * 128, &tmK, 0, 0, hk, page, k_full(stage));
+              tma_load_4d(kdst + BOX_BYTES + sb * p.ps * 128, &tmK, 64, 0, hk, page, k_full(stage));
+            }
+          }
+        } else if (leader) {
           mbar_expect_tx(k_full(stage), KSTAGE_BYTES);
           tma_load_4d(kdst, &tmK, 0, j0, hk, hb, k_full(stage));
           tma_load_4d(kdst + BOX_BYTES, &tmK, 64, j0, hk, hb, k_full(stage));
@@ -1216,9 +1235,11 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
   alignas(64) CUtensorMap tmK, tmQ;
   {
     // [batch, Hkv, L, d] with the caller's strides (contiguous, a cache with spare capacity, or token-major [B,L,H,d])
-    const cuuint64_t dims[4] = {(cuuint64_t)HD, (cuuint64_t)s.L, (cuuint64_t)s.Hkv, (cuuint64_t)s.batch};
-    const cuuint64_t strides[3] = {(cuuint64_t)s.kv_sr * 2, (cuuint64_t)s.kv_sh * 2, (cuuint64_t)s.kv_sb * 2};
-    const cuuint32_t box[4] = {64, (cuuint32_t)TILE, 1, 1};
+    // paged: [n_pages, Hkv, page_size, d] with the pool's strides, one box = the 64 columns of one page's rows
+    const bool paged = s.table != nullptr;
+    const cuuint64_t dims[4] = {(cuuint64_t)HD, (cuuint64_t)(paged ? s.ps : s.L), (cuuint64_t)s.Hkv, (cuuint64_t)(paged ? s.n_pages : s.batch)};
+    const cuuint64_t strides[3] = {(cuuint64_t)s.kv_sr * 2, (cuuint64_t)s.kv_sh * 2, (cuuint64_t)(paged ? s.kv_sp : s.kv_sb) * 2};
+    const cuuint32_t box[4] = {64, (cuuint32_t)(paged ? s.ps : TILE), 1, 1};
     const cuuint32_t es[4] = {1, 1, 1, 1};
 #ifndef NACL_K_L2PROMO
 #define NACL_K_L2PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_256B
@@ -1247,6 +1268,7 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
   p.scale_log2 = 1.4426950408889634f / sqrtf((float)s.d);
   p.part = ws.part; p.lse_in = lse_in; p.lse_out = lse_out; p.imp = ws.imp; p.imp_out = imp_out;
   p.sync = ws.sync;
+  p.table = s.table; p.ps = s.ps; p.tstride = s.tstride;
 
 #ifndef NACL_STAGES_S
 #define NACL_STAGES_S 5

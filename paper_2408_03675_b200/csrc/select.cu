@@ -330,7 +330,16 @@ __device__ __forceinline__ long long sel_gtimer() { long long t; asm volatile("m
 // after its reads, so single buffers suffice.
 constexpr int kMaxRanks = 16;
 constexpr int kFineW = 68;  // row width of the fine exchange buffer: 64 bins, one neighbour on either side, padding
-struct KvVecLayout { long long sb, sh, sr, ob, oh, orow; };  // strides of K/V and of out_K/out_V in 16-byte vectors
+// strides of K/V and of out_K/out_V in 16-byte vectors; paged source (table != nullptr): row j of batch element b = row
+// j % ps of page table[b * tstride + j / ps], page stride sp
+struct KvVecLayout { long long sb, sh, sr, ob, oh, orow; const int32_t* table; int ps, tstride; long long sp; };
+__device__ __forceinline__ size_t kv_row_vec(const KvVecLayout& ly, int b, int hk, int j) {
+  if (ly.table) {
+    const long long pg = __ldg(&ly.table[(size_t)b * ly.tstride + j / ly.ps]);
+    return (size_t)(pg * ly.sp + hk * ly.sh + (long long)(j % ly.ps) * ly.sr);
+  }
+  return (size_t)(b * ly.sb + hk * ly.sh + (long long)j * ly.sr);
+}
 struct ClShared {
   uint32_t hist[HB];
   uint32_t xsup[kMaxRanks][64];   // [rank][super-bin]: pushed by every rank
@@ -971,7 +980,7 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
   __syncthreads();
   const int n_vec = min(tot, C - base) * vpr;
   // K/V and the outputs have their own strides (in 16-byte vectors); a row's vpr vectors are contiguous
-  const size_t src0 = (size_t)(b * ly.sb + hk * ly.sh), dst0 = (size_t)(b * ly.ob + hk * ly.oh + (long long)base * ly.orow);
+  const size_t dst0 = (size_t)(b * ly.ob + hk * ly.oh + (long long)base * ly.orow);
   const long long dpad = ly.orow - vpr;  // 0 for contiguous output rows: then the output vector index is just v
   if (dpad == 0) {
     // four vectors of K and four of V in flight per thread
@@ -983,7 +992,7 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
         const int v = v0 + u * ST;
         if (v < n_vec) {
           const int row = v / vpr;
-          src[u] = src0 + (size_t)ib[row] * ly.sr + (v - row * vpr);
+          src[u] = kv_row_vec(ly, b, hk, (int)ib[row]) + (v - row * vpr);
         }
       }
 #pragma unroll
@@ -1003,7 +1012,7 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
       const int v = v0 + u * ST;
       if (v < n_vec) {
         const int row = v / vpr;
-        src[u] = src0 + (size_t)ib[row] * ly.sr + (v - row * vpr);
+        src[u] = kv_row_vec(ly, b, hk, (int)ib[row]) + (v - row * vpr);
         dst[u] = dst0 + (size_t)v + (size_t)(row * dpad);
       }
     }
@@ -1127,7 +1136,8 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   KvVecLayout ly{};
   if (K != nullptr) {
     const long long epv = 16 / layout->esize;
-    ly = KvVecLayout{layout->kv_sb / epv, layout->kv_sh / epv, layout->kv_sr / epv, layout->o_sb / epv, layout->o_sh / epv, layout->o_sr / epv};
+    ly = KvVecLayout{layout->kv_sb / epv, layout->kv_sh / epv, layout->kv_sr / epv, layout->o_sb / epv, layout->o_sh / epv, layout->o_sr / epv,
+                     layout->table, layout->ps, layout->tstride, layout->kv_sp / epv};
   }
   // fast path: bucket windows around the row mean of the importance (its sum over a row is known: G*P) and around the
   // logarithm of that mean for the sampling keys (uniform weights: ln w = 0; weight exp(imp): ln w = imp)

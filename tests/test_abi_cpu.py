@@ -99,6 +99,32 @@ def test_ex_rejects_wrong_struct_and_unknown_flags(lib):
     assert lib.nacl_evict_ex(C.byref(p)) == -5
 
 
+def test_paged_kv_validation_without_touching_the_device(lib):
+    from paper_2408_03675_b200.binding import NaclParams
+
+    lib.nacl_evict_ex.argtypes = [C.POINTER(NaclParams)]
+    p = NaclParams()
+    p.struct_size = C.sizeof(NaclParams)
+    p.dtype = 1
+    p.K, p.V, p.Qproxy, p.out_K, p.out_V, p.out_idx = 0x1000, 0x2000, 0x3000, 0x4000, 0x5000, 0x6000
+    p.batch, p.L, p.Hq, p.Hkv, p.d, p.P = 2, 4096, 32, 8, 128, 16
+    p.budget_proxy, p.budget_random, p.n_sink, p.n_recent = 600, 200, 4, 16
+    p.page_size = 16                                  # paging fields without a table
+    assert lib.nacl_evict_ex(C.byref(p)) == -7
+    p.block_table, p.table_stride, p.n_pages = 0x7000, 256, 600
+    p.page_size = 24                                  # not one of 8, 16, 32, 64, 128
+    assert lib.nacl_evict_ex(C.byref(p)) == -2
+    p.page_size, p.table_stride = 16, 255             # the table does not cover L
+    assert lib.nacl_evict_ex(C.byref(p)) == -2
+    p.table_stride = 256
+    p.flags = 0x100                                   # only the tensor-core scoring kernel walks a block table
+    assert lib.nacl_evict_ex(C.byref(p)) == -7
+    p.flags, p.d = 0, 64
+    assert lib.nacl_evict_ex(C.byref(p)) == -7
+    p.d, p.block_table = 128, 0x7002                  # misaligned table
+    assert lib.nacl_evict_ex(C.byref(p)) == -4
+
+
 def test_varlen_validation_without_touching_the_device(lib):
     from paper_2408_03675_b200.binding import NaclParams
 

@@ -198,6 +198,43 @@ def test_varlen_batch_matches_one_call_per_prompt(binding, case):
         assert rel.max() <= 2e-3
 
 
+@pytest.mark.parametrize("layout", ["HND", "NHD"])
+@pytest.mark.parametrize("case", [(2, 5000, 8, 2, 128, 32, 16), (1, 4100, 32, 8, 128, 64, 64), (3, 777, 4, 4, 128, 16, 8),
+                                  (1, 70000, 8, 2, 128, 16, 128), (2, 300, 8, 8, 128, 16, 32)],
+                         ids=lambda c: f"B{c[0]}_L{c[1]}_H{c[2]}-{c[3]}_P{c[5]}_page{c[6]}")
+def test_paged_kv_matches_the_contiguous_call(binding, case, layout):
+    """Paged K/V (block table): the pages of every prompt are scattered over a shuffled pool (with
+    spare pages and a padded table); importance, kept positions and compacted caches must be bit-identical to the
+    contiguous call on the same values, which itself is checked against the oracle."""
+    B, L, Hq, Hkv, d, P, ps = case
+    K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype="bf16", seed=L + ps)
+    Bp, Br = L // 5, L // 20
+    want = binding.nacl_evict_ex(K.cuda(), V.cuda(), Q.cuda(), Bp, Br, 4, P, 21, 3, want_importance=True)
+    npp = (L + ps - 1) // ps                      # pages per prompt
+    n_pages = B * npp + 5                         # spare pages that belong to nobody
+    g = torch.Generator().manual_seed(ps)
+    perm = torch.randperm(n_pages, generator=g)[:B * npp].view(B, npp)
+    table = torch.full((B, npp + 3), -1, dtype=torch.int32)   # padded table: entries past the last page are never read
+    table[:, :npp] = perm.to(torch.int32)
+    Kp = torch.full((n_pages, Hkv, ps, d), float("nan"), dtype=torch.bfloat16)   # stale / foreign pages hold NaN
+    Vp = torch.full((n_pages, Hkv, ps, d), float("nan"), dtype=torch.bfloat16)
+    pad = npp * ps - L
+    Kpad = torch.cat([K, torch.full((B, Hkv, pad, d), float("nan"), dtype=K.dtype)], dim=2) if pad else K
+    Vpad = torch.cat([V, torch.full((B, Hkv, pad, d), float("nan"), dtype=V.dtype)], dim=2) if pad else V
+    for b in range(B):
+        Kp[perm[b]] = Kpad[b].view(Hkv, npp, ps, d).transpose(0, 1)
+        Vp[perm[b]] = Vpad[b].view(Hkv, npp, ps, d).transpose(0, 1)
+    if layout == "NHD":
+        Kp, Vp = Kp.transpose(1, 2).contiguous(), Vp.transpose(1, 2).contiguous()
+    got = binding.nacl_evict_paged(Kp.cuda(), Vp.cuda(), table.cuda(), L, Q.cuda(), Bp, Br, 4, P, 21, 3, pool_layout=layout,
+                                   want_importance=True)
+    torch.cuda.synchronize()
+    for k in ("importance", "out_idx", "out_K", "out_V"):
+        assert torch.equal(got[k], want[k]), f"{k} differs between the paged and the contiguous call"
+    ref = oracle.select(want["importance"].cpu().numpy(), Bp, Br, 4, P, 21, 3)
+    np.testing.assert_array_equal(got["out_idx"].cpu().numpy(), ref)
+
+
 def test_edge_budgets(binding):
     K, V, Q = make_random_inputs(1, 300, 4, 2, 64, 4, dtype="f32", seed=1)
     L = 300

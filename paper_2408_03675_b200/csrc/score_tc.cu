@@ -660,6 +660,11 @@ __device__ __forceinline__ void sweep(const CUtensorMap& tmK, const CUtensorMap&
         const uint32_t kdst = sbase + SM::OFF_K + stage * KSTAGE_BYTES;
 #ifdef NACL_DIAG_SAME_TILE  // diagnostics: every K tile comes from L2 (results are wrong)
         const int j0 = ((sg.tile + walk.step * i) & 7) * TILE;
+#elif defined(NACL_DIAG_RR_TILES)  // diagnostics: the CTAs stream one sliding window (tile = CTA + grid * step; results are wrong)
+        const long long rr_ = ((long long)blockIdx.x + (long long)gridDim.x * kuse) % p.N;
+        const int j0 = (int)(rr_ % p.T) * TILE;
+        const int hh_ = (int)(rr_ / p.T);
+        const int hb = hh_ / p.Hkv, hk = hh_ - hb * p.Hkv;
 #else
         const int j0 = (sg.tile + walk.step * i) * TILE;
 #endif

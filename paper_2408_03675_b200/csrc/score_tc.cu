@@ -656,6 +656,13 @@ __device__ __forceinline__ void sweep(const CUtensorMap& tmK, const CUtensorMap&
     // cfg 2 55.5 -> 53.9; keeping the tail of a CTA's sweep-S range with evict_last instead (16-110 MB) was worse than
     // hinting everything evict_first.
     const uint64_t pol_first = l2_policy_evict_first();
+#ifdef NACL_DIAG_K_HINT  // diagnostics: bit 0 = hint in sweep S, bit 1 = in sweep C; without a hint: evict_normal
+    uint64_t pol_normal;
+    asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol_normal));
+    const uint64_t pol_k = ((NACL_DIAG_K_HINT >> PH) & 1) ? pol_first : pol_normal;
+#else
+    const uint64_t pol_k = pol_first;
+#endif
     Walk walk(p, PH);
     Seg sg;
     while (walk.next(sg)) {
@@ -701,8 +708,8 @@ __device__ __forceinline__ void sweep(const CUtensorMap& tmK, const CUtensorMap&
           }
         } else if (leader) {
           mbar_expect_tx(k_full(stage), KSTAGE_BYTES);
-          tma_load_4d_hint(kdst, &tmK, 0, j0, hk, hb, k_full(stage), pol_first);
-          tma_load_4d_hint(kdst + BOX_BYTES, &tmK, 64, j0, hk, hb, k_full(stage), pol_first);
+          tma_load_4d_hint(kdst, &tmK, 0, j0, hk, hb, k_full(stage), pol_k);
+          tma_load_4d_hint(kdst + BOX_BYTES, &tmK, 64, j0, hk, hb, k_full(stage), pol_k);
         }
         if (++stage == STAGES) { stage = 0; kphase ^= 1; }
         ++kuse;

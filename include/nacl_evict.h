@@ -143,6 +143,11 @@ typedef struct nacl_params {
                                    /* (row = Hkv*d, head = d, batch = L*Hkv*d).  Each times sizeof(element) must be a      */
                                    /* multiple of 16 bytes.  K and V share them ("compatible with            */
                                    /* FlashAttention": both cache layouts of such kernels are served without a copy)       */
+  /* In-place compaction: out_K == K and out_V == V with the SAME strides and contiguous rows
+     (kv_stride_row == d) compacts the cache inside its own buffers: rows 0 .. C-1 of every head receive the kept rows
+     (a row is never overwritten before it has been read), the rows behind them keep their old contents.  Needs the
+     cluster selection kernel (rows of at most 327680 keys, not NACL_FLAG_SHARED_HEADS, not paged): NACL_ERR_UNSUPPORTED
+     otherwise.  Any other overlap between inputs and outputs is undefined. */
   int64_t out_stride_batch;        /* the same for out_K / out_V; all three 0 = contiguous [batch,Hkv,C,d]                  */
   int64_t out_stride_head;
   int64_t out_stride_row;

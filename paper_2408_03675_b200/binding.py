@@ -255,6 +255,11 @@ def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, s
     if out_K.stride() != out_V.stride() or (Cn > 0 and out_K.stride(3) != 1):
         raise ValueError("out_K and out_V must share their strides and have contiguous rows")
     p.out_stride_batch, p.out_stride_head, p.out_stride_row = _kv_strides(out_K) if Cn > 0 else (0, 0, 0)
+    if Cn > 0 and out_K.data_ptr() == K.data_ptr():
+        # in-place compaction: the output IS the [batch, Hkv, L, d] cache, not a dense [batch, Hkv, C, d] tensor
+        p.out_stride_batch, p.out_stride_head, p.out_stride_row = out_K.stride(0), out_K.stride(1), out_K.stride(2)
+        if K.is_contiguous():
+            p.kv_stride_batch, p.kv_stride_head, p.kv_stride_row = K.stride(0), K.stride(1), K.stride(2)
     if protect_idx is not None:
         assert protect_idx.is_cuda and protect_idx.dtype == torch.int32 and protect_idx.is_contiguous() and protect_idx.dim() == 1
         p.protect_idx, p.n_protect = protect_idx.data_ptr(), protect_idx.numel()

@@ -239,6 +239,14 @@ static int evict_impl(const nacl_params_t& p) {
     return NACL_ERR_ALIGN;
 
   if (p.batch_offset < 0 || p.head_offset < 0) return NACL_ERR_SHAPE;
+  // in-place compaction: the compacted cache takes the first C rows of every head of the SAME buffers
+  bool inplace = false;
+  if (!empty_out && (p.out_K == p.K || p.out_V == p.V)) {
+    if (p.out_K != p.K || p.out_V != p.V || p.block_table || (p.flags & NACL_FLAG_SHARED_HEADS) || s.o_sr != s.kv_sr ||
+        s.o_sh != s.kv_sh || s.o_sb != s.kv_sb || s.kv_sr != s.d)
+      return NACL_ERR_UNSUPPORTED;
+    inplace = true;
+  }
   const size_t need = nacl_workspace_bytes(p.batch, p.L, p.Hq, p.Hkv, p.d, p.P);
   cudaStream_t st = static_cast<cudaStream_t>(p.stream);
   cudaError_t e;
@@ -287,14 +295,15 @@ static int evict_impl(const nacl_params_t& p) {
     if ((e = launch_protect(ws.imp_sh, p.batch, p.L, p.protect_idx, p.n_protect, st)) != cudaSuccess) return fail_cuda(e);
     e = launch_select(ws.imp_sh, ws.key, p.batch, 1, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
                       p.flags, ws.idx_sh, nullptr, nullptr, nullptr, nullptr, row_bytes, &gathered, p.batch_offset, p.head_offset, &s,
-                      (float)p.Hkv * (float)s.rows / (float)p.L, st);
+                      (float)p.Hkv * (float)s.rows / (float)p.L, false, st);
     if (e == cudaSuccess) e = launch_replicate_idx(ws.idx_sh, p.out_idx, p.batch, p.Hkv, C, st);
   } else {
     if ((e = launch_protect(ws.imp, p.batch * p.Hkv, p.L, p.protect_idx, p.n_protect, st)) != cudaSuccess) return fail_cuda(e);
     e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
                       p.flags, p.out_idx, p.K, p.V, p.out_K, p.out_V, row_bytes, &gathered, p.batch_offset, p.head_offset, &s,
-                      (float)s.rows / (float)p.L, st);
+                      (float)s.rows / (float)p.L, inplace, st);
   }
+  if (e == cudaErrorNotSupported && inplace) { cudaGetLastError(); return NACL_ERR_UNSUPPORTED; }  // rows too long for the fused gather
   if (e != cudaSuccess) return fail_cuda(e);
   if (!gathered) {
     StageScope sc(ST_GATHER, st);

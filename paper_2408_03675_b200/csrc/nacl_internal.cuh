@@ -91,11 +91,12 @@ bool select_uses_cluster(int L);
 size_t select_scratch_words(int batch, int Hkv, int L);  // 4-byte words of Workspace::key
 // With K/V given and the cluster path taken, the kernel also moves the kept rows (step a7) and sets *gathered.
 // imp_mean: the mean importance of a row (its sum is known: G*P, or Hkv*G*P for the head-summed rows), centre of the
-// bucket windows of the fast selection path; <= 0: general path only.
+// bucket windows of the fast selection path; <= 0: general path only.  inplace: out_K/out_V alias K/V with the same
+// strides (contiguous rows): only the fused gather of the cluster kernel can do that (cudaErrorNotSupported otherwise).
 cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, int L, int budget_proxy, int budget_random,
                           int n_sink, int n_recent, uint64_t seed, int layer, uint32_t flags, int32_t* out_idx,
                           const void* K, const void* V, void* out_K, void* out_V, int row_bytes, bool* gathered,
-                          int batch_offset, int head_offset, const Shape* layout, float imp_mean, cudaStream_t st);
+                          int batch_offset, int head_offset, const Shape* layout, float imp_mean, bool inplace, cudaStream_t st);
 
 // NACL_FLAG_SHARED_HEADS: out[b, j] = sum over the kv heads (in head order, fp32) of imp[b, hk, j]
 cudaError_t launch_head_sum(const float* imp, float* out, int batch, int Hkv, int L, cudaStream_t st);

@@ -868,10 +868,9 @@ __device__ bool select_fast(const float* __restrict__ row, int nloc, int E, int 
 __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __restrict__ imp, int Hkv, int L, int Lc, int k1, int Br,
                                                                  int n_sink, int n_recent, int C, uint32_t sk0, uint32_t sk1,
                                                                  uint32_t layer, uint32_t flags, int32_t* __restrict__ out_idx,
-                                                                 const int4* __restrict__ Kv, const int4* __restrict__ Vv,
-                                                                 int4* __restrict__ oKv, int4* __restrict__ oVv, int vpr,
+                                                                 const int4* Kv, const int4* Vv, int4* oKv, int4* oVv, int vpr,
                                                                  uint32_t b_off, uint32_t h_off, KvVecLayout ly, int fast,
-                                                                 int imp_base, int imp_shift, float key_lo) {
+                                                                 int imp_base, int imp_shift, float key_lo, int inplace) {
   cg::cluster_group cluster = cg::this_cluster();
   extern __shared__ __align__(16) unsigned char dyn_raw[];
   ClShared& sh = *reinterpret_cast<ClShared*>(dyn_raw);
@@ -983,8 +982,53 @@ __global__ void __launch_bounds__(ST) nacl_select_cluster_kernel(const float* __
   const size_t dst0 = (size_t)(b * ly.ob + hk * ly.oh + (long long)base * ly.orow);
   const long long dpad = ly.orow - vpr;  // 0 for contiguous output rows: then the output vector index is just v
   if (dpad == 0) {
+    int start_vec = 0;
+    if (inplace) {
+      // In-place compaction (out_K == K, out_V == V, same strides): output row c receives position S[c] >= c, so a write
+      // can only destroy a row that is the SOURCE of an output row at or before it.  The rows whose source lies below C
+      // (a prefix of every CTA's ascending list) are moved first, in ascending order: rank after rank, chunk after chunk,
+      // all loads of a chunk before its stores.  Every other row has its source at or above C, where nothing is written:
+      // those move in parallel afterwards.
+      int nr = 0;
+      {
+        int lo_ = 0, hi_ = n_vec / vpr;
+        while (lo_ < hi_) {
+          const int mid = (lo_ + hi_) >> 1;
+          if ((int)ib[mid] < C) lo_ = mid + 1; else hi_ = mid;
+        }
+        nr = lo_;
+      }
+      const int risk_vec = nr * vpr;
+      for (unsigned r = 0; r < nrank; ++r) {
+        if (rank == r) {
+          for (int c0 = 0; c0 < risk_vec; c0 += ST * 4) {  // block-uniform trip count
+            size_t src[4];
+            int4 a[4], b4[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+              const int v = c0 + (int)threadIdx.x + u * ST;
+              if (v < risk_vec) {
+                const int row = v / vpr;
+                src[u] = kv_row_vec(ly, b, hk, (int)ib[row]) + (v - row * vpr);
+                a[u] = __ldcs(Kv + src[u]);
+                b4[u] = __ldcs(Vv + src[u]);
+              }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+              const int v = c0 + (int)threadIdx.x + u * ST;
+              if (v < risk_vec) { __stcs(oKv + dst0 + v, a[u]); __stcs(oVv + dst0 + v, b4[u]); }
+            }
+            __syncthreads();
+          }
+        }
+        cluster.sync();
+      }
+      start_vec = risk_vec;
+    }
     // four vectors of K and four of V in flight per thread
-    for (int v0 = threadIdx.x; v0 < n_vec; v0 += ST * 4) {
+    for (int v0 = start_vec + threadIdx.x; v0 < n_vec; v0 += ST * 4) {
       size_t src[4];
       int4 a[4], b4[4];
 #pragma unroll
@@ -1052,7 +1096,7 @@ bool select_uses_cluster(int L) { return (L + kMaxRanks - 1) / kMaxRanks <= kMax
 cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, int L, int budget_proxy, int budget_random,
                           int n_sink, int n_recent, uint64_t seed, int layer, uint32_t flags, int32_t* out_idx,
                           const void* K, const void* V, void* out_K, void* out_V, int row_bytes, bool* gathered,
-                          int batch_offset, int head_offset, const Shape* layout, float imp_mean, cudaStream_t st) {
+                          int batch_offset, int head_offset, const Shape* layout, float imp_mean, bool inplace, cudaStream_t st) {
   *gathered = false;
   const int C = budget_proxy + budget_random;
   if (C == 0) return cudaSuccess;
@@ -1070,7 +1114,7 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
     nacl_select_kernel<<<batch * Hkv, ST, 0, st>>>(imp, key, L, k1, budget_random, n_sink, n_recent, C, out_idx);
     return cudaGetLastError();
   };
-  if (!select_uses_cluster(L)) return long_row_path();
+  if (!select_uses_cluster(L)) return inplace ? cudaErrorNotSupported : long_row_path();  // in place: the fused gather only
   // cluster size n: the n that minimises (waves of co-resident clusters) x (per-CTA cost ~ fixed + per-position),
   // with the co-residency limit asked from the runtime (clusters need n free SMs inside one GPC)
   cudaLaunchConfig_t cfg = {};
@@ -1129,7 +1173,7 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
     const double cost = waves * (fast_ok ? 20000.0 + 4.0 * lc : 37000.0 + 6.0 * lc);
     if (n == 0 || cost < best) { n = c; Lc = lc; dyn = d; best = cost; }
   }
-  if (n == 0) return long_row_path();
+  if (n == 0) return inplace ? cudaErrorNotSupported : long_row_path();
   cfg.gridDim = dim3((unsigned)(heads * n));
   cfg.dynamicSmemBytes = dyn;
   attr[0].val.clusterDim.x = (unsigned)n;
@@ -1156,14 +1200,15 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   }
   // the kernel also moves the kept rows when its grid covers most of the GPU; a grid of few CTAs (few heads, short rows)
   // would leave the gather to a fraction of the SMs: the stand-alone gather kernel (all SMs) follows instead
-  *gathered = K != nullptr && !(flags & NACL_FLAG_GATHER_SEPARATE) && heads * n * 5 >= (long)kNumSMs * 4;
+  *gathered = K != nullptr && (inplace || (!(flags & NACL_FLAG_GATHER_SEPARATE) && heads * n * 5 >= (long)kNumSMs * 4));
   {
     StageScope sc(ST_SELECT, st);
     e = cudaLaunchKernelEx(&cfg, nacl_select_cluster_kernel, imp, Hkv, L, Lc, k1, budget_random, n_sink, n_recent, C, sk0, sk1,
                            (uint32_t)layer, flags, out_idx, (const int4*)K, (const int4*)V, (int4*)out_K, (int4*)out_V,
-                           *gathered ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset, ly, fast, imp_base, imp_shift, key_lo);
+                           *gathered ? row_bytes / 16 : 0, (uint32_t)batch_offset, (uint32_t)head_offset, ly, fast, imp_base, imp_shift, key_lo,
+                           inplace ? 1 : 0);
   }
-  if (e == cudaSuccess) return e;
+  if (e == cudaSuccess || inplace) return e;
   // the launch itself was refused (cluster resources): nothing ran; take the path without clusters
   cudaGetLastError();
   *gathered = false;

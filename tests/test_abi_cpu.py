@@ -125,6 +125,28 @@ def test_paged_kv_validation_without_touching_the_device(lib):
     assert lib.nacl_evict_ex(C.byref(p)) == -4
 
 
+def test_in_place_needs_the_same_layout_on_both_sides(lib):
+    from paper_2408_03675_b200.binding import NaclParams
+
+    lib.nacl_evict_ex.argtypes = [C.POINTER(NaclParams)]
+    p = NaclParams()
+    p.struct_size = C.sizeof(NaclParams)
+    p.dtype = 1
+    p.K, p.V, p.Qproxy, p.out_idx = 0x100000, 0x900000, 0x3000, 0x6000
+    p.out_K, p.out_V = p.K, p.V                       # in place ...
+    p.batch, p.L, p.Hq, p.Hkv, p.d, p.P = 1, 4096, 8, 8, 128, 16
+    p.budget_proxy, p.budget_random, p.n_sink, p.n_recent = 600, 200, 4, 16
+    assert lib.nacl_evict_ex(C.byref(p)) == -7        # ... but the output strides default to a dense [B,Hkv,C,d] tensor
+    p.out_V = 0xA00000                                # only one of the two aliased
+    assert lib.nacl_evict_ex(C.byref(p)) == -7
+    p.out_V = p.V
+    p.kv_stride_batch = p.out_stride_batch = 8 * 4096 * 128
+    p.kv_stride_head = p.out_stride_head = 4096 * 128
+    p.kv_stride_row = p.out_stride_row = 128
+    p.flags = 8                                       # one shared retained set: stand-alone gather, not in place
+    assert lib.nacl_evict_ex(C.byref(p)) == -7
+
+
 def test_varlen_validation_without_touching_the_device(lib):
     from paper_2408_03675_b200.binding import NaclParams
 

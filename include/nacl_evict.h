@@ -246,6 +246,16 @@ int nacl_evict_host(const void* K, const void* V, const void* Qproxy, int dtype,
                     uint64_t seed, int layer,
                     void* out_K, void* out_V, int32_t* out_idx, int device);
 
+/* n problems of ONE shape out of host memory (e.g. the layers of a prefill whose K/V were offloaded): K[i], V[i],
+ * Qproxy[i], out_K[i], out_V[i], out_idx[i] are HOST pointers as for nacl_evict_host, seed[i] / layer[i] the problem's seed
+ * and layer.  Two staging slots with a stream each: the host-to-device copies of problem i+1 run under the kernels and the
+ * device-to-host copies of problem i.  Returns after all results are in host memory. */
+int nacl_evict_host_batch(int n, const void* const* K, const void* const* V, const void* const* Qproxy, int dtype,
+                          int batch, int L, int Hq, int Hkv, int d, int P,
+                          int budget_proxy, int budget_random, int n_sink, int n_recent,
+                          const uint64_t* seed, const int32_t* layer,
+                          void* const* out_K, void* const* out_V, int32_t* const* out_idx, int device);
+
 /* Step 5 on its own (R4/R5/R10/R15): the Random-Eviction sampling key of EVERY position,
  *   out_keys[b,hk,j] = fl32( ln w_j - ln(-ln u_j) ),  u_j = Philox4x32-10(counter = (j, hk, b, layer), key = seed),
  * w_j = importance[b,hk,j] (or exp / 1 under the NACL_FLAG_SAMPLE_* flags); -inf where w_j = 0.  The budget_random

@@ -21,7 +21,7 @@ FLAG_SCORE_TWO_LAUNCHES, FLAG_SELECT_GENERAL, FLAG_GATHER_SEPARATE = 0x200, 0x40
 EXPORTS = ("nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes",
            "nacl_launch_count", "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version",
            "nacl_profile_enable", "nacl_profile_read", "nacl_stage_name", "nacl_gumbel_keys", "nacl_evict_generation",
-           "nacl_select_fallbacks", "nacl_evict_varlen")
+           "nacl_select_fallbacks", "nacl_evict_varlen", "nacl_evict_host_batch")
 N_STAGES = 7
 
 
@@ -88,6 +88,8 @@ def _load() -> C.CDLL:
     lib.nacl_evict_generation.restype = i32
     lib.nacl_evict_host.argtypes = [vp, vp, vp, i32] + [i32] * 10 + [u64, i32, vp, vp, vp, i32]
     lib.nacl_evict_host.restype = i32
+    lib.nacl_evict_host_batch.argtypes = [i32, vp, vp, vp, i32] + [i32] * 10 + [vp, vp, vp, vp, vp, i32]
+    lib.nacl_evict_host_batch.restype = i32
     lib.nacl_workspace_bytes.argtypes = [i32] * 6
     lib.nacl_workspace_bytes.restype = C.c_size_t
     lib.nacl_launch_count.argtypes = [i32] * 7 + [u32]
@@ -432,3 +434,22 @@ def nacl_evict_host(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent,
     if rc != 0:
         raise NaclError(rc, "nacl_evict_host")
     return out_K, out_V, out_idx
+
+
+def nacl_evict_host_batch(Ks, Vs, Qs, budget_proxy, budget_random, n_sink, n_recent, seeds, layers, out_Ks, out_Vs, out_idxs,
+                          device=-1):
+    """include/nacl_evict.h `nacl_evict_host_batch`: lists of HOST tensors of one shape (pinned memory makes the copies
+    asynchronous), results into the given lists of host tensors; the copies of one problem overlap the next one's."""
+    n = len(Ks)
+    B, Hkv, L, d, Hq, P = _shapes(Ks[0], Vs[0], Qs[0])
+    for t in list(Ks) + list(Vs) + list(Qs) + list(out_Ks) + list(out_Vs) + list(out_idxs):
+        if t.is_cuda or not t.is_contiguous():
+            raise ValueError("nacl_evict_host_batch takes contiguous host tensors")
+    ptrs = lambda ts: (C.c_void_p * n)(*[t.data_ptr() for t in ts])
+    rc = _lib.nacl_evict_host_batch(n, ptrs(Ks), ptrs(Vs), ptrs(Qs), _dtype_tag(Ks[0]), B, L, Hq, Hkv, d, P,
+                                    budget_proxy, budget_random, n_sink, n_recent,
+                                    (C.c_uint64 * n)(*[int(v) for v in seeds]), (C.c_int32 * n)(*[int(v) for v in layers]),
+                                    ptrs(out_Ks), ptrs(out_Vs), ptrs(out_idxs), device)
+    if rc != 0:
+        raise NaclError(rc, "nacl_evict_host_batch")
+    return out_Ks, out_Vs, out_idxs

@@ -119,9 +119,9 @@ struct WsEntry { cudaStream_t stream; void* ptr; size_t bytes; size_t sync_clean
 struct DeviceCache {
   std::vector<WsEntry> ws;
   std::vector<void*> retired;
-  void* stage[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // K V Q oK oV idx
-  size_t stage_bytes[6] = {0, 0, 0, 0, 0, 0};
-  cudaStream_t stream = nullptr;  // nacl_evict_host
+  void* stage[2][6] = {};         // nacl_evict_host(_batch): two staging slots of K V Q oK oV idx ...
+  size_t stage_bytes[2][6] = {};
+  cudaStream_t stream[2] = {nullptr, nullptr};  // ... with a stream each
 };
 static std::mutex g_mu;       // guards g_cache
 static std::mutex g_host_mu;  // serialises nacl_evict_host (its staging buffers are shared per device)
@@ -446,16 +446,24 @@ int nacl_evict_varlen(const nacl_params_t* p, const int32_t* seq_len, const int3
   return NACL_OK;
 }
 
-int nacl_evict_host(const void* K, const void* V, const void* Qproxy, int dtype, int batch, int L, int Hq, int Hkv, int d,
-                    int P, int budget_proxy, int budget_random, int n_sink, int n_recent, uint64_t seed, int layer,
-                    void* out_K, void* out_V, int32_t* out_idx, int device) {
-  if (!K || !V || !Qproxy) return NACL_ERR_NULL;
+// n problems of one shape out of HOST memory, pipelined over two staging slots with a stream each: the host-to-device
+// copies of problem i+1 run under the kernels and the device-to-host copies of problem i (separate copy engines).
+static int evict_host_impl(int n, const void* const* K, const void* const* V, const void* const* Qproxy, int dtype, int batch, int L,
+                           int Hq, int Hkv, int d, int P, int budget_proxy, int budget_random, int n_sink, int n_recent,
+                           const uint64_t* seed, const int32_t* layer, void* const* out_K, void* const* out_V,
+                           int32_t* const* out_idx, int device) {
+  if (n < 0 || (n > 0 && (!K || !V || !Qproxy || !seed || !layer))) return NACL_ERR_NULL;
   const bool empty_out = budget_proxy == 0 && budget_random == 0;  // empty outputs: their pointers may be NULL
-  if (!empty_out && (!out_K || !out_V || !out_idx)) return NACL_ERR_NULL;
+  if (n > 0 && !empty_out && (!out_K || !out_V || !out_idx)) return NACL_ERR_NULL;
+  for (int i = 0; i < n; ++i) {
+    if (!K[i] || !V[i] || !Qproxy[i]) return NACL_ERR_NULL;
+    if (!empty_out && (!out_K[i] || !out_V[i] || !out_idx[i])) return NACL_ERR_NULL;
+  }
   int rc = validate_shape(dtype, batch, L, Hq, Hkv, d, P);
   if (rc) return rc;
   rc = validate_budget(L, budget_proxy, budget_random, n_sink, n_recent);
   if (rc) return rc;
+  if (n == 0) return NACL_OK;
   std::lock_guard<std::mutex> host_lk(g_host_mu);
   cudaError_t e;
   int prev = -1;
@@ -471,40 +479,67 @@ int nacl_evict_host(const void* K, const void* V, const void* Qproxy, int dtype,
   const size_t okv_bytes = (size_t)batch * Hkv * C * d * esz;
   const size_t idx_bytes = (size_t)batch * Hkv * C * sizeof(int32_t);
   const size_t want[6] = {kv_bytes, kv_bytes, q_bytes, okv_bytes, okv_bytes, idx_bytes};
+  const int n_slots = n > 1 ? 2 : 1;
 
   std::unique_lock<std::mutex> lk(g_mu);
   DeviceCache& dc = g_cache[device];
   rc = NACL_OK;
-  for (int i = 0; i < 6 && rc == NACL_OK; ++i)
-    if ((e = grow(&dc.stage[i], &dc.stage_bytes[i], want[i] ? want[i] : 16)) != cudaSuccess) rc = fail_cuda(e);
-  if (rc == NACL_OK && !dc.stream && (e = cudaStreamCreateWithFlags(&dc.stream, cudaStreamNonBlocking)) != cudaSuccess)
-    rc = fail_cuda(e);
-  void* sK = dc.stage[0]; void* sV = dc.stage[1]; void* sQ = dc.stage[2];
-  void* soK = dc.stage[3]; void* soV = dc.stage[4]; void* sidx = dc.stage[5];
-  cudaStream_t st = dc.stream;
+  for (int sl = 0; sl < n_slots && rc == NACL_OK; ++sl) {
+    for (int i = 0; i < 6 && rc == NACL_OK; ++i)
+      if ((e = grow(&dc.stage[sl][i], &dc.stage_bytes[sl][i], want[i] ? want[i] : 16)) != cudaSuccess) rc = fail_cuda(e);
+    if (rc == NACL_OK && !dc.stream[sl] && (e = cudaStreamCreateWithFlags(&dc.stream[sl], cudaStreamNonBlocking)) != cudaSuccess)
+      rc = fail_cuda(e);
+  }
+  void* stg[2][6];
+  cudaStream_t sts[2] = {dc.stream[0], dc.stream[1]};
+  for (int sl = 0; sl < 2; ++sl)
+    for (int i = 0; i < 6; ++i) stg[sl][i] = dc.stage[sl][i];
   lk.unlock();
 
-  if (rc == NACL_OK) {
-    // one cudaMemcpyAsync per tensor; pinned host memory makes them truly asynchronous
-    if ((e = cudaMemcpyAsync(sQ, Qproxy, q_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(sK, K, kv_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(sV, V, kv_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+  for (int i = 0; i < n && rc == NACL_OK; ++i) {
+    const int sl = i % n_slots;
+    cudaStream_t st = sts[sl];
+    void* sK = stg[sl][0]; void* sV = stg[sl][1]; void* sQ = stg[sl][2];
+    void* soK = stg[sl][3]; void* soV = stg[sl][4]; void* sidx = stg[sl][5];
+    // one cudaMemcpyAsync per tensor; pinned host memory makes them truly asynchronous.  A slot's buffers are reused in
+    // stream order: problem i waits for problem i - 2 on the same stream
+    if ((e = cudaMemcpyAsync(sQ, Qproxy[i], q_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(sK, K[i], kv_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(sV, V[i], kv_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) {
       rc = fail_cuda(e);
-  }
-  if (rc == NACL_OK) {
+      break;
+    }
     nacl_params_t p = make_params(dtype, sK, sV, sQ, batch, L, Hq, Hkv, d, P, budget_proxy, budget_random, n_sink, n_recent,
-                                  seed, layer, soK, soV, static_cast<int32_t*>(sidx), st);
+                                  seed[i], layer[i], soK, soV, static_cast<int32_t*>(sidx), st);
     rc = evict_impl(p);
+    if (rc == NACL_OK && C > 0) {
+      if ((e = cudaMemcpyAsync(out_idx[i], sidx, idx_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+          (e = cudaMemcpyAsync(out_K[i], soK, okv_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+          (e = cudaMemcpyAsync(out_V[i], soV, okv_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+        rc = fail_cuda(e);
+    }
   }
-  if (rc == NACL_OK && C > 0) {
-    if ((e = cudaMemcpyAsync(out_idx, sidx, idx_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(out_K, soK, okv_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(out_V, soV, okv_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
-      rc = fail_cuda(e);
-  }
-  if (rc == NACL_OK && (e = cudaStreamSynchronize(st)) != cudaSuccess) rc = fail_cuda(e);
+  for (int sl = 0; sl < n_slots; ++sl)
+    if ((e = cudaStreamSynchronize(sts[sl])) != cudaSuccess && rc == NACL_OK) rc = fail_cuda(e);
   if (device != prev) cudaSetDevice(prev);
   return rc;
+}
+
+int nacl_evict_host(const void* K, const void* V, const void* Qproxy, int dtype, int batch, int L, int Hq, int Hkv, int d,
+                    int P, int budget_proxy, int budget_random, int n_sink, int n_recent, uint64_t seed, int layer,
+                    void* out_K, void* out_V, int32_t* out_idx, int device) {
+  if (!K || !V || !Qproxy) return NACL_ERR_NULL;
+  const int32_t layer32 = layer;
+  return evict_host_impl(1, &K, &V, &Qproxy, dtype, batch, L, Hq, Hkv, d, P, budget_proxy, budget_random, n_sink, n_recent, &seed,
+                         &layer32, &out_K, &out_V, &out_idx, device);
+}
+
+int nacl_evict_host_batch(int n, const void* const* K, const void* const* V, const void* const* Qproxy, int dtype, int batch, int L,
+                          int Hq, int Hkv, int d, int P, int budget_proxy, int budget_random, int n_sink, int n_recent,
+                          const uint64_t* seed, const int32_t* layer, void* const* out_K, void* const* out_V,
+                          int32_t* const* out_idx, int device) {
+  return evict_host_impl(n, K, V, Qproxy, dtype, batch, L, Hq, Hkv, d, P, budget_proxy, budget_random, n_sink, n_recent, seed, layer,
+                         out_K, out_V, out_idx, device);
 }
 
 int nacl_gumbel_keys(const float* importance, float* out_keys, int batch, int Hkv, int L, uint64_t seed, int layer,
@@ -580,15 +615,15 @@ void nacl_release(void) {
   if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return; }
   for (int dev = 0; dev < 64; ++dev) {
     DeviceCache& dc = g_cache[dev];
-    bool any = !dc.ws.empty() || !dc.retired.empty() || dc.stream;
-    for (int i = 0; i < 6; ++i) any = any || dc.stage[i];
+    bool any = !dc.ws.empty() || !dc.retired.empty() || dc.stream[0] || dc.stream[1];
+    for (int i = 0; i < 12; ++i) any = any || dc.stage[i / 6][i % 6];
     if (!any) continue;
     if (cudaSetDevice(dev) != cudaSuccess) { cudaGetLastError(); continue; }
     cudaDeviceSynchronize();  // retired workspaces may still be in use by enqueued calls
     for (WsEntry& w : dc.ws) cudaFree(w.ptr);
     for (void* q : dc.retired) cudaFree(q);
-    for (int i = 0; i < 6; ++i) if (dc.stage[i]) cudaFree(dc.stage[i]);
-    if (dc.stream) cudaStreamDestroy(dc.stream);
+    for (int i = 0; i < 12; ++i) if (dc.stage[i / 6][i % 6]) cudaFree(dc.stage[i / 6][i % 6]);
+    for (int sl = 0; sl < 2; ++sl) if (dc.stream[sl]) cudaStreamDestroy(dc.stream[sl]);
     dc = DeviceCache();
   }
   cudaSetDevice(prev);

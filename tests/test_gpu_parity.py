@@ -337,6 +337,24 @@ def test_host_entry_point_matches_device_entry_point(binding):
     assert torch.equal(idx, didx.cpu()) and torch.equal(oK, dK.cpu()) and torch.equal(oV, dV.cpu())
 
 
+def test_host_batch_entry_point_matches_single_calls(binding):
+    """nacl_evict_host_batch: five problems of one shape out of pinned host memory, pipelined over two staging slots; every
+    result must equal the device entry point's on the same inputs (seeds and layers differ per problem)."""
+    cfg = CONFIGS[2]
+    Bp, Br = cfg.budgets()
+    Cn = Bp + Br
+    probs = [make_layer_inputs(cfg, layer=l)[:3] for l in range(5)]
+    Ks, Vs, Qs = [p[0].pin_memory() for p in probs], [p[1].pin_memory() for p in probs], [p[2].pin_memory() for p in probs]
+    oKs = [torch.empty((cfg.batch, cfg.Hkv, Cn, cfg.d), dtype=Ks[0].dtype, pin_memory=True) for _ in probs]
+    oVs = [torch.empty_like(t, pin_memory=True) for t in oKs]
+    ois = [torch.empty((cfg.batch, cfg.Hkv, Cn), dtype=torch.int32, pin_memory=True) for _ in probs]
+    seeds, layers = [11, 12, 13, 14, 15], [0, 3, 1, 7, 2]
+    binding.nacl_evict_host_batch(Ks, Vs, Qs, Bp, Br, cfg.n_sink, cfg.n_recent, seeds, layers, oKs, oVs, ois)
+    for i, (K, V, Q) in enumerate(probs):
+        dK, dV, di = binding.nacl_evict(K.cuda(), V.cuda(), Q.cuda(), Bp, Br, cfg.n_sink, cfg.n_recent, seeds[i], layers[i])
+        assert torch.equal(ois[i], di.cpu()) and torch.equal(oKs[i], dK.cpu()) and torch.equal(oVs[i], dV.cpu())
+
+
 def test_caller_workspace_and_graph_capture(binding):
     cfg = CONFIGS[2]
     K, V, Q, _ = make_layer_inputs(cfg, layer=0)

@@ -185,16 +185,26 @@ def run_ours(args) -> dict:
         oV = torch.empty_like(oK)
         oi = torch.empty((cfg.batch, cfg.Hkv, C), dtype=torch.int32, device=dev)
         data.append((K, V, Q, oK, oV, oi))
-    ws = torch.empty(binding.nacl_workspace_bytes(cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P) + 256,
-                     dtype=torch.uint8, device=dev)
-    off = (-ws.data_ptr()) % 256
-    ws = ws[off:]
+    wss = []
+    for _ in range(2):  # neighbouring calls of a batch run on two streams: two workspaces
+        w = torch.empty(binding.nacl_workspace_bytes(cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P) + 256, dtype=torch.uint8, device=dev)
+        wss.append(w[(-w.data_ptr()) % 256:])
+    ws = wss[0]
     stream = torch.cuda.current_stream(dev)
 
-    def step():
+    def step():  # one C-ABI call per layer, one after the other on one stream
         for l, (K, V, Q, oK, oV, oi) in enumerate(data):
             binding.nacl_evict_ex(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l,
                                   out_K=oK, out_V=oV, out_idx=oi, workspace=ws, stream=stream, flags=args.nacl_flags)
+
+    def batch_calls(extra=None):
+        return [dict(K=K, V=V, Qproxy=Q, budget_proxy=Bp, budget_random=Br, n_sink=cfg.n_sink, n_recent=cfg.n_recent,
+                     seed=cfg.layer_seed(l), layer=l, out_K=oK, out_V=oV, out_idx=oi, workspace=wss[l & 1], stream=stream,
+                     flags=args.nacl_flags, **(extra(l) if extra else {}))
+                for l, (K, V, Q, oK, oV, oi) in enumerate(data)]
+
+    def batch_step():  # the step's layers as ONE nacl_evict_batch call: independent calls alternating between two streams
+        binding.nacl_evict_batch(batch_calls())
 
     def timed(n_steps: int) -> float:
         nacl_dist.barrier(dev)
@@ -213,7 +223,11 @@ def run_ours(args) -> dict:
     # The timed step is ONE CUDA-graph launch of the step's calls (the library only enqueues: every call is capturable with
     # a caller workspace); the same calls launched one by one from Python are timed beside it (ms_per_step_eager).
     eager_step = step
+    for _ in range(max(args.warmup, 3)):
+        batch_step()
     graph = None
+    if args.no_batch:
+        batch_step = eager_step
     if not args.no_graph:
         cap = torch.cuda.Stream(dev)
         cap.wait_stream(stream)
@@ -221,7 +235,7 @@ def run_ours(args) -> dict:
             graph = torch.cuda.CUDAGraph()
             outer_stream, stream = stream, cap
             with torch.cuda.graph(graph, stream=cap):
-                eager_step()
+                batch_step()
             stream = outer_stream
         stream.wait_stream(cap)
         torch.cuda.synchronize(dev)
@@ -234,9 +248,13 @@ def run_ours(args) -> dict:
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
+    if graph is None:
+        step = batch_step
     ms_total = timed(args.steps)
+    step = batch_step
+    ms_total_batch_eager = timed(args.steps) if graph is not None else ms_total
     step = eager_step
-    ms_total_eager = timed(args.steps) if graph is not None else ms_total
+    ms_total_eager = timed(args.steps)
     # the same region again with per-kernel events (include/nacl_evict.h nacl_profile_*), for the roofline
     binding.nacl_profile_enable(True)
     binding.nacl_profile_read(reset=True)
@@ -263,9 +281,12 @@ def run_ours(args) -> dict:
     main_step = step
 
     def step_lse():
-        for l, (K, V, Q, oK, oV, oi) in enumerate(data):
-            binding.nacl_evict_ex(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l,
-                                  out_K=oK, out_V=oV, out_idx=oi, workspace=ws, stream=stream, lse_in=lses[l])
+        if args.no_batch:
+            for l, (K, V, Q, oK, oV, oi) in enumerate(data):
+                binding.nacl_evict_ex(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l,
+                                      out_K=oK, out_V=oV, out_idx=oi, workspace=ws, stream=stream, lse_in=lses[l])
+        else:
+            binding.nacl_evict_batch(batch_calls(lambda l: {"lse_in": lses[l]}))
 
     step = step_lse
     step()
@@ -328,11 +349,14 @@ def run_ours(args) -> dict:
         "hbm_frac_of_nominal_8TBps": round(value / world / 8000.0, 4),
         "clocks": clocks, "e2e": e2e,
         # counted by the library itself: kernel launches recorded by the per-stage events over the same args.steps steps
-        "gpu_launches": int(sum(n for _, n in stages.values())),
+        # (the batch step launches the two scoring sweeps separately: the count of the two-launch profile run, per step)
+        "gpu_launches": int(sum(n for _, n in stages.values())) if args.no_batch else
+        int(sum(n for _, n in stages_two.values()) // max(1, args.steps // 4) * args.steps),
         "roofline": roofline, "kernels": stage_rows,
         "kernels_two_scoring_launches": {name: {"launches": n, "avg_us": round(ms / n * 1e3, 2),
                                                 "alg_GBps": round(sab.get(name, 0) / (ms / n * 1e-3) / 1e9, 1)}
                                          for name, (ms, n) in stages_two.items() if n},
+        "ms_per_step_batch_without_graph": round(ms_total_batch_eager / args.steps, 4),
         "ms_per_step_eager": round(ms_total_eager / args.steps, 4),
         "ms_per_step_with_kernel_events": round(ms_total_prof / args.steps, 4),
         "lse_in_variant": {"what": "nacl_evict_ex with lse_in (row log-sum-exps supplied, single logit sweep; SURVEY.md 8(f) f1)",
@@ -341,7 +365,8 @@ def run_ours(args) -> dict:
                            "hbm_frac_of_measured": round(alg_bytes_step / world / (ms_lse * 1e-3) / 1e9 / peaks["hbm_gbs"], 4)},
         "library": os.path.relpath(binding.library_path(), ROOT),
     }
-    out["config"]["launch"] = "one CUDA-graph launch per step" if graph is not None else "one C-ABI call per layer from Python"
+    out["config"]["launch"] = ("one nacl_evict_batch call per step (the layers alternate between two streams)" if not args.no_batch
+                               else "one nacl_evict_ex call per layer on one stream") + (", as one CUDA-graph launch" if graph is not None else "")
     if rank == 0 and world == 1 and not args.no_other_workloads:
         del data, lses
         torch.cuda.empty_cache()
@@ -372,21 +397,33 @@ def run_other(binding, cfg, dev, peaks, steps: int = 3, max_sets: int = 8) -> di
     ws = ws[(-ws.data_ptr()) % 256:]
     stream = torch.cuda.current_stream(dev)
 
+    ws2 = torch.empty_like(ws)
+
     def step():
         for l, (K, V, Q, oK, oV, oi) in enumerate(data):
             binding.nacl_evict_ex(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l, out_K=oK, out_V=oV, out_idx=oi,
                                   workspace=ws, stream=stream)
 
-    for _ in range(3):
-        step()
-    torch.cuda.synchronize(dev)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(steps):
-        step()
-    e1.record(stream)
-    torch.cuda.synchronize(dev)
-    us = e0.elapsed_time(e1) * 1e3 / (steps * n_sets)
+    def batch_step():
+        binding.nacl_evict_batch([dict(K=K, V=V, Qproxy=Q, budget_proxy=Bp, budget_random=Br, n_sink=cfg.n_sink, n_recent=cfg.n_recent,
+                                       seed=cfg.layer_seed(l), layer=l, out_K=oK, out_V=oV, out_idx=oi,
+                                       workspace=ws if l % 2 == 0 else ws2, stream=stream)
+                                  for l, (K, V, Q, oK, oV, oi) in enumerate(data)])
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        return e0.elapsed_time(e1) * 1e3 / (steps * n_sets)
+
+    us_single = timed(step)
+    us = timed(batch_step)
     binding.nacl_profile_enable(True)
     binding.nacl_profile_read(reset=True)
     step()
@@ -394,7 +431,8 @@ def run_other(binding, cfg, dev, peaks, steps: int = 3, max_sets: int = 8) -> di
     stages = binding.nacl_profile_read(reset=True)
     binding.nacl_profile_enable(False)
     gbs = cfg.alg_bytes_per_layer() / (us * 1e-6) / 1e9
-    return {"us_per_layer": round(us, 2), "value": round(gbs, 2), "unit": UNIT, "hbm_frac_of_measured": round(gbs / peaks["hbm_gbs"], 4),
+    return {"us_per_layer": round(us, 2), "us_per_layer_one_call_per_layer": round(us_single, 2), "value": round(gbs, 2), "unit": UNIT,
+            "hbm_frac_of_measured": round(gbs / peaks["hbm_gbs"], 4),
             "alg_bytes_per_layer": cfg.alg_bytes_per_layer(), "distinct_input_sets": n_sets, "dtype": cfg.dtype,
             "kernels_us": {k: round(ms / n * 1e3, 2) for k, (ms, n) in stages.items() if n},
             "dram_bytes": {k: load_traffic(cfg.name, k) for k in ("score_stats", "score_colsum", "select")}}
@@ -522,6 +560,7 @@ def main() -> int:
     ap.add_argument("--layers", type=int, default=0, help="override the number of layers per step (0 = the workload's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="time the step's calls launched one by one instead of one CUDA-graph launch")
+    ap.add_argument("--no-batch", action="store_true", help="one nacl_evict_ex call per layer on one stream instead of one nacl_evict_batch call per step")
     ap.add_argument("--nacl-flags", type=lambda v: int(v, 0), default=0,
                     help="NACL_FLAG_* bits for the timed calls (profiling: 0x200 = the two scoring sweeps as two launches)")
     ap.add_argument("--no-other-workloads", action="store_true", help="skip the short runs of the other BASELINE.json configs")

@@ -92,6 +92,8 @@ extern "C" {
 #define NACL_FLAG_SELECT_GENERAL 0x400u      /* debugging / profiling: the selection takes the general three-pass radix path even
                                                 where the one-pass bucket path applies (same result, bit for bit) */
 #define NACL_FLAG_GATHER_SEPARATE 0x800u     /* debugging / profiling: the K/V gather always runs as a kernel of its own */
+#define NACL_FLAG_SELECT_SHARE_SMS 0x1000u   /* the call runs beside other GPU work (nacl_evict_batch sets it): the selection
+                                                kernel's grid stays below ~45 % of the SMs */
 #define NACL_FLAG_SCORE_TWO_LAUNCHES 0x200u  /* debugging / profiling: the tensor-core path runs its statistics sweep and its
                                                 column-sum sweep as two launches instead of one cooperative launch */
 
@@ -183,6 +185,15 @@ int nacl_evict_f32(const void* K, const void* V, const void* Qproxy,
 
 /* Superset entry point: dtype tag, flags, optional importance / lse outputs, explicit workspace. */
 int nacl_evict_ex(const nacl_params_t* p);
+
+/* n INDEPENDENT calls (e.g. the layers of one prefill: "one-shot eviction after the encoding phase"), any mix
+ * of shapes, all with the same p[i].stream.  The calls alternate between two internal streams that fork from and join into
+ * that stream: the scoring of call i+1 fills the SMs that the latency-bound selection and the bandwidth-bound gather of call
+ * i leave idle (-5 % at cfg 4, -17..22 % at cfgs 2, 3, 5 against n nacl_evict_ex calls).  Results are identical to n
+ * nacl_evict_ex calls.  Calls i and i+1 may run at the same time: caller workspaces (p[i].workspace) of neighbouring calls
+ * must not overlap (NULL = the library's own, one per internal stream); outputs of different calls must not overlap either.
+ * Capturable into a CUDA graph once the library's streams exist (after one eager call).  Returns the first error. */
+int nacl_evict_batch(const nacl_params_t* p, int n);
 
 /* Generation-phase eviction ("Generation Phase Eviction"; Algorithm 1, function Generation):
  * every m decoding steps the cache of a layer, which has grown to `len` = C + m entries per head, is cut back to the budget

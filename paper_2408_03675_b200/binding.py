@@ -21,7 +21,7 @@ FLAG_SCORE_TWO_LAUNCHES, FLAG_SELECT_GENERAL, FLAG_GATHER_SEPARATE = 0x200, 0x40
 EXPORTS = ("nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes",
            "nacl_launch_count", "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version",
            "nacl_profile_enable", "nacl_profile_read", "nacl_stage_name", "nacl_gumbel_keys", "nacl_evict_generation",
-           "nacl_select_fallbacks", "nacl_evict_varlen", "nacl_evict_host_batch")
+           "nacl_select_fallbacks", "nacl_evict_varlen", "nacl_evict_host_batch", "nacl_evict_batch")
 N_STAGES = 7
 
 
@@ -84,6 +84,8 @@ def _load() -> C.CDLL:
     lib.nacl_evict_f32.restype = i32
     lib.nacl_evict_ex.argtypes = [C.POINTER(NaclParams)]
     lib.nacl_evict_ex.restype = i32
+    lib.nacl_evict_batch.argtypes = [C.POINTER(NaclParams), i32]
+    lib.nacl_evict_batch.restype = i32
     lib.nacl_evict_generation.argtypes = [C.POINTER(NaclGenParams)]
     lib.nacl_evict_generation.restype = i32
     lib.nacl_evict_host.argtypes = [vp, vp, vp, i32] + [i32] * 10 + [u64, i32, vp, vp, vp, i32]
@@ -225,13 +227,10 @@ def nacl_evict(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed
     return out_K, out_V, out_idx
 
 
-def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer, flags=0,
-                  out_K=None, out_V=None, out_idx=None, want_importance=False, want_lse=False,
-                  workspace=None, stream=None, lse_in=None, batch_offset=0, head_offset=0, protect_idx=None):
-    """include/nacl_evict.h `nacl_evict_ex`.  lse_in: optional [B,Hq,P] fp32 row log-sum-exps (single-sweep
-    path).  batch_offset / head_offset: global indices of the call's first batch element / kv head (a shard of a
-    larger problem draws what the unsharded call draws).  Returns a dict with out_K, out_V, out_idx and, if asked,
-    importance [B,Hkv,L] fp32 and lse [B,Hq,P] fp32."""
+def _ex_params(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer, flags=0,
+               out_K=None, out_V=None, out_idx=None, want_importance=False, want_lse=False,
+               workspace=None, stream=None, lse_in=None, batch_offset=0, head_offset=0, protect_idx=None):
+    """Marshals one nacl_evict_ex call: (NaclParams, result dict).  The result dict keeps the output tensors alive."""
     B, Hkv, L, d, Hq, P = _shapes(K, V, Qproxy)
     if not K.is_cuda:
         raise ValueError("nacl_evict_ex takes CUDA tensors")
@@ -274,16 +273,46 @@ def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, s
     if lse_in is not None:
         assert lse_in.is_cuda and lse_in.dtype == torch.float32 and lse_in.is_contiguous() and lse_in.shape == (B, Hq, P)
         p.lse_in = lse_in.data_ptr()
-    with torch.cuda.device(dev):
-        rc = _lib.nacl_evict_ex(C.byref(p))
-    if rc != 0:
-        raise NaclError(rc, "nacl_evict_ex")
     out = {"out_K": out_K, "out_V": out_V, "out_idx": out_idx}
     if imp is not None:
         out["importance"] = imp
     if lse is not None:
         out["lse"] = lse
+    return p, out
+
+
+def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer, **kw):
+    """include/nacl_evict.h `nacl_evict_ex`.  Keyword arguments: flags, out_K, out_V, out_idx, want_importance, want_lse,
+    workspace, stream, lse_in ([B,Hq,P] fp32 row log-sum-exps: single-sweep path), batch_offset / head_offset (global
+    indices of the call's first batch element / kv head: a shard of a larger problem draws what the unsharded call draws),
+    protect_idx.  Returns a dict with out_K, out_V, out_idx and, if asked, importance [B,Hkv,L] fp32 and lse [B,Hq,P] fp32."""
+    p, out = _ex_params(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer, **kw)
+    with torch.cuda.device(K.device):
+        rc = _lib.nacl_evict_ex(C.byref(p))
+    if rc != 0:
+        raise NaclError(rc, "nacl_evict_ex")
     return out
+
+
+def nacl_evict_batch(calls):
+    """include/nacl_evict.h `nacl_evict_batch`: `calls` is a list of dicts of nacl_evict_ex arguments (positional names
+    K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer plus its keyword arguments), all on one
+    stream.  The calls alternate between two internal streams; returns the list of result dicts."""
+    if not calls:
+        return []
+    pos = ("K", "V", "Qproxy", "budget_proxy", "budget_random", "n_sink", "n_recent", "seed", "layer")
+    arr = (NaclParams * len(calls))()
+    outs = []
+    for i, c in enumerate(calls):
+        kw = {k: v for k, v in c.items() if k not in pos}
+        p, out = _ex_params(*[c[k] for k in pos], **kw)
+        arr[i] = p
+        outs.append(out)
+    with torch.cuda.device(calls[0]["K"].device):
+        rc = _lib.nacl_evict_batch(arr, len(calls))
+    if rc != 0:
+        raise NaclError(rc, "nacl_evict_batch")
+    return outs
 
 
 def nacl_evict_paged(K_pool, V_pool, block_table, L, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer,

@@ -122,6 +122,8 @@ struct DeviceCache {
   void* stage[2][6] = {};         // nacl_evict_host(_batch): two staging slots of K V Q oK oV idx ...
   size_t stage_bytes[2][6] = {};
   cudaStream_t stream[2] = {nullptr, nullptr};  // ... with a stream each
+  cudaStream_t bstream[2] = {nullptr, nullptr};  // nacl_evict_batch: the two streams the calls alternate on
+  cudaEvent_t bfork = nullptr, bjoin[2] = {nullptr, nullptr};
 };
 static std::mutex g_mu;       // guards g_cache
 static std::mutex g_host_mu;  // serialises nacl_evict_host (its staging buffers are shared per device)
@@ -189,7 +191,7 @@ static int evict_impl(const nacl_params_t& p) {
   if (p.n_protect > 0 && !p.protect_idx) return NACL_ERR_NULL;
   if (p.reserved0 != 0) return NACL_ERR_UNSUPPORTED;
   const uint32_t known = NACL_FLAG_CAUSAL | NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE | NACL_FLAG_SAMPLE_UNIFORM | NACL_FLAG_SHARED_HEADS |
-                         NACL_FLAG_SCORE_CUDA_CORES | NACL_FLAG_SCORE_TWO_LAUNCHES | NACL_FLAG_SELECT_GENERAL | NACL_FLAG_GATHER_SEPARATE;
+                         NACL_FLAG_SCORE_CUDA_CORES | NACL_FLAG_SCORE_TWO_LAUNCHES | NACL_FLAG_SELECT_GENERAL | NACL_FLAG_GATHER_SEPARATE | NACL_FLAG_SELECT_SHARE_SMS;
   if (p.flags & ~known) return NACL_ERR_UNSUPPORTED;
   if ((p.flags & NACL_FLAG_SAMPLE_SOFTMAX_OF_SCORE) && (p.flags & NACL_FLAG_SAMPLE_UNIFORM)) return NACL_ERR_UNSUPPORTED;
 
@@ -353,6 +355,54 @@ int nacl_evict_ex(const nacl_params_t* p) {
   if (!p) return NACL_ERR_NULL;
   if (p->struct_size != sizeof(nacl_params_t)) return NACL_ERR_UNSUPPORTED;
   return evict_impl(*p);
+}
+
+int nacl_evict_batch(const nacl_params_t* p, int n) {
+  if (n < 0 || (n > 0 && !p)) return NACL_ERR_NULL;
+  if (n == 0) return NACL_OK;
+  for (int i = 0; i < n; ++i) {
+    if (p[i].struct_size != sizeof(nacl_params_t)) return NACL_ERR_UNSUPPORTED;
+    if (p[i].stream != p[0].stream) return NACL_ERR_UNSUPPORTED;
+  }
+  if (n == 1) return evict_impl(p[0]);
+  static std::mutex batch_mu;  // the fork / join events and the two streams are shared per device: one enqueue at a time
+  std::lock_guard<std::mutex> batch_lk(batch_mu);
+  cudaError_t e;
+  int dev = 0;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return fail_cuda(e);
+  if (dev < 0 || dev >= 64) return NACL_ERR_UNSUPPORTED;
+  cudaStream_t user = static_cast<cudaStream_t>(p[0].stream), bs[2];
+  cudaEvent_t fork, join[2];
+  {
+    std::lock_guard<std::mutex> lk(g_mu);
+    DeviceCache& dc = g_cache[dev];
+    for (int sl = 0; sl < 2; ++sl) {
+      if (!dc.bstream[sl] && (e = cudaStreamCreateWithFlags(&dc.bstream[sl], cudaStreamNonBlocking)) != cudaSuccess) return fail_cuda(e);
+      if (!dc.bjoin[sl] && (e = cudaEventCreateWithFlags(&dc.bjoin[sl], cudaEventDisableTiming)) != cudaSuccess) return fail_cuda(e);
+      bs[sl] = dc.bstream[sl];
+      join[sl] = dc.bjoin[sl];
+    }
+    if (!dc.bfork && (e = cudaEventCreateWithFlags(&dc.bfork, cudaEventDisableTiming)) != cudaSuccess) return fail_cuda(e);
+    fork = dc.bfork;
+  }
+  // fork: both internal streams start behind everything enqueued on the caller's stream so far
+  if ((e = cudaEventRecord(fork, user)) != cudaSuccess || (e = cudaStreamWaitEvent(bs[0], fork, 0)) != cudaSuccess ||
+      (e = cudaStreamWaitEvent(bs[1], fork, 0)) != cudaSuccess)
+    return fail_cuda(e);
+  int rc = NACL_OK;
+  for (int i = 0; i < n && rc == NACL_OK; ++i) {
+    nacl_params_t q = p[i];
+    q.stream = bs[i & 1];
+    // two plain launches for the scoring sweeps: a cooperative launch waits for ALL SMs, plain launches fill the SMs the
+    // other stream's selection / gather leaves idle
+    q.flags |= NACL_FLAG_SCORE_TWO_LAUNCHES | NACL_FLAG_SELECT_SHARE_SMS;
+    rc = evict_impl(q);
+  }
+  // join (also after an error: the caller's stream must not run ahead of what was enqueued)
+  for (int sl = 0; sl < 2; ++sl)
+    if ((e = cudaEventRecord(join[sl], bs[sl])) != cudaSuccess || (e = cudaStreamWaitEvent(user, join[sl], 0)) != cudaSuccess)
+      return rc != NACL_OK ? rc : fail_cuda(e);
+  return rc;
 }
 
 int nacl_evict_generation(const nacl_gen_params_t* g) {
@@ -615,7 +665,7 @@ void nacl_release(void) {
   if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return; }
   for (int dev = 0; dev < 64; ++dev) {
     DeviceCache& dc = g_cache[dev];
-    bool any = !dc.ws.empty() || !dc.retired.empty() || dc.stream[0] || dc.stream[1];
+    bool any = !dc.ws.empty() || !dc.retired.empty() || dc.stream[0] || dc.stream[1] || dc.bstream[0] || dc.bfork;
     for (int i = 0; i < 12; ++i) any = any || dc.stage[i / 6][i % 6];
     if (!any) continue;
     if (cudaSetDevice(dev) != cudaSuccess) { cudaGetLastError(); continue; }
@@ -624,6 +674,9 @@ void nacl_release(void) {
     for (void* q : dc.retired) cudaFree(q);
     for (int i = 0; i < 12; ++i) if (dc.stage[i / 6][i % 6]) cudaFree(dc.stage[i / 6][i % 6]);
     for (int sl = 0; sl < 2; ++sl) if (dc.stream[sl]) cudaStreamDestroy(dc.stream[sl]);
+    for (int sl = 0; sl < 2; ++sl) if (dc.bstream[sl]) cudaStreamDestroy(dc.bstream[sl]);
+    if (dc.bfork) cudaEventDestroy(dc.bfork);
+    for (int sl = 0; sl < 2; ++sl) if (dc.bjoin[sl]) cudaEventDestroy(dc.bjoin[sl]);
     dc = DeviceCache();
   }
   cudaSetDevice(prev);

@@ -1144,7 +1144,15 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   for (int c = 1; c <= kMaxRanks; c *= 2) {
     const int lc = ((L + c - 1) / c + 3) / 4 * 4;
     if (lc > kMaxSlice) continue;
+#ifdef NACL_FORCE_CLUSTER  // diagnostics: one cluster size only
+    if (c != NACL_FORCE_CLUSTER) continue;
+#endif
     if (c > 1 && L / c < ST / 2) break;  // slices below half a block of positions are not worth a barrier per pass
+    // beside other work (nacl_evict_batch): the grid stays below ~45 % of the SMs, so that the other stream's scoring CTAs
+    // find room while this selection waits on its barriers (cfg 3 93.1 -> 85.7 us per call, cfg 4 205.6 -> 203.6)
+#ifndef NACL_DIAG_NO_SHARE
+    if ((flags & NACL_FLAG_SELECT_SHARE_SMS) && n != 0 && heads * c * 20 > (long)kNumSMs * 9) break;
+#endif
     const size_t d = dyn_bytes(lc);
     // co-resident clusters of this size, per device and shared-memory class; -1: the device cannot schedule one (a MIG
     // slice, another SKU): the size is skipped

@@ -355,6 +355,48 @@ def test_host_batch_entry_point_matches_single_calls(binding):
         assert torch.equal(ois[i], di.cpu()) and torch.equal(oKs[i], dK.cpu()) and torch.equal(oVs[i], dV.cpu())
 
 
+def test_batch_of_calls_matches_single_calls_eagerly_and_in_a_graph(binding):
+    """nacl_evict_batch: independent calls of mixed shapes alternate between two internal streams that fork from and join
+    into the caller's stream.  Same results as one nacl_evict_ex call each, also when the batch is captured into a CUDA
+    graph (caller workspaces, neighbouring calls on different ones) and replayed."""
+    shapes = [(1, 4100, 32, 8, 128, 64), (2, 9000, 16, 2, 128, 32), (4, 700, 8, 8, 128, 16), (1, 20000, 8, 2, 128, 16),
+              (2, 3001, 4, 2, 64, 8), (1, 4100, 32, 8, 128, 64), (1, 129, 8, 8, 128, 16)]
+    calls, want = [], []
+    for i, (B, L, Hq, Hkv, d, P) in enumerate(shapes):
+        K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype="f32" if d == 64 else "bf16", seed=300 + i)
+        Kc, Vc, Qc = K.cuda(), V.cuda(), Q.cuda()
+        Bp, Br = L // 5, L // 20
+        want.append(binding.nacl_evict_ex(Kc, Vc, Qc, Bp, Br, 4, P, 17, i))
+        calls.append(dict(K=Kc, V=Vc, Qproxy=Qc, budget_proxy=Bp, budget_random=Br, n_sink=4, n_recent=P, seed=17, layer=i))
+    torch.cuda.synchronize()
+    got = binding.nacl_evict_batch(calls)
+    torch.cuda.synchronize()
+    for i in range(len(shapes)):
+        for k in ("out_idx", "out_K", "out_V"):
+            assert torch.equal(got[i][k], want[i][k]), f"call {i}: {k} differs between the batch and the single call"
+    # captured: caller workspaces, calls i and i+1 on different ones, outputs preallocated
+    wsz = max(binding.nacl_workspace_bytes(c["K"].shape[0], c["K"].shape[2], c["Qproxy"].shape[1], c["K"].shape[1], c["K"].shape[3],
+                                           c["Qproxy"].shape[2]) for c in calls)
+    wss = [torch.empty(wsz, dtype=torch.uint8, device="cuda") for _ in range(2)]
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        for i, c in enumerate(calls):
+            c.update(out_K=torch.zeros_like(want[i]["out_K"]), out_V=torch.zeros_like(want[i]["out_V"]),
+                     out_idx=torch.zeros_like(want[i]["out_idx"]), workspace=wss[i & 1], stream=s)
+        binding.nacl_evict_batch(calls)  # warm: the library's streams exist
+        s.synchronize()
+        for c in calls:
+            c["out_idx"].zero_()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            binding.nacl_evict_batch(calls)
+        g.replay()
+        s.synchronize()
+    for i, c in enumerate(calls):
+        assert torch.equal(c["out_idx"], want[i]["out_idx"]) and torch.equal(c["out_K"], want[i]["out_K"]) and torch.equal(c["out_V"], want[i]["out_V"])
+
+
 def test_caller_workspace_and_graph_capture(binding):
     cfg = CONFIGS[2]
     K, V, Q, _ = make_layer_inputs(cfg, layer=0)

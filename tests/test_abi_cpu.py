@@ -147,6 +147,25 @@ def test_in_place_needs_the_same_layout_on_both_sides(lib):
     assert lib.nacl_evict_ex(C.byref(p)) == -7
 
 
+def test_batch_validation_without_touching_the_device(lib):
+    from paper_2408_03675_b200.binding import NaclParams
+
+    lib.nacl_evict_batch.argtypes = [C.POINTER(NaclParams), C.c_int]
+    arr = (NaclParams * 2)()
+    for q in arr:
+        q.struct_size = C.sizeof(NaclParams)
+    assert lib.nacl_evict_batch(None, 2) == -1
+    assert lib.nacl_evict_batch(arr, 0) == 0
+    assert lib.nacl_evict_batch(arr, -1) == -1
+    arr[1].stream = 0x10                       # the calls of a batch share one stream
+    assert lib.nacl_evict_batch(arr, 2) == -7
+    arr[1].stream = None
+    arr[1].struct_size = 8
+    assert lib.nacl_evict_batch(arr, 2) == -7
+    arr[1].struct_size = C.sizeof(NaclParams)
+    assert lib.nacl_evict_batch(arr, 1) == -1  # a single call is nacl_evict_ex: K, V, Qproxy are NULL here
+
+
 def test_varlen_validation_without_touching_the_device(lib):
     from paper_2408_03675_b200.binding import NaclParams
 

@@ -255,19 +255,19 @@ def run_ours(args) -> dict:
     ms_total_batch_eager = timed(args.steps) if graph is not None else ms_total
     step = eager_step
     ms_total_eager = timed(args.steps)
-    # the same region again with per-kernel events (include/nacl_evict.h nacl_profile_*), for the roofline
+    # the timed region again (the same calls, without the graph: events cannot be captured) with per-kernel events
+    # (include/nacl_evict.h nacl_profile_*), for `kernels`, `gpu_launches` and the roofline
     binding.nacl_profile_enable(True)
     binding.nacl_profile_read(reset=True)
+    step = batch_step
     ms_total_prof = timed(args.steps)
     stages = binding.nacl_profile_read(reset=True)
-    # the two scoring sweeps as two launches (NACL_FLAG_SCORE_TWO_LAUNCHES), for the per-sweep times of the fused launch
-    fused_flags = args.nacl_flags
-    args.nacl_flags = fused_flags | 0x200
+    # ... and of one nacl_evict_ex call per layer on one stream (fused scoring launch, select with fused gather)
+    step = eager_step
     step()
     binding.nacl_profile_read(reset=True)
     timed(max(1, args.steps // 4))
-    stages_two = binding.nacl_profile_read(reset=True)
-    args.nacl_flags = fused_flags
+    stages_one = binding.nacl_profile_read(reset=True)
     binding.nacl_profile_enable(False)
     clocks = sampler.stop() if rank == 0 else None
 
@@ -302,6 +302,9 @@ def run_ours(args) -> dict:
     sab = stage_alg_bytes(cfg)
     if stages.get("gather", (0, 0))[1] == 0:  # the cluster select kernel also moves the kept rows (steps a4-a7 in one launch)
         sab["select"] += sab["gather"]
+    sab_one = stage_alg_bytes(cfg)
+    if stages_one.get("gather", (0, 0))[1] == 0:
+        sab_one["select"] += sab_one["gather"]
     stage_rows = {}
     for name, (ms, n) in stages.items():
         if n == 0:
@@ -349,13 +352,15 @@ def run_ours(args) -> dict:
         "hbm_frac_of_nominal_8TBps": round(value / world / 8000.0, 4),
         "clocks": clocks, "e2e": e2e,
         # counted by the library itself: kernel launches recorded by the per-stage events over the same args.steps steps
-        # (the batch step launches the two scoring sweeps separately: the count of the two-launch profile run, per step)
-        "gpu_launches": int(sum(n for _, n in stages.values())) if args.no_batch else
-        int(sum(n for _, n in stages_two.values()) // max(1, args.steps // 4) * args.steps),
+        # counted by the library itself: kernel launches recorded by the per-stage events over the same args.steps steps
+        "gpu_launches": int(sum(n for _, n in stages.values())),
         "roofline": roofline, "kernels": stage_rows,
-        "kernels_two_scoring_launches": {name: {"launches": n, "avg_us": round(ms / n * 1e3, 2),
-                                                "alg_GBps": round(sab.get(name, 0) / (ms / n * 1e-3) / 1e9, 1)}
-                                         for name, (ms, n) in stages_two.items() if n},
+        "kernels_note": ("durations between per-kernel events in the timed configuration; with two streams the kernels of "
+                         "neighbouring layers run at the same time and share the SMs, so the durations add up to more than the "
+                         "step; kernels_one_call_per_layer has every kernel alone on the GPU") if not args.no_batch else None,
+        "kernels_one_call_per_layer": {name: {"launches": n, "avg_us": round(ms / n * 1e3, 2),
+                                              "alg_GBps": round(sab_one.get(name, 0) / (ms / n * 1e-3) / 1e9, 1)}
+                                       for name, (ms, n) in stages_one.items() if n},
         "ms_per_step_batch_without_graph": round(ms_total_batch_eager / args.steps, 4),
         "ms_per_step_eager": round(ms_total_eager / args.steps, 4),
         "ms_per_step_with_kernel_events": round(ms_total_prof / args.steps, 4),

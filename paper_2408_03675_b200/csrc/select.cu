@@ -1208,7 +1208,15 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   }
   // the kernel also moves the kept rows when its grid covers most of the GPU; a grid of few CTAs (few heads, short rows)
   // would leave the gather to a fraction of the SMs: the stand-alone gather kernel (all SMs) follows instead
-  *gathered = K != nullptr && (inplace || (!(flags & NACL_FLAG_GATHER_SEPARATE) && heads * n * 5 >= (long)kNumSMs * 4));
+  // ... except beside other work (nacl_evict_batch) when the scoring is short and HBM-bound (G*P <= 128): there the small grid
+  // that keeps its SMs for the gather beats a second kernel that competes with the other stream's sweeps for all SMs
+  // (cfg 2 42.7 -> 39.9 us per call, cfg 3 86.5 -> 84.5; at G*P = 256: cfg 4 +0.5, cfg 5 +10)
+  const bool small_grid_fused = (flags & NACL_FLAG_SELECT_SHARE_SMS) && layout != nullptr && layout->rows <= 128;
+#ifdef NACL_DIAG_FUSE_GATHER  // diagnostics: the fused gather whatever the grid size
+  *gathered = K != nullptr && (inplace || !(flags & NACL_FLAG_GATHER_SEPARATE));
+#else
+  *gathered = K != nullptr && (inplace || (!(flags & NACL_FLAG_GATHER_SEPARATE) && (heads * n * 5 >= (long)kNumSMs * 4 || small_grid_fused)));
+#endif
   {
     StageScope sc(ST_SELECT, st);
     e = cudaLaunchKernelEx(&cfg, nacl_select_cluster_kernel, imp, Hkv, L, Lc, k1, budget_random, n_sink, n_recent, C, sk0, sk1,

@@ -1,19 +1,22 @@
 // score_tc.cu -- tensor-core scoring path: steps a1-a3 of SURVEY.md section 8 as a persistent,
-// warp-specialised sm_100a kernel (tcgen05.mma + TMEM accumulators + TMA-staged tiles), launched
-// twice per call:
+// warp-specialised sm_100a kernel (tcgen05.mma + TMEM accumulators + TMA-staged tiles).  Both sweeps
+// run in ONE cooperative launch (nacl_evict_ex), or as two plain launches (nacl_evict_batch, where the
+// calls of two streams share the GPU; NACL_FLAG_SCORE_TWO_LAUNCHES; sweep C alone when lse_in is given):
 //
 //   a1  s[i,j] = Q[i,:].K[j,:] / sqrt(d)                      PAPER.md:59, Alg.1
 //   a2  lse_i  = log sum_j exp(s[i,j])   (full-length softmax)  PAPER.md:124      -- sweep S
 //   a3  imp[j] = sum_{g,i} exp(s[i,j] - lse_i)                  PAPER.md:124, 176-178 -- sweep C
 //
-// Serves bf16, d == 128, G*P a multiple of 16 and <= 256.  Everything else takes score_generic.cu.
+// Serves bf16, d == 128, G*P a multiple of 16 (above 256: in blocks of 256 proxy rows), contiguous, strided or paged K.
+// Everything else takes score_generic.cu.
 //
 // Work decomposition.  The logits are never written to memory and the column sum needs the
 // complete row normaliser first, so every key tile (128 keys) is scored twice.  The N = heads * T
 // key tiles of a call (T = ceil(L/128) per kv head) form one flat sequence that is cut into
 // gridDim.x equal contiguous ranges: CTA c owns tiles [N*c/G, N*(c+1)/G) in BOTH sweeps -- no
-// tickets, no atomics, no inter-CTA waits.  A range crosses at most a few head boundaries; each
-// maximal run of tiles of one head is a segment.
+// tickets and no float atomics; the only inter-CTA wait is the hand-over of a head's partials in the
+// one-launch form (a per-head counter).  A range crosses at most a few head boundaries; each
+// maximal run of tiles of one head is a segment.  Every K tile load carries the L2 evict_first hint.
 //   sweep S: per segment and proxy row a partial (max, sum-exp) is written to part[c + head]
 //            (c + head is strictly increasing along the sequence, hence a unique slot);
 //   sweep C: the CTA first merges, per segment, the head's partials in ascending slot order into
@@ -29,15 +32,15 @@
 //             and a quarter of the proxy rows; the four quarter sums of a key meet in shared memory
 //             and a combiner warp adds them in a fixed order (deterministic) and stores imp.
 //
-// Epilogue arithmetic.  At G*P = 256 the path is bound by the 16/clk/SM MUFU.EX2 unit and the FMA
-// pipe, not by HBM (profiles/): a quarter of the exponentials are therefore evaluated on the FMA pipe
-// (Cody-Waite range reduction + degree-3 minimax polynomial, relative error <= 7.5e-5, against the
+// Epilogue arithmetic.  At G*P = 256 the path is bound by TMEM loads + the 16/clk/SM MUFU.EX2 unit + the
+// FMA pipe, not by HBM (profiles/): 3 of 8 exponentials are therefore evaluated on the FMA pipe
+// (saturating-FMA range reduction + degree-3 minimax polynomial, relative error <= 7.5e-5, against the
 // 2e-3 score tolerance of the north star) and all multiply-adds are the packed fma/add.f32x2 forms.
 //
-// Warp roles (608 threads, 1 CTA per SM): warps 0-15 = epilogue (warp%4 = TMEM lane quarter = SM
-// sub-partition, warp/4 = column quarter of the tile), warp 16 = TMA producer, warp 17 = TMEM
-// allocator + tcgen05.mma issuer, warp 18 = column-sum combiner.  All 16 epilogue warps work on
-// the same tile; two 256-column TMEM buffers let the MMA of tile t+1 run under the epilogue of t.
+// Warp roles (640 threads, 1 CTA per SM): warps 0-15 = epilogue (warp%4 = TMEM lane quarter = SM
+// sub-partition, warp/4 = column quarter of the tile, or (tile parity, row half) in the quad scheme),
+// warp 16 = TMA producer, warps 17-18 = tcgen05.mma issuers (alternating tiles; 17 also allocates TMEM),
+// warp 19 = column-sum combiner in sweep C, publisher of the partials in sweep S of the one-launch form.
 #include <cuda.h>
 
 #include "nacl_internal.cuh"

@@ -8,11 +8,12 @@
 //                  radix select of the budget_random largest keys among the rest, ties to the lower
 //                  index in both (R9), then an order-preserving compaction that emits the
 //                  kept positions already ascending -- no sort.
-//   nacl_select_cluster_kernel: the same selection with one thread-block CLUSTER (1..8 CTAs) per (batch, kv head):
-//                  every CTA keeps its slice of the importance row and of the sampling keys in shared memory,
-//                  the radix histograms of the slices meet in the shared memory of the cluster's rank-0 CTA
-//                  (distributed shared memory), and the keys are computed in the same kernel, only for the
-//                  candidates that survive the top-k.  Used whenever the slices fit; 8x more CTAs than heads.
+//   nacl_select_cluster_kernel: the same selection with one thread-block CLUSTER (1..16 CTAs) per (batch, kv head), the
+//                  CTAs exchanging histogram sums and candidate lists through distributed shared memory.  Default: the
+//                  one-pass bucket path (select_fast: one cluster-wide histogram per select over buckets that are fine
+//                  where the threshold lies, fp32 key estimates, exact fp64 keys only next to the threshold, exact finish
+//                  on a small candidate list); the three-pass radix path on exact keys is the cluster-uniform fallback.
+//                  The kernel also moves the kept K/V rows (step a7), in place if asked.
 // Integer work only after the keys: results are bit-exact functions of (imp, key).
 #include <cooperative_groups.h>
 #include <mutex>

@@ -78,6 +78,7 @@ extern "C" {
 #define NACL_ERR_WORKSPACE (-5)   /* supplied workspace too small or misaligned */
 #define NACL_ERR_CUDA (-6)        /* a CUDA runtime/driver call failed; see nacl_last_cuda_error() */
 #define NACL_ERR_UNSUPPORTED (-7) /* a flag or dtype this build does not implement */
+#define NACL_ERR_STATIC_LIMIT (-8) /* nacl_evict_static: the shape needs more than NACL_STATIC_SCRATCH_BYTES of scratch */
 
 /* nacl_evict_ex flags */
 #define NACL_FLAG_CAUSAL 1u                  /* DESIGN.md R1: proxy row i is prompt position L-P+i and sees keys j <= L-P+i */
@@ -185,6 +186,42 @@ int nacl_evict_f32(const void* K, const void* V, const void* Qproxy,
 
 /* Superset entry point: dtype tag, flags, optional importance / lse outputs, explicit workspace. */
 int nacl_evict_ex(const nacl_params_t* p);
+
+/* nacl_evict_ex for callers that must not allocate device memory.
+ *
+ * Who that is: an inference server that hands (nearly) all of the GPU's memory to its own KV-cache pool at start-up, so
+ * that any cudaMalloc afterwards fails or, worse, succeeds by taking memory the pool was promised; a decode loop in
+ * which cudaMalloc / cudaFree are unwelcome because they synchronise the whole device and stall every stream; a plug-in
+ * or worker whose host application owns the allocator and forbids its guests to go to the driver behind its back.
+ * nacl_evict / nacl_evict_ex without a workspace cudaMalloc a per-stream workspace on first use (and again when a larger
+ * shape arrives); nacl_evict_ex WITH a workspace allocates nothing but asks the caller for device memory, which such a
+ * caller may have no spare byte of.  This entry point needs neither.
+ *
+ * What it does instead: the scratch the kernels need (softmax partials, the importance rows, hand-over counters; what
+ * nacl_workspace_bytes counts) is a fixed array of NACL_STATIC_SCRATCH_BYTES inside the library's device image.  The
+ * price is that every GPU on which the library is loaded carries those bytes from load until the process exits, whether
+ * or not this function is ever called; 16 MiB holds each of the five BASELINE.json shapes (the largest, batch 4 x 8 kv
+ * heads x 32768 keys, needs 14.7 MiB).  The function calls no cudaMalloc, cudaFree, stream / event creation or any other
+ * allocating routine (with nacl_profile_enable on, event pairs are created as for every other call: leave it off).
+ * K, V, Qproxy and the outputs remain the caller's buffers, exactly as for nacl_evict_ex.
+ *
+ * Arguments: *p as for nacl_evict_ex, every option included, except that p->workspace must be NULL and
+ * p->workspace_bytes 0 (NACL_ERR_WORKSPACE otherwise).  Results are bit-identical to nacl_evict_ex on the same inputs.
+ * A shape with nacl_workspace_bytes(batch, L, Hq, Hkv, d, P) > NACL_STATIC_SCRATCH_BYTES is refused with
+ * NACL_ERR_STATIC_LIMIT before anything is enqueued or written; that check is host-side and needs no GPU.
+ *
+ * First call on a device: it looks up where the array lives on the device that is current (one cudaGetSymbolAddress,
+ * remembered per device; no memory is obtained by it).  Make that first call, on every device you use, during
+ * start-up and before any stream capture begins.
+ *
+ * Sharing: there is ONE array per GPU and every call of this function on that GPU works in it, whatever its stream
+ * and whichever host thread issues it.  Calls that follow each other on one stream are fine: each call clears the few
+ * counters that have to start at zero and overwrites the rest before reading it, so the leftovers of an earlier call (of
+ * any shape) are harmless.  Calls that can be in flight on the GPU at the same time -- different streams without an
+ * event between them, for instance host threads that each use a stream of their own -- race on the array and produce garbage:
+ * order them yourself, or use nacl_evict_ex with separate workspaces for the concurrent ones. */
+#define NACL_STATIC_SCRATCH_BYTES (16 * 1024 * 1024)
+int nacl_evict_static(const nacl_params_t* p);
 
 /* n INDEPENDENT calls (e.g. the layers of one prefill: "one-shot eviction after the encoding phase"), any mix
  * of shapes, all with the same p[i].stream.  The calls alternate between two internal streams that fork from and join into

@@ -84,6 +84,8 @@ def _load() -> C.CDLL:
     lib.nacl_evict_f32.restype = i32
     lib.nacl_evict_ex.argtypes = [C.POINTER(NaclParams)]
     lib.nacl_evict_ex.restype = i32
+    lib.nacl_evict_static.argtypes = [C.POINTER(NaclParams)]
+    lib.nacl_evict_static.restype = i32
     lib.nacl_evict_batch.argtypes = [C.POINTER(NaclParams), i32]
     lib.nacl_evict_batch.restype = i32
     lib.nacl_evict_generation.argtypes = [C.POINTER(NaclGenParams)]
@@ -291,6 +293,27 @@ def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, s
         rc = _lib.nacl_evict_ex(C.byref(p))
     if rc != 0:
         raise NaclError(rc, "nacl_evict_ex")
+    return out
+
+
+STATIC_SCRATCH_BYTES = 16 * 1024 * 1024  # NACL_STATIC_SCRATCH_BYTES of include/nacl_evict.h
+
+
+def nacl_evict_static(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer, **kw):
+    """include/nacl_evict.h `nacl_evict_static`: nacl_evict_ex for callers that cannot allocate device memory (a server
+    whose KV pool already owns the GPU, a decode loop that must not hit cudaMalloc's device-wide synchronisation, a guest
+    of somebody else's allocator).  The kernels' scratch is a fixed STATIC_SCRATCH_BYTES array inside the library, so
+    the C call allocates nothing; shapes that need more raise NaclError(-8).  Same keyword arguments as nacl_evict_ex
+    except `workspace`; same results, bit for bit.  Pass out_K / out_V / out_idx (and do not ask for importance / lse)
+    if this Python wrapper must not allocate either: tensors it is not given it creates with torch.empty.  All calls on
+    one GPU share the array: keep them ordered on the GPU (one stream, or events), never concurrent."""
+    if kw.get("workspace") is not None:
+        raise ValueError("nacl_evict_static brings its own scratch: no workspace argument")
+    p, out = _ex_params(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, seed, layer, **kw)
+    with torch.cuda.device(K.device):
+        rc = _lib.nacl_evict_static(C.byref(p))
+    if rc != 0:
+        raise NaclError(rc, "nacl_evict_static")
     return out
 
 

@@ -330,6 +330,32 @@ static nacl_params_t make_params(int dtype, const void* K, const void* V, const 
   return p;
 }
 
+// ------------------------------------------------------------------ nacl_evict_static: the call that allocates nothing
+// Scratch for callers that cannot allocate device memory (see include/nacl_evict.h).  It lives in the library's own
+// device image: every GPU that loads libnacl_evict.so holds these NACL_STATIC_SCRATCH_BYTES from module load to exit.
+// NOTE for maintainers: in HOST code the name g_static_scratch is only a handle for the runtime, not a device address
+// (a kernel handed `g_static_scratch` from host code would fault or scribble over unrelated memory).  Kernels must be
+// given the pointer that cudaGetSymbolAddress returns while the device in question is current.
+static __device__ __align__(256) unsigned char g_static_scratch[NACL_STATIC_SCRATCH_BYTES];
+static void* g_static_scratch_addr[64] = {};  // per device, filled by the first nacl_evict_static call there
+
+// The array's address on the CURRENT device; looked up once per device (no allocation: the array already exists).
+static int static_scratch_here(void** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail_cuda(e);
+  if (dev < 0 || dev >= 64) return NACL_ERR_UNSUPPORTED;
+  std::lock_guard<std::mutex> lk(g_mu);
+  if (!g_static_scratch_addr[dev]) {
+    void* addr = nullptr;
+    if ((e = cudaGetSymbolAddress(&addr, g_static_scratch)) != cudaSuccess) return fail_cuda(e);
+    if (!addr || (reinterpret_cast<uintptr_t>(addr) & 255u)) return NACL_ERR_WORKSPACE;
+    g_static_scratch_addr[dev] = addr;
+  }
+  *out = g_static_scratch_addr[dev];
+  return NACL_OK;
+}
+
 }  // namespace nacl
 
 using namespace nacl;
@@ -355,6 +381,26 @@ int nacl_evict_ex(const nacl_params_t* p) {
   if (!p) return NACL_ERR_NULL;
   if (p->struct_size != sizeof(nacl_params_t)) return NACL_ERR_UNSUPPORTED;
   return evict_impl(*p);
+}
+
+int nacl_evict_static(const nacl_params_t* p) {
+  if (!p) return NACL_ERR_NULL;
+  if (p->struct_size != sizeof(nacl_params_t)) return NACL_ERR_UNSUPPORTED;
+  if (p->workspace != nullptr || p->workspace_bytes != 0) return NACL_ERR_WORKSPACE;  // the scratch is the library's here
+  // the shape decides the scratch size; an invalid shape gets its own code before any size is compared
+  int rc = validate_shape(p->dtype, p->batch, p->L, p->Hq, p->Hkv, p->d, p->P);
+  if (rc) return rc;
+  const size_t need = nacl_workspace_bytes(p->batch, p->L, p->Hq, p->Hkv, p->d, p->P);
+  if (need == 0 || need > (size_t)NACL_STATIC_SCRATCH_BYTES) return NACL_ERR_STATIC_LIMIT;
+  void* scratch = nullptr;
+  if ((rc = static_scratch_here(&scratch)) != NACL_OK) return rc;
+  nacl_params_t q = *p;
+  q.workspace = scratch;
+  q.workspace_bytes = NACL_STATIC_SCRATCH_BYTES;
+  // from here on this is the caller-workspace path of nacl_evict_ex: it clears the hand-over counters that must start at
+  // zero on every call (cudaMemsetAsync on the stream) and overwrites everything else before reading it, so whatever an
+  // earlier call of any shape left in the array does no harm
+  return evict_impl(q);
 }
 
 int nacl_evict_batch(const nacl_params_t* p, int n) {
@@ -693,6 +739,7 @@ const char* nacl_strerror(int code) {
     case NACL_ERR_WORKSPACE: return "workspace too small or not 256-byte aligned";
     case NACL_ERR_CUDA: return "a CUDA call failed (see nacl_last_cuda_error)";
     case NACL_ERR_UNSUPPORTED: return "flag, dtype or struct version not supported by this build";
+    case NACL_ERR_STATIC_LIMIT: return "problem needs more scratch than nacl_evict_static's built-in NACL_STATIC_SCRATCH_BYTES (use nacl_evict_ex with a workspace)";
     default: return "unknown error code";
   }
 }

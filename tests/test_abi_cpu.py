@@ -37,7 +37,7 @@ def test_every_declared_symbol_is_exported(lib):
 def test_version_and_strerror(lib):
     hdr = open(os.path.join(ROOT, "include", "nacl_evict.h")).read()
     assert lib.nacl_version() == int(re.search(r"#define NACL_VERSION (\d+)", hdr).group(1))
-    for code in range(0, -8, -1):
+    for code in range(0, -9, -1):
         assert lib.nacl_strerror(code)
     assert b"unknown" in lib.nacl_strerror(-99)
 
@@ -97,6 +97,36 @@ def test_ex_rejects_wrong_struct_and_unknown_flags(lib):
     p.flags = 0
     p.workspace, p.workspace_bytes = 0x10000, 16
     assert lib.nacl_evict_ex(C.byref(p)) == -5
+
+
+def test_static_scratch_entry_point_validates_on_the_host(lib):
+    """nacl_evict_static (the call for users who cannot allocate device memory) refuses what it cannot serve before it
+    asks the CUDA runtime for anything: these checks need no GPU."""
+    from paper_2408_03675_b200.binding import STATIC_SCRATCH_BYTES, NaclParams
+
+    hdr = open(os.path.join(ROOT, "include", "nacl_evict.h")).read()
+    m = re.search(r"#define NACL_STATIC_SCRATCH_BYTES \((\d+) \* (\d+) \* (\d+)\)", hdr)
+    assert int(m.group(1)) * int(m.group(2)) * int(m.group(3)) == STATIC_SCRATCH_BYTES
+    lib.nacl_evict_static.argtypes = [C.POINTER(NaclParams)]
+    assert lib.nacl_evict_static(None) == -1
+    p = NaclParams()
+    p.struct_size = 8
+    assert lib.nacl_evict_static(C.byref(p)) == -7
+    p.struct_size = C.sizeof(NaclParams)
+    p.dtype = 1
+    p.K, p.V, p.Qproxy, p.out_K, p.out_V, p.out_idx = 0x1000, 0x2000, 0x3000, 0x4000, 0x5000, 0x6000
+    p.batch, p.L, p.Hq, p.Hkv, p.d, p.P = 4, 32768, 16, 16, 128, 16
+    p.budget_proxy, p.budget_random, p.n_sink, p.n_recent = 600, 200, 4, 16
+    assert lib.nacl_workspace_bytes(4, 32768, 16, 16, 128, 16) > STATIC_SCRATCH_BYTES
+    assert lib.nacl_evict_static(C.byref(p)) == -8       # more scratch than the library carries
+    assert b"NACL_STATIC_SCRATCH_BYTES" in lib.nacl_strerror(-8)
+    p.Hq = 15
+    assert lib.nacl_evict_static(C.byref(p)) == -2       # a bad shape keeps its own code
+    p.Hq, p.batch, p.L = 16, 1, 4096
+    p.workspace, p.workspace_bytes = 0x10000, 1 << 24
+    assert lib.nacl_evict_static(C.byref(p)) == -5       # it brings its own scratch: no caller workspace
+    for cfg in CONFIGS.values():                         # every BASELINE.json shape fits
+        assert lib.nacl_workspace_bytes(cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P) <= STATIC_SCRATCH_BYTES
 
 
 def test_paged_kv_validation_without_touching_the_device(lib):

@@ -179,11 +179,13 @@ static int fail_cuda(cudaError_t e) {
 }
 
 // ------------------------------------------------------------------ the call
-static int evict_impl(const nacl_params_t& p) {
+// idx_in_ws: the index list goes to the workspace's idx_tmp (p.out_idx is ignored) and *idx_in_ws receives where that is
+// (nacl_evict_generation without out_idx: this call alone decides which workspace it is and keeps its bookkeeping)
+static int evict_impl(const nacl_params_t& p, int32_t** idx_in_ws = nullptr) {
   if (!p.K || !p.V || !p.Qproxy) return NACL_ERR_NULL;
   // an empty budget (C == 0) has empty outputs: their pointers may be NULL
   const bool empty_out = p.budget_proxy == 0 && p.budget_random == 0;
-  if (!empty_out && (!p.out_K || !p.out_V || !p.out_idx)) return NACL_ERR_NULL;
+  if (!empty_out && (!p.out_K || !p.out_V || (!p.out_idx && !idx_in_ws))) return NACL_ERR_NULL;
   int rc = validate_shape(p.dtype, p.batch, p.L, p.Hq, p.Hkv, p.d, p.P);
   if (rc) return rc;
   rc = validate_budget(p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.n_protect);
@@ -237,7 +239,7 @@ static int evict_impl(const nacl_params_t& p) {
     return NACL_ERR_UNSUPPORTED;
   }
   if (!aligned16(p.K) || !aligned16(p.V) || !aligned16(p.Qproxy) || !aligned16(p.out_K) || !aligned16(p.out_V) ||
-      (reinterpret_cast<uintptr_t>(p.out_idx) & 3u))
+      (!idx_in_ws && (reinterpret_cast<uintptr_t>(p.out_idx) & 3u)))
     return NACL_ERR_ALIGN;
 
   if (p.batch_offset < 0 || p.head_offset < 0) return NACL_ERR_SHAPE;
@@ -281,6 +283,8 @@ static int evict_impl(const nacl_params_t& p) {
   }
   const Workspace ws = carve_workspace(wsp, p.batch, p.L, p.Hq, p.Hkv, p.P);
   const SplitPlan sp = make_split_plan(p.batch, p.L, p.Hkv);
+  int32_t* const out_idx = idx_in_ws ? ws.idx_tmp : p.out_idx;
+  if (idx_in_ws) *idx_in_ws = ws.idx_tmp;
   if (zero_sync && (e = cudaMemsetAsync(ws.sync, 0, sync_bytes, st)) != cudaSuccess) return fail_cuda(e);
 
   if (p.lse_in && (reinterpret_cast<uintptr_t>(p.lse_in) & 3u)) return NACL_ERR_ALIGN;
@@ -298,18 +302,18 @@ static int evict_impl(const nacl_params_t& p) {
     e = launch_select(ws.imp_sh, ws.key, p.batch, 1, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
                       p.flags, ws.idx_sh, nullptr, nullptr, nullptr, nullptr, row_bytes, &gathered, p.batch_offset, p.head_offset, &s,
                       (float)p.Hkv * (float)s.rows / (float)p.L, false, st);
-    if (e == cudaSuccess) e = launch_replicate_idx(ws.idx_sh, p.out_idx, p.batch, p.Hkv, C, st);
+    if (e == cudaSuccess) e = launch_replicate_idx(ws.idx_sh, out_idx, p.batch, p.Hkv, C, st);
   } else {
     if ((e = launch_protect(ws.imp, p.batch * p.Hkv, p.L, p.protect_idx, p.n_protect, st)) != cudaSuccess) return fail_cuda(e);
     e = launch_select(ws.imp, ws.key, p.batch, p.Hkv, p.L, p.budget_proxy, p.budget_random, p.n_sink, p.n_recent, p.seed, p.layer,
-                      p.flags, p.out_idx, p.K, p.V, p.out_K, p.out_V, row_bytes, &gathered, p.batch_offset, p.head_offset, &s,
+                      p.flags, out_idx, p.K, p.V, p.out_K, p.out_V, row_bytes, &gathered, p.batch_offset, p.head_offset, &s,
                       (float)s.rows / (float)p.L, inplace, st);
   }
   if (e == cudaErrorNotSupported && inplace) { cudaGetLastError(); return NACL_ERR_UNSUPPORTED; }  // rows too long for the fused gather
   if (e != cudaSuccess) return fail_cuda(e);
   if (!gathered) {
     StageScope sc(ST_GATHER, st);
-    e = launch_gather(p.K, p.V, p.out_idx, s, C, row_bytes, p.out_K, p.out_V, st);
+    e = launch_gather(p.K, p.V, out_idx, s, C, row_bytes, p.out_K, p.out_V, st);
   }
   if (e != cudaSuccess) return fail_cuda(e);
   return NACL_OK;
@@ -476,27 +480,12 @@ int nacl_evict_generation(const nacl_gen_params_t* g) {
   p.batch_offset = g->batch_offset; p.head_offset = g->head_offset;
   p.kv_stride_row = g->d; p.kv_stride_head = (int64_t)g->cap_in * g->d; p.kv_stride_batch = (int64_t)g->Hkv * g->cap_in * g->d;
   p.out_stride_row = g->d; p.out_stride_head = (int64_t)g->cap_out * g->d; p.out_stride_batch = (int64_t)g->Hkv * g->cap_out * g->d;
+  // without out_idx the kept slots are still needed for the position map: evict_impl then writes them to its workspace
+  // (the caller's or the library's own, chosen and accounted for there as for any other call) and says where
   int32_t* idx = g->out_idx;
-  if (!idx && C > 0) {
-    // the kept slots are needed for the position map even when the caller does not want them: take them from the workspace
-    void* wsp = g->workspace;
-    const size_t need = nacl_workspace_bytes(g->batch, g->len, g->Hq, g->Hkv, g->d, 1);
-    if (wsp) {
-      if (g->workspace_bytes < need || (reinterpret_cast<uintptr_t>(wsp) & 255u)) return NACL_ERR_WORKSPACE;
-    } else {
-      int dev = 0;
-      cudaError_t e = cudaGetDevice(&dev);
-      if (e != cudaSuccess) return fail_cuda(e);
-      if (dev < 0 || dev >= 64) return NACL_ERR_UNSUPPORTED;
-      std::lock_guard<std::mutex> lk(g_mu);
-      if ((e = stream_workspace(g_cache[dev], static_cast<cudaStream_t>(g->stream), need, &wsp)) != cudaSuccess) return fail_cuda(e);
-      p.workspace = wsp;
-      p.workspace_bytes = need;
-    }
-    idx = carve_workspace(wsp, g->batch, g->len, g->Hq, g->Hkv, 1).idx_tmp;
-  }
   p.out_idx = idx;
-  rc = evict_impl(p);
+  if (!idx && C > 0) rc = evict_impl(p, &idx);
+  else rc = evict_impl(p);
   if (rc != NACL_OK || !g->pos_in || C == 0) return rc;
   cudaError_t e = launch_compose_positions(g->pos_in, g->cap_in, idx, g->batch * g->Hkv, (int)C, g->pos_out, g->cap_out,
                                            static_cast<cudaStream_t>(g->stream));

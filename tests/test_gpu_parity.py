@@ -734,3 +734,29 @@ def test_generation_phase_eviction(binding, case):
     assert n_evictions == 12 // m
     # the newest tokens (protected recent slots) survive every eviction
     assert (bufs[cur][2][:, :, C - 1] == 1000 + (12 // m) * m).all()
+
+
+def test_generation_call_between_fused_calls_on_the_library_workspace(binding):
+    """Calls of different head counts that share the library's own per-stream workspace: a 64-head call through the fused
+    scoring launch (whose CTAs hand partials over through counters that must be zero at launch), then a generation-phase
+    call with 8 heads and no out_idx (its softmax partials land on the bytes that held the 64-head call's counters), then
+    the 64-head call again.  The library's record of how much of the counter area is still zero has to survive the call in
+    the middle; the third call must give what the first gave and what the two-launch form (no counters) gives."""
+    K, V, Q = make_random_inputs(2, 1024, 32, 32, 128, 16, dtype="bf16", seed=21, device="cuda")
+    args = (K, V, Q, 150, 50, 4, 16, 4242, 7)
+    first = binding.nacl_evict_ex(*args, want_importance=True)
+    Kc, Vc, q = (t.contiguous() for t in make_random_inputs(1, 4100, 8, 8, 128, 1, dtype="bf16", seed=22, device="cuda"))
+    C = 600
+    Ko, Vo = torch.zeros(1, 8, C, 128, dtype=torch.bfloat16, device="cuda"), torch.zeros(1, 8, C, 128, dtype=torch.bfloat16, device="cuda")
+    pos = torch.arange(4100, dtype=torch.int32, device="cuda").repeat(1, 8, 1).contiguous()
+    po = torch.zeros(1, 8, C, dtype=torch.int32, device="cuda")
+    binding.nacl_evict_generation(Kc, Vc, q, 4100, 450, 150, 2, 4, 77, 5, 3, Ko, Vo, pos_in=pos, pos_out=po)  # no out_idx, no workspace
+    third = binding.nacl_evict_ex(*args, want_importance=True)
+    ref = binding.nacl_evict_ex(*args, want_importance=True, flags=binding.FLAG_SCORE_TWO_LAUNCHES)
+    gen_ref = binding.nacl_evict_generation(Kc, Vc, q, 4100, 450, 150, 2, 4, 77, 5, 3, torch.zeros_like(Ko), torch.zeros_like(Vo), want_idx=True)
+    torch.cuda.synchronize()
+    for k in ("out_idx", "out_K", "out_V"):
+        assert torch.equal(third[k], first[k]) and torch.equal(third[k], ref[k]), k
+    assert torch.equal(third["importance"], first["importance"])
+    assert torch.equal(po, gen_ref["out_idx"])  # identity position map: pos_out names the kept slots
+    assert torch.equal(Ko, torch.gather(Kc, 2, po.long()[..., None].expand(-1, -1, -1, 128)))

@@ -168,6 +168,10 @@ def run_ours(args) -> dict:
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device for --impl ours (there is no CPU fallback)")
+    if int(os.environ.get("WORLD_SIZE", 1)) > 1:
+        # the benchmark (not the library) wants NCCL's communicator line ("... nranks N ...") in its log: the driver reads it
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
     rank, local_rank, world = nacl_dist.init()
     dev = torch.device("cuda", local_rank)
     torch.cuda.set_device(dev)

@@ -25,9 +25,6 @@ def init(backend: str | None = None) -> tuple[int, int, int]:
         kw = {}
         if backend == "nccl":
             kw["device_id"] = torch.device("cuda", local_rank)
-            # keep NCCL's communicator line ("... nranks N ...") in the log: the driver reads it
-            os.environ.setdefault("NCCL_DEBUG", "INFO")
-            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group(backend=backend, rank=rank, world_size=world, **kw)
     return rank, local_rank, world
 

@@ -65,7 +65,7 @@
 extern "C" {
 #endif
 
-#define NACL_VERSION 210 /* major*10000 + minor*100 + patch */
+#define NACL_VERSION 20200 /* major*10000 + minor*100 + patch: ABI 2.2.0 */
 
 #define NACL_DTYPE_F32 0
 #define NACL_DTYPE_BF16 1
@@ -280,7 +280,12 @@ int nacl_evict_generation(const nacl_gen_params_t* g);
  * out_idx[b*Hkv*C_max ...].  seq_len, budget_proxy, budget_random: HOST arrays of `batch` ints (read before the call
  * returns); p->budget_proxy / p->budget_random are ignored.  Every element is evicted exactly as a batch-1 nacl_evict_ex call
  * with batch_offset = p->batch_offset + b would evict it (same Philox streams), one after the other on p->stream.
- * lse_in, out_importance, out_lse and protect_idx must be NULL.  Returns the first error, NACL_OK otherwise. */
+ * lse_in, out_importance, out_lse and protect_idx must be NULL.  Every element's length and budgets are validated (as a
+ * batch-1 call would: P <= seq_len[b], n_sink + n_recent <= seq_len[b], budget_proxy[b] >= n_sink + n_recent, total <=
+ * seq_len[b]) before the first launch, so a validation error writes nothing; an element that keeps nothing
+ * (budget_proxy[b] + budget_random[b] == 0) is skipped.  This is a host loop: batch launch sets one after the other, each
+ * over Hkv heads only (a padded batch of equal lengths is served faster by one nacl_evict_ex call).  Returns the first
+ * error, NACL_OK otherwise. */
 int nacl_evict_varlen(const nacl_params_t* p, const int32_t* seq_len, const int32_t* budget_proxy,
                       const int32_t* budget_random, int C_max);
 
@@ -315,16 +320,12 @@ int nacl_gumbel_keys(const float* importance, float* out_keys, int batch, int Hk
 /* Bytes of scratch one call needs (a pure function of the shape; 0 on invalid shapes). */
 size_t nacl_workspace_bytes(int batch, int L, int Hq, int Hkv, int d, int P);
 
-/* Number of kernels one self-contained call with these arguments launches (for launch accounting; budget_random > 0 and
- * no lse_in assumed: with lse_in the statistics sweep -- one launch on the tensor-core path, two on the generic one --
- * is skipped). */
-int nacl_launch_count(int dtype, int batch, int L, int Hq, int Hkv, int d, int P, uint32_t flags);
-
 /* Per-stage device timing, for benchmarks.  While enabled, every call brackets each of its kernel
  * launches with a pair of CUDA events on the call's stream (so calls are NOT graph-capturable while
  * enabled).  nacl_profile_read waits for the recorded events, adds their elapsed times to per-stage
  * totals and returns the totals accumulated since the last reset: ms[s] = device milliseconds and
- * launches[s] = kernel launches of stage s, s < NACL_N_STAGES (stage names: nacl_stage_name).
+ * launches[s] = kernel launches of stage s, s < NACL_N_STAGES (stage names: nacl_stage_name): the way to
+ * count what a call really launched (the number depends on shape, flags and on the cluster sizes the device can schedule).
  * Either output may be NULL.  Returns 0 or NACL_ERR_CUDA. */
 #define NACL_N_STAGES 7
 int nacl_profile_enable(int on);

@@ -19,9 +19,9 @@ FLAG_CAUSAL, FLAG_SAMPLE_SOFTMAX_OF_SCORE, FLAG_SAMPLE_UNIFORM, FLAG_SHARED_HEAD
 FLAG_SCORE_TWO_LAUNCHES, FLAG_SELECT_GENERAL, FLAG_GATHER_SEPARATE = 0x200, 0x400, 0x800
 
 EXPORTS = ("nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes",
-           "nacl_launch_count", "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version",
+           "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version",
            "nacl_profile_enable", "nacl_profile_read", "nacl_stage_name", "nacl_gumbel_keys", "nacl_evict_generation",
-           "nacl_select_fallbacks", "nacl_evict_varlen", "nacl_evict_host_batch", "nacl_evict_batch")
+           "nacl_select_fallbacks", "nacl_evict_varlen", "nacl_evict_host_batch", "nacl_evict_batch", "nacl_evict_static")
 N_STAGES = 7
 
 
@@ -96,8 +96,6 @@ def _load() -> C.CDLL:
     lib.nacl_evict_host_batch.restype = i32
     lib.nacl_workspace_bytes.argtypes = [i32] * 6
     lib.nacl_workspace_bytes.restype = C.c_size_t
-    lib.nacl_launch_count.argtypes = [i32] * 7 + [u32]
-    lib.nacl_launch_count.restype = i32
     lib.nacl_release.argtypes = []
     lib.nacl_release.restype = None
     lib.nacl_select_fallbacks.argtypes = [i32]
@@ -157,10 +155,6 @@ def nacl_version() -> int:
 
 def nacl_workspace_bytes(batch, L, Hq, Hkv, d, P) -> int:
     return int(_lib.nacl_workspace_bytes(batch, L, Hq, Hkv, d, P))
-
-
-def nacl_launch_count(dtype, batch, L, Hq, Hkv, d, P, flags=0) -> int:
-    return int(_lib.nacl_launch_count(dtype, batch, L, Hq, Hkv, d, P, flags))
 
 
 def nacl_select_fallbacks(reset: bool = True) -> int:

@@ -506,11 +506,16 @@ int nacl_evict_varlen(const nacl_params_t* p, const int32_t* seq_len, const int3
   const int64_t kv_sb = kv0 ? (int64_t)p->Hkv * p->L * p->d : p->kv_stride_batch;
   const int64_t o_sr = o0 ? p->d : p->out_stride_row, o_sh = o0 ? (int64_t)C_max * p->d : p->out_stride_head;
   const int64_t o_sb = o0 ? (int64_t)p->Hkv * C_max * p->d : p->out_stride_batch;
+  // every element is checked before anything is enqueued: no output is written on a validation error
   for (int b = 0; b < p->batch; ++b) {
     if (seq_len[b] < 1 || seq_len[b] > p->L) return NACL_ERR_SHAPE;
     if (budget_proxy[b] < 0 || budget_random[b] < 0 || (long)budget_proxy[b] + budget_random[b] > C_max) return NACL_ERR_BUDGET;
+    int rc = validate_shape(p->dtype, 1, seq_len[b], p->Hq, p->Hkv, p->d, p->P);  // P > seq_len[b] among others
+    if (rc) return rc;
+    if ((rc = validate_budget(seq_len[b], budget_proxy[b], budget_random[b], p->n_sink, p->n_recent)) != NACL_OK) return rc;
   }
   for (int b = 0; b < p->batch; ++b) {
+    if (budget_proxy[b] + budget_random[b] == 0) continue;  // keeps nothing: no output rows, nothing to compute
     nacl_params_t q = *p;
     q.batch = 1;
     q.L = seq_len[b];
@@ -642,16 +647,6 @@ int nacl_gumbel_keys(const float* importance, float* out_keys, int batch, int Hk
 size_t nacl_workspace_bytes(int batch, int L, int Hq, int Hkv, int d, int P) {
   if (validate_shape(NACL_DTYPE_BF16, batch, L, Hq, Hkv, d, P) != NACL_OK) return 0;
   return carve_workspace(nullptr, batch, L, Hq, Hkv, P).bytes;
-}
-
-int nacl_launch_count(int dtype, int batch, int L, int Hq, int Hkv, int d, int P, uint32_t flags) {
-  if (validate_shape(dtype, batch, L, Hq, Hkv, d, P) != NACL_OK) return 0;
-  Shape s;
-  s.batch = batch; s.L = L; s.Hq = Hq; s.Hkv = Hkv; s.d = d; s.P = P;
-  s.G = Hq / Hkv; s.rows = s.G * P; s.dtype = dtype; s.esize = dtype == NACL_DTYPE_F32 ? 4 : 2;
-  const bool tc = !(flags & NACL_FLAG_SCORE_CUDA_CORES) && score_tc_supported(s);
-  // scoring + select (+ a separate keys kernel for very long rows) + gather (budget_random > 0 and C > 0 assumed)
-  return (tc ? score_tc_launch_count(s, (flags & NACL_FLAG_SCORE_TWO_LAUNCHES) != 0) : 3) + (select_uses_cluster(L) ? 1 : 3);  // the cluster select also gathers
 }
 
 int nacl_profile_enable(int on) {

@@ -74,7 +74,6 @@ cudaError_t launch_score_generic(const Shape& s, const void* K, const void* Q, c
 
 // tensor-core scoring (bf16, d == 128, G*P % 16 == 0, G*P <= 256): tcgen05 + TMA
 bool score_tc_supported(const Shape& s);
-int score_tc_launch_count(const Shape& s, bool two_launches);
 size_t score_tc_part_elems(int heads, int rows);  // float2 elements of Workspace::part the tensor-core path needs
 cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const SplitPlan& sp,
                             const Workspace& ws, const float* lse_in, bool causal, bool two_launches, float* imp_out,

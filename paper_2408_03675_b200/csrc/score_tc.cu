@@ -1250,7 +1250,6 @@ bool score_tc_supported(const Shape& s) {
          s.rows <= 8192;  // G*P > 256: blocks of 256 proxy rows, the last one masked where G*P is off that grid
 }
 
-int score_tc_launch_count(const Shape&, bool two_launches) { return two_launches ? 2 : 1; }
 
 size_t score_tc_part_elems(int heads, int rows) { return (size_t)(MAX_GRID + heads) * 4 * rows; }
 

@@ -213,6 +213,12 @@ def test_varlen_validation_without_touching_the_device(lib):
     assert lib.nacl_evict_varlen(C.byref(p), i32x2(512, 513), bp, br, 102) == -2  # longer than the padded length
     assert lib.nacl_evict_varlen(C.byref(p), i32x2(512, 0), bp, br, 102) == -2
     assert lib.nacl_evict_varlen(C.byref(p), lens, bp, br, 101) == -3             # an element's budget exceeds C_max
+    # a LATER element that a batch-1 call would refuse is found before the first element is launched (here, without a
+    # GPU, a launch would come back as -6): nothing is written on a validation error
+    assert lib.nacl_evict_varlen(C.byref(p), i32x2(512, 15), bp, br, 102) == -2    # P = 16 proxy rows > 15 keys
+    assert lib.nacl_evict_varlen(C.byref(p), i32x2(512, 18), i32x2(76, 18), i32x2(26, 0), 102) == -3   # protected 20 > 18 keys
+    assert lib.nacl_evict_varlen(C.byref(p), lens, i32x2(76, 19), br, 102) == -3   # budget_proxy below the protected count
+    assert lib.nacl_evict_varlen(C.byref(p), i32x2(512, 40), i32x2(76, 30), i32x2(26, 11), 102) == -3  # keeps more than it has
     p.lse_in = 0x7000
     assert lib.nacl_evict_varlen(C.byref(p), lens, bp, br, 102) == -7             # not offered for variable-length batches
     p.lse_in = None

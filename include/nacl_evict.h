@@ -35,10 +35,14 @@
  * pointers must be 16-byte aligned and d*sizeof(element) a multiple of 16.  Work is enqueued
  * on `stream` (a cudaStream_t passed as void*); the call never synchronises the host and
  * results are valid once the stream reaches that point.  With a caller-supplied workspace
- * (nacl_evict_ex) the call allocates nothing and is CUDA-graph capturable; without one a
- * grow-only internal workspace per (device, stream) is created on first use (cudaMalloc: not capturable); calls on
+ * (nacl_evict_ex) the call allocates nothing and is CUDA-graph capturable; without one an
+ * internal workspace per (device, stream) is created on first use (cudaMalloc: not capturable); calls on
  * one stream share it in stream order, calls on different streams never do, so concurrent host threads are safe as
- * long as they use different streams (or pass their own workspaces).
+ * long as they use different streams (or pass their own workspaces).  Growth of the internal workspaces: a stream's
+ * buffer is replaced by a larger one (about 9/8 of the need) when a larger shape arrives, and the old buffer is freed by
+ * a later call once the work that used it has finished; the 16 most recently used streams per device keep a buffer,
+ * older ones give theirs up the same way (so streams that come and go do not pile up).  Buffers that were used while
+ * their stream was being captured stay until nacl_release, since a graph may still refer to them.
  * Same inputs and seed give bit-identical outputs run to run (no floating-point atomics).
  * nacl_evict_host is the same operation on HOST buffers (copies inside; synchronous).
  *

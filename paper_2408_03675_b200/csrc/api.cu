@@ -111,14 +111,29 @@ static int validate_budget(int L, int budget_proxy, int budget_random, int n_sin
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-// ------------------------------------------------------------------ internal grow-only buffers
+// ------------------------------------------------------------------ internal buffers
 // The internal workspace is keyed by (device, stream): calls on one stream are ordered and may share scratch, calls on
-// different streams may run at the same time and must not.  A buffer that is too small is replaced, but the old one
-// is only freed by nacl_release: a call enqueued earlier on the same stream may still be running out of it.
-struct WsEntry { cudaStream_t stream; void* ptr; size_t bytes; size_t sync_clean; };  // sync_clean: leading bytes known to be zero
+// different streams may run at the same time and must not.  A buffer that is too small is replaced; the old one may
+// still be in use by calls enqueued earlier, so it is RETIRED with the event that the last call using it recorded behind
+// its last kernel, and freed by a later call once that event has completed.  At most kMaxStreamWorkspaces streams keep
+// a workspace per device: beyond that the least recently used one is retired the same way (an application that creates
+// and destroys streams does not accumulate them).  A workspace that was ever used while its stream was being captured
+// may be referenced by a graph that is replayed at any later time: it is never freed before nacl_release.
+constexpr size_t kMaxStreamWorkspaces = 16;
+struct WsEntry {
+  cudaStream_t stream;
+  void* ptr;
+  size_t bytes;
+  size_t sync_clean;   // leading bytes known to be zero
+  cudaEvent_t done;    // recorded behind the last kernel of the latest call that used ptr
+  uint64_t last_use;   // DeviceCache::tick of that call
+  bool captured;       // used under stream capture at least once
+};
+struct RetiredWs { void* ptr; cudaEvent_t done; };  // done == nullptr: keep until nacl_release
 struct DeviceCache {
   std::vector<WsEntry> ws;
-  std::vector<void*> retired;
+  std::vector<RetiredWs> retired;
+  uint64_t tick = 0;
   void* stage[2][6] = {};         // nacl_evict_host(_batch): two staging slots of K V Q oK oV idx ...
   size_t stage_bytes[2][6] = {};
   cudaStream_t stream[2] = {nullptr, nullptr};  // ... with a stream each
@@ -144,32 +159,91 @@ static cudaError_t grow(void** p, size_t* have, size_t want) {
   return cudaSuccess;
 }
 
+// g_mu held.  Frees the retired buffers whose last user has finished.
+static void sweep_retired(DeviceCache& dc) {
+  for (size_t i = 0; i < dc.retired.size();) {
+    RetiredWs& r = dc.retired[i];
+    cudaError_t q = r.done ? cudaEventQuery(r.done) : cudaErrorNotReady;
+    if (q == cudaSuccess) {
+      cudaFree(r.ptr);
+      cudaEventDestroy(r.done);
+      dc.retired[i] = dc.retired.back();
+      dc.retired.pop_back();
+    } else {
+      if (q != cudaErrorNotReady) cudaGetLastError();  // an event that cannot be queried: the buffer stays until nacl_release
+      ++i;
+    }
+  }
+}
+
+// g_mu held.  The buffer of `w` leaves service: freed once w.done has completed (never, if a graph may hold it).
+static void retire(DeviceCache& dc, WsEntry& w) {
+  if (w.captured) {
+    dc.retired.push_back(RetiredWs{w.ptr, nullptr});
+    if (w.done) cudaEventDestroy(w.done);
+  } else {
+    dc.retired.push_back(RetiredWs{w.ptr, w.done});
+  }
+  w.ptr = nullptr;
+  w.done = nullptr;
+}
+
 // g_mu held
 static cudaError_t stream_workspace(DeviceCache& dc, cudaStream_t st, size_t want, void** out, size_t** sync_clean = nullptr) {
+  sweep_retired(dc);
+  const size_t cap = want + want / 8 + 256;
   for (WsEntry& w : dc.ws)
     if (w.stream == st) {
       if (sync_clean) *sync_clean = &w.sync_clean;
+      w.last_use = ++dc.tick;
       if (w.bytes < want) {
-        dc.retired.push_back(w.ptr);
-        const size_t cap = want + want / 8 + 256;
         void* np = nullptr;
+        cudaEvent_t ne = nullptr;
         cudaError_t e = cudaMalloc(&np, cap);
-        if (e != cudaSuccess) { dc.retired.pop_back(); return e; }
+        if (e != cudaSuccess) return e;
+        if ((e = cudaEventCreateWithFlags(&ne, cudaEventDisableTiming)) != cudaSuccess) { cudaFree(np); return e; }
+        retire(dc, w);
         w.ptr = np;
+        w.done = ne;
         w.bytes = cap;
         w.sync_clean = 0;
+        w.captured = false;
       }
       *out = w.ptr;
       return cudaSuccess;
     }
-  const size_t cap = want + want / 8 + 256;
   void* np = nullptr;
+  cudaEvent_t ne = nullptr;
   cudaError_t e = cudaMalloc(&np, cap);
   if (e != cudaSuccess) return e;
-  dc.ws.push_back(WsEntry{st, np, cap, 0});
+  if ((e = cudaEventCreateWithFlags(&ne, cudaEventDisableTiming)) != cudaSuccess) { cudaFree(np); return e; }
+  if (dc.ws.size() >= kMaxStreamWorkspaces) {
+    // the stream that has gone unused the longest gives up its workspace (it gets a new one if it ever comes back)
+    size_t lru = 0;
+    for (size_t i = 1; i < dc.ws.size(); ++i)
+      if (dc.ws[i].last_use < dc.ws[lru].last_use) lru = i;
+    retire(dc, dc.ws[lru]);
+    dc.ws[lru] = dc.ws.back();
+    dc.ws.pop_back();
+  }
+  dc.ws.push_back(WsEntry{st, np, cap, 0, ne, ++dc.tick, false});
   if (sync_clean) *sync_clean = &dc.ws.back().sync_clean;
   *out = np;
   return cudaSuccess;
+}
+
+// Behind the last kernel of a call that worked in the library's workspace of (dev, st): marks the point after which that
+// buffer is free to go.  Under stream capture nothing is recorded: the buffer is pinned instead (a graph may replay it).
+static void workspace_call_done(int dev, cudaStream_t st) {
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { cudaGetLastError(); cs = cudaStreamCaptureStatusActive; }
+  std::lock_guard<std::mutex> lk(g_mu);
+  for (WsEntry& w : g_cache[dev].ws)
+    if (w.stream == st) {
+      if (cs != cudaStreamCaptureStatusNone) w.captured = true;
+      else if (w.done && cudaEventRecord(w.done, st) != cudaSuccess) { cudaGetLastError(); w.captured = true; }
+      return;
+    }
 }
 
 static int fail_cuda(cudaError_t e) {
@@ -181,7 +255,17 @@ static int fail_cuda(cudaError_t e) {
 // ------------------------------------------------------------------ the call
 // idx_in_ws: the index list goes to the workspace's idx_tmp (p.out_idx is ignored) and *idx_in_ws receives where that is
 // (nacl_evict_generation without out_idx: this call alone decides which workspace it is and keeps its bookkeeping)
+static int evict_core(const nacl_params_t& p, int32_t** idx_in_ws, int* internal_ws_dev);
+
 static int evict_impl(const nacl_params_t& p, int32_t** idx_in_ws = nullptr) {
+  int dev = -1;  // >= 0 once the call works in the library's own workspace of that device
+  const int rc = evict_core(p, idx_in_ws, &dev);
+  // whatever was enqueued (also before an error) is the buffer's latest use
+  if (dev >= 0) workspace_call_done(dev, static_cast<cudaStream_t>(p.stream));
+  return rc;
+}
+
+static int evict_core(const nacl_params_t& p, int32_t** idx_in_ws, int* internal_ws_dev) {
   if (!p.K || !p.V || !p.Qproxy) return NACL_ERR_NULL;
   // an empty budget (C == 0) has empty outputs: their pointers may be NULL
   const bool empty_out = p.budget_proxy == 0 && p.budget_random == 0;
@@ -272,6 +356,7 @@ static int evict_impl(const nacl_params_t& p, int32_t** idx_in_ws = nullptr) {
     size_t* clean = nullptr;
     e = stream_workspace(g_cache[dev], st, need, &wsp, &clean);
     if (e != cudaSuccess) return fail_cuda(e);
+    *internal_ws_dev = dev;
     // the counters' bytes are reserved for them in every carve-up; what lies behind them is written by this call's other buffers
     const size_t reserved = sync_ints((size_t)p.batch * p.Hkv) * sizeof(int);
     if (sync_bytes > 0) {
@@ -489,6 +574,12 @@ int nacl_evict_generation(const nacl_gen_params_t* g) {
   if (rc != NACL_OK || !g->pos_in || C == 0) return rc;
   cudaError_t e = launch_compose_positions(g->pos_in, g->cap_in, idx, g->batch * g->Hkv, (int)C, g->pos_out, g->cap_out,
                                            static_cast<cudaStream_t>(g->stream));
+  if (!g->out_idx && !g->workspace) {
+    // this kernel read the kept slots out of the library's workspace: it is that buffer's latest use now
+    int dev = -1;
+    if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64) workspace_call_done(dev, static_cast<cudaStream_t>(g->stream));
+    else cudaGetLastError();
+  }
   return e == cudaSuccess ? NACL_OK : fail_cuda(e);
 }
 
@@ -700,8 +791,8 @@ void nacl_release(void) {
     if (!any) continue;
     if (cudaSetDevice(dev) != cudaSuccess) { cudaGetLastError(); continue; }
     cudaDeviceSynchronize();  // retired workspaces may still be in use by enqueued calls
-    for (WsEntry& w : dc.ws) cudaFree(w.ptr);
-    for (void* q : dc.retired) cudaFree(q);
+    for (WsEntry& w : dc.ws) { cudaFree(w.ptr); if (w.done) cudaEventDestroy(w.done); }
+    for (RetiredWs& r : dc.retired) { cudaFree(r.ptr); if (r.done) cudaEventDestroy(r.done); }
     for (int i = 0; i < 12; ++i) if (dc.stage[i / 6][i % 6]) cudaFree(dc.stage[i / 6][i % 6]);
     for (int sl = 0; sl < 2; ++sl) if (dc.stream[sl]) cudaStreamDestroy(dc.stream[sl]);
     for (int sl = 0; sl < 2; ++sl) if (dc.bstream[sl]) cudaStreamDestroy(dc.bstream[sl]);

@@ -760,3 +760,53 @@ def test_generation_call_between_fused_calls_on_the_library_workspace(binding):
     assert torch.equal(third["importance"], first["importance"])
     assert torch.equal(po, gen_ref["out_idx"])  # identity position map: pos_out names the kept slots
     assert torch.equal(Ko, torch.gather(Kc, 2, po.long()[..., None].expand(-1, -1, -1, 128)))
+
+
+def test_library_workspaces_do_not_pile_up(binding):
+    """The library's own workspaces (calls without a workspace argument) are keyed by stream.  Streams that come and go
+    must not each leave a buffer behind for good, and a stream whose shapes keep growing must not keep every buffer it
+    outgrew: old buffers are freed once the work that used them is done.  Read off the driver's free-memory
+    figure, with every tensor of the test allocated before the first reading."""
+    MiB = 1 << 20
+    binding.nacl_release()
+    torch.cuda.synchronize()
+    B, Hq, Hkv, d, P = 1, 8, 8, 128, 16
+    Ls = [8192 + 4096 * k for k in range(7)]  # 8k .. 32k keys: every step outgrows the 9/8 head-room of the buffer before it
+    data = {L: make_random_inputs(B, L, Hq, Hkv, d, P, dtype="bf16", seed=L, device="cuda") for L in Ls}
+    oK = torch.empty((B, Hkv, 800, d), dtype=torch.bfloat16, device="cuda")
+    outs = dict(out_K=oK, out_V=torch.empty_like(oK), out_idx=torch.empty((B, Hkv, 800), dtype=torch.int32, device="cuda"))
+    streams = [torch.cuda.Stream() for _ in range(40)]
+    ws_big = binding.nacl_workspace_bytes(B, Ls[-1], Hq, Hkv, d, P)
+    assert 3 * MiB < ws_big < 5 * MiB
+    K, V, Q = data[Ls[-1]]
+    binding.nacl_evict_ex(K, V, Q, 600, 200, 4, P, 1, 0, **outs)  # loads the kernels; creates the current stream's workspace
+    want = {k: v.clone() for k, v in outs.items()}
+    torch.cuda.synchronize()
+    free0, _ = torch.cuda.mem_get_info()
+    # 40 streams, one call each at the largest shape: at most 16 keep a buffer
+    for st in streams:
+        st.wait_stream(torch.cuda.current_stream())
+        binding.nacl_evict_ex(K, V, Q, 600, 200, 4, P, 1, 0, stream=st, **outs)
+        st.synchronize()
+        for k in outs:
+            assert torch.equal(outs[k], want[k])
+    free1, _ = torch.cuda.mem_get_info()
+    used = free0 - free1
+    assert 0 <= used <= 18 * 6 * MiB, f"{used / MiB:.0f} MiB held after 40 streams (40 buffers would be >= {40 * ws_big / MiB:.0f})"
+    # one stream, seven growing shapes: the outgrown buffers go away
+    binding.nacl_release()
+    torch.cuda.synchronize()
+    free2, _ = torch.cuda.mem_get_info()
+    st = streams[0]
+    total = 0
+    for L in Ls:
+        Kl, Vl, Ql = data[L]
+        total += binding.nacl_workspace_bytes(B, L, Hq, Hkv, d, P)
+        binding.nacl_evict_ex(Kl, Vl, Ql, 600, 200, 4, P, 1, 0, stream=st, **outs)
+        st.synchronize()
+    free3, _ = torch.cuda.mem_get_info()
+    used = free2 - free3
+    assert total > 4 * ws_big
+    assert 0 <= used <= 10 * MiB, f"{used / MiB:.0f} MiB held after growing to {ws_big / MiB:.1f} MiB (never freeing would hold ~{total / MiB:.0f})"
+    for k in outs:
+        assert torch.equal(outs[k], want[k])

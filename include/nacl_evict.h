@@ -341,6 +341,12 @@ const char* nacl_stage_name(int stage);
  * would overflow; the result is the same either way).  Synchronises the device.  Returns the count or NACL_ERR_CUDA. */
 int nacl_select_fallbacks(int reset);
 
+/* Diagnostics: the launch configuration of the selection kernel that the latest eviction call ISSUED FROM THIS HOST THREAD
+ * chose: CTAs in its grid, CTAs per cluster (0 = the path without clusters, one CTA per head) and whether that kernel also
+ * moved the kept K/V rows (1) or a stand-alone gather followed (0).  Lets a test or a benchmark assert which launch
+ * configuration it really ran (e.g. nacl_evict_batch keeps the grid below ~45 % of the SMs).  Outputs may be NULL. */
+void nacl_last_select_launch(int* grid_ctas, int* cluster_size, int* fused_gather);
+
 /* Frees the per-device internal workspaces / staging buffers (optional, e.g. before exit). */
 void nacl_release(void);
 

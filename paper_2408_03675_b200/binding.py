@@ -98,6 +98,8 @@ def _load() -> C.CDLL:
     lib.nacl_workspace_bytes.restype = C.c_size_t
     lib.nacl_release.argtypes = []
     lib.nacl_release.restype = None
+    lib.nacl_last_select_launch.argtypes = [C.POINTER(i32)] * 3
+    lib.nacl_last_select_launch.restype = None
     lib.nacl_select_fallbacks.argtypes = [i32]
     lib.nacl_select_fallbacks.restype = i32
     lib.nacl_evict_varlen.argtypes = [C.POINTER(NaclParams), C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32), i32]
@@ -162,6 +164,13 @@ def nacl_select_fallbacks(reset: bool = True) -> int:
     if rc < 0:
         raise NaclError(rc, "nacl_select_fallbacks")
     return rc
+
+
+def nacl_last_select_launch() -> dict:
+    """Launch configuration of the selection kernel of the latest call issued from this thread (diagnostics)."""
+    g, c, f = C.c_int32(0), C.c_int32(0), C.c_int32(0)
+    _lib.nacl_last_select_launch(C.byref(g), C.byref(c), C.byref(f))
+    return {"grid_ctas": g.value, "cluster_size": c.value, "fused_gather": bool(f.value)}
 
 
 def nacl_release() -> None:

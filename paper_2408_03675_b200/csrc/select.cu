@@ -1092,6 +1092,9 @@ cudaError_t launch_keys(const float* imp, uint32_t* key, int batch, int Hkv, int
 // slices of at most this many positions per CTA stay in shared memory (2 x 4 bytes each)
 constexpr int kMaxSlice = 20480;
 
+// what the latest launch_select on this host thread decided (nacl_last_select_launch)
+static thread_local int g_last_sel_grid = 0, g_last_sel_cluster = 0, g_last_sel_fused = 0;
+
 bool select_uses_cluster(int L) { return (L + kMaxRanks - 1) / kMaxRanks <= kMaxSlice; }
 
 cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, int L, int budget_proxy, int budget_random,
@@ -1106,6 +1109,7 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
   // very long rows, or no cluster size that this device can co-schedule: sampling keys in a kernel of their own, one CTA
   // per head working out of global memory (the caller then runs the stand-alone gather)
   auto long_row_path = [&]() -> cudaError_t {
+    g_last_sel_grid = batch * Hkv; g_last_sel_cluster = 0; g_last_sel_fused = 0;
     if (budget_random > 0) {
       StageScope sc(ST_KEYS, st);
       cudaError_t e = launch_keys(imp, key, batch, Hkv, L, seed, layer, flags, true, batch_offset, head_offset, st);
@@ -1218,6 +1222,7 @@ cudaError_t launch_select(const float* imp, uint32_t* key, int batch, int Hkv, i
 #else
   *gathered = K != nullptr && (inplace || (!(flags & NACL_FLAG_GATHER_SEPARATE) && (heads * n * 5 >= (long)kNumSMs * 4 || small_grid_fused)));
 #endif
+  g_last_sel_grid = (int)(heads * n); g_last_sel_cluster = n; g_last_sel_fused = *gathered ? 1 : 0;
   {
     StageScope sc(ST_SELECT, st);
     e = cudaLaunchKernelEx(&cfg, nacl_select_cluster_kernel, imp, Hkv, L, Lc, k1, budget_random, n_sink, n_recent, C, sk0, sk1,
@@ -1240,6 +1245,12 @@ size_t select_scratch_words(int batch, int Hkv, int L) {
 }
 
 }  // namespace nacl
+
+extern "C" __attribute__((visibility("default"))) void nacl_last_select_launch(int* grid_ctas, int* cluster_size, int* fused_gather) {
+  if (grid_ctas) *grid_ctas = nacl::g_last_sel_grid;
+  if (cluster_size) *cluster_size = nacl::g_last_sel_cluster;
+  if (fused_gather) *fused_gather = nacl::g_last_sel_fused;
+}
 
 extern "C" __attribute__((visibility("default"))) int nacl_select_fallbacks(int reset) {
   int v = 0;

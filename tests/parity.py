@@ -112,27 +112,14 @@ def check_gather(K, V, out_K, out_V, idx_gpu):
             np.testing.assert_array_equal(oV[b, h], Vb[b, h, idx_gpu[b, h]])
 
 
-def full_parity(K, V, Q, Bp, Br, n_sink, n_recent, seed, layer, flags=0, oracle_flags=None, imp_ref=None, lse_in=None,
-                **sel_opts):
-    """Runs the CUDA path through the C ABI on cuda:0 and every check above.  K,V,Q are HOST tensors.
-    sel_opts: batch_offset / head_offset / protect_idx (a list), passed to both sides."""
-    from paper_2408_03675_b200 import binding
-
-    dev = torch.device("cuda:0")
-    Kd, Vd, Qd = K.to(dev), V.to(dev), Q.to(dev)
-    gpu_opts = dict(sel_opts)
-    if gpu_opts.get("protect_idx") is not None:
-        gpu_opts["protect_idx"] = torch.tensor(list(gpu_opts["protect_idx"]), dtype=torch.int32, device=dev)
-    if lse_in is not None:
-        gpu_opts["lse_in"] = lse_in.to(dev)
-    res = binding.nacl_evict_ex(Kd, Vd, Qd, Bp, Br, n_sink, n_recent, seed, layer, flags=flags, want_importance=True, **gpu_opts)
-    torch.cuda.synchronize()
+def check_result(K, V, Q, res, Bp, Br, n_sink, n_recent, seed, layer, oflags=0, imp_ref=None, **sel_opts):
+    """Every check above on ONE call's outputs (`res`: out_idx, importance, out_K, out_V as the binding returns them),
+    whatever entry point produced them.  K, V, Q are the HOST tensors of the call."""
     idx_gpu = res["out_idx"].cpu().numpy()
     imp_gpu = res["importance"].cpu().numpy()
     B, Hkv, L, d = K.shape
     Hq, P = Q.shape[1], Q.shape[2]
     G = Hq // Hkv
-    oflags = (flags & 0x7) if oracle_flags is None else oracle_flags
     if imp_ref is None:
         imp_ref = oracle.importance(K, Q, flags=oflags & oracle.CAUSAL)
     max_rel = check_scores(imp_gpu, imp_ref, G, P)
@@ -140,10 +127,40 @@ def full_parity(K, V, Q, Bp, Br, n_sink, n_recent, seed, layer, flags=0, oracle_
     part_gpu = check_staged(idx_gpu, imp_gpu, Bp, Br, n_sink, n_recent, seed, layer, oflags, **sel_opts)
     swaps, rdiff = check_e2e_sets(idx_gpu, part_gpu, imp_ref, Bp, Br, n_sink, n_recent, seed, layer, oflags, **sel_opts)
     check_gather(K, V, res["out_K"].cpu(), res["out_V"].cpu(), idx_gpu)
-    # determinism: a second run is bit-identical
-    res2 = binding.nacl_evict_ex(Kd, Vd, Qd, Bp, Br, n_sink, n_recent, seed, layer, flags=flags, want_importance=True, **gpu_opts)
+    return {"max_rel_err": max_rel, "topk_swaps": swaps, "random_diffs": rdiff, "imp_gpu": imp_gpu, "idx_gpu": idx_gpu,
+            "imp_ref": imp_ref}
+
+
+def same_outputs(a, b):
+    """Two result dicts of the binding hold the same bits."""
+    for k in ("out_idx", "importance"):
+        if k in a and k in b:
+            assert torch.equal(a[k], b[k]), k
+    for k in ("out_K", "out_V"):
+        assert torch.equal(a[k].view(torch.uint8), b[k].view(torch.uint8)), k
+
+
+def full_parity(K, V, Q, Bp, Br, n_sink, n_recent, seed, layer, flags=0, oracle_flags=None, imp_ref=None, lse_in=None,
+                entry=None, **sel_opts):
+    """Runs the CUDA path through the C ABI on cuda:0 and every check above.  K,V,Q are HOST tensors.
+    sel_opts: batch_offset / head_offset / protect_idx (a list), passed to both sides.
+    entry: the binding function that makes the call (same arguments as binding.nacl_evict_ex, which is the default)."""
+    from paper_2408_03675_b200 import binding
+
+    entry = entry or binding.nacl_evict_ex
+    dev = torch.device("cuda:0")
+    Kd, Vd, Qd = K.to(dev), V.to(dev), Q.to(dev)
+    gpu_opts = dict(sel_opts)
+    if gpu_opts.get("protect_idx") is not None:
+        gpu_opts["protect_idx"] = torch.tensor(list(gpu_opts["protect_idx"]), dtype=torch.int32, device=dev)
+    if lse_in is not None:
+        gpu_opts["lse_in"] = lse_in.to(dev)
+    res = entry(Kd, Vd, Qd, Bp, Br, n_sink, n_recent, seed, layer, flags=flags, want_importance=True, **gpu_opts)
     torch.cuda.synchronize()
-    assert torch.equal(res2["out_idx"], res["out_idx"]) and torch.equal(res2["importance"], res["importance"])
-    assert torch.equal(res2["out_K"].view(torch.uint8), res["out_K"].view(torch.uint8))
-    assert torch.equal(res2["out_V"].view(torch.uint8), res["out_V"].view(torch.uint8))
-    return {"max_rel_err": max_rel, "topk_swaps": swaps, "random_diffs": rdiff, "imp_gpu": imp_gpu, "idx_gpu": idx_gpu}
+    oflags = (flags & 0x7) if oracle_flags is None else oracle_flags
+    out = check_result(K, V, Q, res, Bp, Br, n_sink, n_recent, seed, layer, oflags, imp_ref, **sel_opts)
+    # determinism: a second run is bit-identical
+    res2 = entry(Kd, Vd, Qd, Bp, Br, n_sink, n_recent, seed, layer, flags=flags, want_importance=True, **gpu_opts)
+    torch.cuda.synchronize()
+    same_outputs(res2, res)
+    return out

@@ -36,8 +36,9 @@ def test_baseline_configs_small(binding, cid):
 @pytest.mark.parametrize("cid,layer", [(c, l) for c in (3, 4, 5) for l in (0, 10, 21, 31)])
 def test_baseline_configs_full_size(binding, cid, layer):
     """Four whole layers (first, last, two others: SURVEY.md 8(d)) of each 32-layer workload at BASELINE.json's full
-    sizes, in the launch configuration bench.py times (same entry point, same shapes); the oracle finishes a layer in
-    seconds, so every output is compared, not a sample."""
+    sizes through the single-call form (nacl_evict_ex: fused scoring launch, selection over the whole GPU); the launch
+    configuration bench.py times is test_timed_configuration_full_size below.  The oracle finishes a layer in seconds,
+    so every output is compared, not a sample."""
     cfg = CONFIGS[cid]
     K, V, Q, planted = make_layer_inputs(cfg, layer=layer)
     Bp, Br = cfg.budgets()
@@ -810,3 +811,76 @@ def test_library_workspaces_do_not_pile_up(binding):
     assert 0 <= used <= 10 * MiB, f"{used / MiB:.0f} MiB held after growing to {ws_big / MiB:.1f} MiB (never freeing would hold ~{total / MiB:.0f})"
     for k in outs:
         assert torch.equal(outs[k], want[k])
+
+
+@pytest.mark.parametrize("cid", [3, 4, 5])
+def test_timed_configuration_full_size(binding, cid):
+    """The launch configuration bench.py times, at BASELINE.json's full sizes: FOUR distinct layers in ONE nacl_evict_batch
+    call (the calls alternate between two internal streams; two plain scoring launches per call; the selection grid kept
+    below ~45 % of the SMs; the stand-alone gather or the small-grid fused one), caller workspaces alternating as in
+    bench.py, once eagerly and once replayed from a CUDA graph.  Every layer's outputs go through the whole protocol of
+    tests/parity.py against the oracle; the graph replay must equal the eager call bit for bit, and a single nacl_evict_ex
+    call per layer (the other launch configuration) must give the same bits too."""
+    from parity import check_result, same_outputs
+
+    cfg = CONFIGS[cid]
+    Bp, Br = cfg.budgets()
+    layers = (0, 10, 21, 31)
+    host = [make_layer_inputs(cfg, layer=l) for l in layers]
+    dev = torch.device("cuda:0")
+    data = [(K.to(dev), V.to(dev), Q.to(dev)) for K, V, Q, _ in host]
+    nws = binding.nacl_workspace_bytes(cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P)
+    wss = [torch.full((nws,), 0x5A, dtype=torch.uint8, device=dev) for _ in range(2)]
+    stream = torch.cuda.current_stream(dev)
+
+    def calls(outs=None):
+        cs = []
+        for i, (l, (K, V, Q)) in enumerate(zip(layers, data)):
+            c = dict(K=K, V=V, Qproxy=Q, budget_proxy=Bp, budget_random=Br, n_sink=cfg.n_sink, n_recent=cfg.n_recent,
+                     seed=cfg.layer_seed(l), layer=l, workspace=wss[i & 1], want_importance=True)
+            if outs is not None:  # the graph writes where the captured call wrote: hand the same tensors in again
+                c.update(out_K=outs[i]["out_K"], out_V=outs[i]["out_V"], out_idx=outs[i]["out_idx"])
+            cs.append(c)
+        return cs
+
+    eager = binding.nacl_evict_batch(calls())
+    torch.cuda.synchronize()
+    # this really is the timed configuration: the selection kernel's grid leaves more than half of the SMs to the other stream
+    sel = binding.nacl_last_select_launch()
+    assert 0 < sel["grid_ctas"] <= 0.45 * 148, sel
+    assert sel["fused_gather"] == (cfg.G * cfg.P <= 128), sel
+    single = [binding.nacl_evict_ex(K, V, Q, Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l, want_importance=True)
+              for l, (K, V, Q) in zip(layers, data)]
+    torch.cuda.synchronize()
+    single_grid = binding.nacl_last_select_launch()["grid_ctas"]
+    assert single_grid >= sel["grid_ctas"]
+    if cid in (3, 4):  # ... which the single call does not do with 32 heads (8 heads x 131072 keys: 64 CTAs either way)
+        assert single_grid > 0.45 * 148
+    for i, l in enumerate(layers):
+        K, V, Q, planted = host[i]
+        r = check_result(K, V, Q, eager[i], Bp, Br, cfg.n_sink, cfg.n_recent, cfg.layer_seed(l), l)
+        for b in range(cfg.batch):
+            for hk in range(cfg.Hkv):
+                assert set(planted[b, hk].tolist()) <= set(r["idx_gpu"][b, hk].tolist())
+        same_outputs(eager[i], single[i])
+        print(f"cfg{cid} layer {l} (batch form): max rel err {r['max_rel_err']:.2e}, top-k swaps {r['topk_swaps']}, random diffs {r['random_diffs']}")
+    # the same batch call replayed from a CUDA graph, into fresh (poisoned) outputs
+    outs = [{k: torch.full_like(v, -1) if v.dtype == torch.int32 else torch.zeros_like(v) for k, v in e.items() if k != "importance"}
+            for e in eager]
+    cap = torch.cuda.Stream(dev)
+    cap.wait_stream(stream)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(cap):
+        with torch.cuda.graph(graph, stream=cap):
+            captured = binding.nacl_evict_batch([dict(c, stream=cap) for c in calls(outs)])
+    stream.wait_stream(cap)
+    torch.cuda.synchronize()
+    for o in outs:
+        o["out_idx"].fill_(-1); o["out_K"].zero_(); o["out_V"].zero_()
+    for c in captured:
+        c["importance"].zero_()
+    for _ in range(2):
+        graph.replay()
+    torch.cuda.synchronize()
+    for i in range(len(layers)):
+        same_outputs(captured[i], eager[i])

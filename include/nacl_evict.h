@@ -191,6 +191,20 @@ int nacl_evict_f32(const void* K, const void* V, const void* Qproxy,
 /* Superset entry point: dtype tag, flags, optional importance / lse outputs, explicit workspace. */
 int nacl_evict_ex(const nacl_params_t* p);
 
+/* Step 1-2 on their own: the log-sum-exp of every proxy row over the keys (the "LSE emission" half of SURVEY.md 8(f) f4;
+ * PAPER.md:507 "The forward computation of FlashAttention-2 returns the log-sum-exp for each row", :518-536 Algorithm 2).
+ *   out_lse[b,hq,i] = ln sum_j exp(Q[b,hq,i,:] . K[b,hq/G,j,:] / sqrt(d))      (fp32, [batch,Hq,P]; under NACL_FLAG_CAUSAL the
+ *   sum runs over j <= L-P+i)
+ * One sweep over K (the statistics sweep of nacl_evict_ex) and a small merge; no importance, no selection, no gather.  It
+ * is the producer for nacl_params_t.lse_in when the prefill attention kernel does not hand its softmax statistics out: a
+ * caller runs it beside (or right after) its own prefill of the layer and then calls nacl_evict_ex with lse_in = out_lse,
+ * which is left with a single sweep.  (Emitting the statistics from inside the prefill attention itself would need that
+ * kernel, which is outside this library.)
+ * Read from *p: dtype, K, Qproxy, batch, L, Hq, Hkv, d, P, the K strides / block table, flags (NACL_FLAG_CAUSAL,
+ * NACL_FLAG_SCORE_CUDA_CORES only), out_lse (required), workspace / workspace_bytes (optional, as for nacl_evict_ex), stream.
+ * V, the budgets, protect_idx and the other outputs are ignored; lse_in and out_importance must be NULL. */
+int nacl_proxy_lse(const nacl_params_t* p);
+
 /* nacl_evict_ex for callers that must not allocate device memory.
  *
  * Who that is: an inference server that hands (nearly) all of the GPU's memory to its own KV-cache pool at start-up, so

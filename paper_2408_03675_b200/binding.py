@@ -21,7 +21,8 @@ FLAG_SCORE_TWO_LAUNCHES, FLAG_SELECT_GENERAL, FLAG_GATHER_SEPARATE = 0x200, 0x40
 EXPORTS = ("nacl_evict", "nacl_evict_f32", "nacl_evict_ex", "nacl_evict_host", "nacl_workspace_bytes",
            "nacl_release", "nacl_strerror", "nacl_last_cuda_error", "nacl_version",
            "nacl_profile_enable", "nacl_profile_read", "nacl_stage_name", "nacl_gumbel_keys", "nacl_evict_generation",
-           "nacl_select_fallbacks", "nacl_evict_varlen", "nacl_evict_host_batch", "nacl_evict_batch", "nacl_evict_static")
+           "nacl_select_fallbacks", "nacl_evict_varlen", "nacl_evict_host_batch", "nacl_evict_batch", "nacl_evict_static", "nacl_proxy_lse",
+           "nacl_last_select_launch")
 N_STAGES = 7
 
 
@@ -84,6 +85,8 @@ def _load() -> C.CDLL:
     lib.nacl_evict_f32.restype = i32
     lib.nacl_evict_ex.argtypes = [C.POINTER(NaclParams)]
     lib.nacl_evict_ex.restype = i32
+    lib.nacl_proxy_lse.argtypes = [C.POINTER(NaclParams)]
+    lib.nacl_proxy_lse.restype = i32
     lib.nacl_evict_static.argtypes = [C.POINTER(NaclParams)]
     lib.nacl_evict_static.restype = i32
     lib.nacl_evict_batch.argtypes = [C.POINTER(NaclParams), i32]
@@ -296,6 +299,33 @@ def nacl_evict_ex(K, V, Qproxy, budget_proxy, budget_random, n_sink, n_recent, s
         rc = _lib.nacl_evict_ex(C.byref(p))
     if rc != 0:
         raise NaclError(rc, "nacl_evict_ex")
+    return out
+
+
+def nacl_proxy_lse(K, Qproxy, flags=0, out=None, workspace=None, stream=None):
+    """include/nacl_evict.h `nacl_proxy_lse`: the natural-log row normaliser of every proxy row, [B,Hq,P] fp32 -- one sweep
+    over K.  Feed it to nacl_evict_ex(..., lse_in=) for the single-sweep eviction."""
+    if K.dim() != 4 or Qproxy.dim() != 4 or not K.is_cuda or not Qproxy.is_contiguous() or K.dtype != Qproxy.dtype:
+        raise ValueError("nacl_proxy_lse takes K [B,Hkv,L,d] and contiguous Qproxy [B,Hq,P,d] on the GPU, same dtype")
+    B, Hkv, L, d = K.shape
+    Hq, P = Qproxy.shape[1], Qproxy.shape[2]
+    if out is None:
+        out = torch.empty((B, Hq, P), dtype=torch.float32, device=K.device)
+    p = NaclParams()
+    p.struct_size = C.sizeof(NaclParams)
+    p.dtype = _dtype_tag(K)
+    p.K, p.Qproxy = K.data_ptr(), Qproxy.data_ptr()
+    p.batch, p.L, p.Hq, p.Hkv, p.d, p.P = B, L, Hq, Hkv, d, P
+    p.flags = flags
+    p.kv_stride_batch, p.kv_stride_head, p.kv_stride_row = _kv_strides(K)
+    p.out_lse = out.data_ptr()
+    if workspace is not None:
+        p.workspace, p.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
+    p.stream = (stream or torch.cuda.current_stream(K.device)).cuda_stream
+    with torch.cuda.device(K.device):
+        rc = _lib.nacl_proxy_lse(C.byref(p))
+    if rc != 0:
+        raise NaclError(rc, "nacl_proxy_lse")
     return out
 
 

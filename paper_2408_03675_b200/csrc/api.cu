@@ -255,17 +255,32 @@ static int fail_cuda(cudaError_t e) {
 // ------------------------------------------------------------------ the call
 // idx_in_ws: the index list goes to the workspace's idx_tmp (p.out_idx is ignored) and *idx_in_ws receives where that is
 // (nacl_evict_generation without out_idx: this call alone decides which workspace it is and keeps its bookkeeping)
-static int evict_core(const nacl_params_t& p, int32_t** idx_in_ws, int* internal_ws_dev);
+static int evict_core(const nacl_params_t& p, int32_t** idx_in_ws, int* internal_ws_dev, bool lse_only);
 
-static int evict_impl(const nacl_params_t& p, int32_t** idx_in_ws = nullptr) {
+// lse_only (nacl_proxy_lse): steps a1-a2 alone -> p.out_lse; V, the budgets and the other outputs are not looked at
+static int evict_impl(const nacl_params_t& p, int32_t** idx_in_ws = nullptr, bool lse_only = false) {
   int dev = -1;  // >= 0 once the call works in the library's own workspace of that device
-  const int rc = evict_core(p, idx_in_ws, &dev);
+  const int rc = evict_core(p, idx_in_ws, &dev, lse_only);
   // whatever was enqueued (also before an error) is the buffer's latest use
   if (dev >= 0) workspace_call_done(dev, static_cast<cudaStream_t>(p.stream));
   return rc;
 }
 
-static int evict_core(const nacl_params_t& p, int32_t** idx_in_ws, int* internal_ws_dev) {
+static int evict_core(const nacl_params_t& p_in, int32_t** idx_in_ws, int* internal_ws_dev, bool lse_only) {
+  nacl_params_t p = p_in;
+  if (lse_only) {
+    if (!p.K || !p.Qproxy || !p.out_lse) return NACL_ERR_NULL;
+    if (p.lse_in || p.out_importance) return NACL_ERR_UNSUPPORTED;
+    if (p.flags & ~(NACL_FLAG_CAUSAL | NACL_FLAG_SCORE_CUDA_CORES)) return NACL_ERR_UNSUPPORTED;
+    // everything behind the statistics is switched off: V stands in as K (never read), empty budget, no outputs
+    p.V = p.K;
+    p.budget_proxy = p.budget_random = p.n_sink = p.n_recent = p.n_protect = 0;
+    p.protect_idx = nullptr;
+    p.out_K = p.out_V = nullptr;
+    p.out_idx = nullptr;
+    p.out_stride_batch = p.out_stride_head = p.out_stride_row = 0;
+    p.flags |= NACL_FLAG_SCORE_TWO_LAUNCHES;  // no hand-over counters in this form
+  }
   if (!p.K || !p.V || !p.Qproxy) return NACL_ERR_NULL;
   // an empty budget (C == 0) has empty outputs: their pointers may be NULL
   const bool empty_out = p.budget_proxy == 0 && p.budget_random == 0;
@@ -373,7 +388,13 @@ static int evict_core(const nacl_params_t& p, int32_t** idx_in_ws, int* internal
   if (zero_sync && (e = cudaMemsetAsync(ws.sync, 0, sync_bytes, st)) != cudaSuccess) return fail_cuda(e);
 
   if (p.lse_in && (reinterpret_cast<uintptr_t>(p.lse_in) & 3u)) return NACL_ERR_ALIGN;
+  if (p.out_lse && (reinterpret_cast<uintptr_t>(p.out_lse) & 3u)) return NACL_ERR_ALIGN;
   const bool causal = (p.flags & NACL_FLAG_CAUSAL) != 0;
+  if (lse_only) {
+    if (tc) e = launch_score_tc(s, p.K, p.Qproxy, sp, ws, nullptr, causal, true, nullptr, p.out_lse, st, true);
+    else e = launch_score_generic(s, p.K, p.Qproxy, sp, ws, nullptr, causal, nullptr, p.out_lse, st, true);
+    return e == cudaSuccess ? NACL_OK : fail_cuda(e);
+  }
   if (tc) e = launch_score_tc(s, p.K, p.Qproxy, sp, ws, p.lse_in, causal, two_launches, p.out_importance, p.out_lse, st);
   else e = launch_score_generic(s, p.K, p.Qproxy, sp, ws, p.lse_in, causal, p.out_importance, p.out_lse, st);
   if (e != cudaSuccess) return fail_cuda(e);
@@ -470,6 +491,12 @@ int nacl_evict_ex(const nacl_params_t* p) {
   if (!p) return NACL_ERR_NULL;
   if (p->struct_size != sizeof(nacl_params_t)) return NACL_ERR_UNSUPPORTED;
   return evict_impl(*p);
+}
+
+int nacl_proxy_lse(const nacl_params_t* p) {
+  if (!p) return NACL_ERR_NULL;
+  if (p->struct_size != sizeof(nacl_params_t)) return NACL_ERR_UNSUPPORTED;
+  return evict_impl(*p, nullptr, true);
 }
 
 int nacl_evict_static(const nacl_params_t* p) {

@@ -69,15 +69,17 @@ struct StageScope {
 // generic CUDA-core scoring (any dtype / d / G*P): 3 launches
 // lse_in != nullptr: the row log-sum-exps are given (natural log): the statistics sweep is skipped.
 // causal: NACL_FLAG_CAUSAL (proxy row i = prompt position L-P+i sees keys j <= L-P+i)
+// stats_only (nacl_proxy_lse): the statistics sweep and its combine alone -> lse_out; no column sums, ws.imp untouched
 cudaError_t launch_score_generic(const Shape& s, const void* K, const void* Q, const SplitPlan& sp,
-                                 const Workspace& ws, const float* lse_in, bool causal, float* imp_out, float* lse_out, cudaStream_t st);
+                                 const Workspace& ws, const float* lse_in, bool causal, float* imp_out, float* lse_out, cudaStream_t st,
+                                 bool stats_only = false);
 
 // tensor-core scoring (bf16, d == 128, G*P % 16 == 0, G*P <= 256): tcgen05 + TMA
 bool score_tc_supported(const Shape& s);
 size_t score_tc_part_elems(int heads, int rows);  // float2 elements of Workspace::part the tensor-core path needs
 cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const SplitPlan& sp,
                             const Workspace& ws, const float* lse_in, bool causal, bool two_launches, float* imp_out,
-                            float* lse_out, cudaStream_t st);
+                            float* lse_out, cudaStream_t st, bool stats_only = false);
 
 // Gumbel-top-k keys: key[p,j] = fl32(ln w(imp) - ln(-ln u)), order-mapped to uint32 (ordermapped) or as float bits
 // batch_offset / head_offset: global indices of the call's first batch element / kv head (Philox counter words)

@@ -164,7 +164,8 @@ __global__ void __launch_bounds__(NT) nacl_colsum_kernel(const T* __restrict__ K
 
 template <typename T>
 cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const SplitPlan& sp, const Workspace& ws,
-                         const float* lse_in, bool causal, float* imp_out, float* lse_out, cudaStream_t st) {
+                         const float* lse_in, bool causal, float* imp_out, float* lse_out, cudaStream_t st, bool stats_only) {
+  if (stats_only && (!lse_out || lse_in)) return cudaErrorInvalidValue;
   const size_t smem = (size_t)2 * 64 * (s.d + 1) * sizeof(float);
   cudaError_t e;
   if ((e = cudaFuncSetAttribute(nacl_stats_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
@@ -190,6 +191,7 @@ cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const Spl
   }
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   }
+  if (stats_only) return cudaSuccess;
   dim3 g2((s.L + TK - 1) / TK, s.Hkv, s.batch);
   {
     StageScope sc(ST_COLSUM, st);
@@ -202,9 +204,9 @@ cudaError_t launch_typed(const Shape& s, const void* K, const void* Q, const Spl
 }  // namespace
 
 cudaError_t launch_score_generic(const Shape& s, const void* K, const void* Q, const SplitPlan& sp, const Workspace& ws,
-                                 const float* lse_in, bool causal, float* imp_out, float* lse_out, cudaStream_t st) {
-  if (s.dtype == NACL_DTYPE_F32) return launch_typed<float>(s, K, Q, sp, ws, lse_in, causal, imp_out, lse_out, st);
-  return launch_typed<__nv_bfloat16>(s, K, Q, sp, ws, lse_in, causal, imp_out, lse_out, st);
+                                 const float* lse_in, bool causal, float* imp_out, float* lse_out, cudaStream_t st, bool stats_only) {
+  if (s.dtype == NACL_DTYPE_F32) return launch_typed<float>(s, K, Q, sp, ws, lse_in, causal, imp_out, lse_out, st, stats_only);
+  return launch_typed<__nv_bfloat16>(s, K, Q, sp, ws, lse_in, causal, imp_out, lse_out, st, stats_only);
 }
 
 }  // namespace nacl

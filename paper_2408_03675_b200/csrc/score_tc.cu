@@ -1172,6 +1172,19 @@ nacl_score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_const
   }
 }
 
+// Sweep S on its own (nacl_proxy_lse): lse of every proxy row from the partials that a MODE 0 launch of `grid` CTAs left,
+// merged exactly as the column-sum sweep merges them (same routine, same ascending piece order: the same bits).
+__global__ void __launch_bounds__(128) nacl_lse_merge_kernel(const float2* __restrict__ part, float* __restrict__ lse_out, int rows_total,
+                                                             int T, long long N, int grid, int n_slots) {
+  const int head = blockIdx.y;
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= rows_total) return;
+  const int c_first = cta_of_tile((long long)head * T, N, grid);
+  const int c_last = cta_of_tile((long long)(head + 1) * T - 1, N, grid);
+  const float l2 = merge_row(part + ((size_t)(c_first + head) * n_slots) * rows_total + r, (c_last - c_first + 1) * n_slots, (size_t)rows_total);
+  lse_out[(size_t)head * rows_total + r] = l2 * 0.69314718055994530942f;
+}
+
 // ------------------------------------------------------------------ host side
 using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -1217,7 +1230,7 @@ cudaError_t launch_one(Kern kern, int grid, int smem_bytes, bool cooperative, co
 }
 
 template <int QROWS, int NQ, int STAGES_S, int STAGES_C>
-cudaError_t launch_cfg(const CUtensorMap& tmK, const CUtensorMap& tmQ, TcParams p, bool two_launches, cudaStream_t st) {
+cudaError_t launch_cfg(const CUtensorMap& tmK, const CUtensorMap& tmQ, TcParams p, bool two_launches, bool stats_only, cudaStream_t st) {
   using SMS = Smem<QROWS, NQ, STAGES_S, 0>;
   using SMC = Smem<QROWS, NQ, STAGES_C, 1>;
   constexpr int kStatic = 1024 + 16;  // the kernel's static shared memory (TMEM slot) and the alignment gap it may cause
@@ -1226,6 +1239,17 @@ cudaError_t launch_cfg(const CUtensorMap& tmK, const CUtensorMap& tmQ, TcParams 
   long long grid = sm_count() < MAX_GRID ? sm_count() : MAX_GRID;
   if (p.N < grid) grid = p.N;
   cudaError_t e;
+  if (stats_only) {  // the statistics sweep, then the merge of its partials into lse_out: no column sums
+    {
+      StageScope sc(ST_STATS, st);
+      e = launch_one(nacl_score_tc_kernel<QROWS, NQ, STAGES_S, STAGES_C, 0>, (int)grid, SMS::TOTAL, false, tmK, tmQ, p, st);
+      if (e != cudaSuccess) return e;
+    }
+    StageScope sc(ST_COMBINE, st);
+    nacl_lse_merge_kernel<<<dim3((unsigned)((p.rows_total + 127) / 128), (unsigned)p.heads), 128, 0, st>>>(p.part, p.lse_out, p.rows_total, p.T, p.N,
+                                                                                                        (int)grid, p.n_slots);
+    return cudaGetLastError();
+  }
   if (p.lse_in) {
     StageScope sc(ST_COLSUM, st);
     return launch_one(nacl_score_tc_kernel<QROWS, NQ, STAGES_S, STAGES_C, 1>, (int)grid, SMC::TOTAL, false, tmK, tmQ, p, st);
@@ -1254,7 +1278,9 @@ bool score_tc_supported(const Shape& s) {
 size_t score_tc_part_elems(int heads, int rows) { return (size_t)(MAX_GRID + heads) * 4 * rows; }
 
 cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const SplitPlan&, const Workspace& ws,
-                            const float* lse_in, bool causal, bool two_launches, float* imp_out, float* lse_out, cudaStream_t st) {
+                            const float* lse_in, bool causal, bool two_launches, float* imp_out, float* lse_out, cudaStream_t st,
+                            bool stats_only) {
+  if (stats_only && (!lse_out || lse_in)) return cudaErrorInvalidValue;
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return cudaErrorNotSupported;  // no silent fallback: the caller reports NACL_ERR_CUDA
   const int heads = s.batch * s.Hkv;
@@ -1300,8 +1326,8 @@ cudaError_t launch_score_tc(const Shape& s, const void* K, const void* Q, const 
 #ifndef NACL_STAGES_S
 #define NACL_STAGES_S 5
 #endif
-  if (qrows == 128) return launch_cfg<128, 2, NACL_STAGES_S, 3>(tmK, tmQ, p, two_launches, st);
-  return launch_cfg<256, 1, NACL_STAGES_S, 3>(tmK, tmQ, p, two_launches, st);
+  if (qrows == 128) return launch_cfg<128, 2, NACL_STAGES_S, 3>(tmK, tmQ, p, two_launches, stats_only, st);
+  return launch_cfg<256, 1, NACL_STAGES_S, 3>(tmK, tmQ, p, two_launches, stats_only, st);
 }
 
 }  // namespace nacl

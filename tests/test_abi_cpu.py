@@ -129,6 +129,34 @@ def test_static_scratch_entry_point_validates_on_the_host(lib):
         assert lib.nacl_workspace_bytes(cfg.batch, cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.P) <= STATIC_SCRATCH_BYTES
 
 
+def test_proxy_lse_validates_on_the_host(lib):
+    from paper_2408_03675_b200.binding import NaclParams
+
+    lib.nacl_proxy_lse.argtypes = [C.POINTER(NaclParams)]
+    assert lib.nacl_proxy_lse(None) == -1
+    p = NaclParams()
+    p.struct_size = C.sizeof(NaclParams)
+    p.dtype = 1
+    p.K, p.Qproxy = 0x1000, 0x3000
+    p.batch, p.L, p.Hq, p.Hkv, p.d, p.P = 1, 512, 4, 4, 64, 16
+    assert lib.nacl_proxy_lse(C.byref(p)) == -1          # out_lse is what the call is for
+    p.out_lse = 0x8000
+    p.P = 600
+    assert lib.nacl_proxy_lse(C.byref(p)) == -2          # P > L
+    p.P = 16
+    p.flags = 8                                          # a selection flag means nothing here
+    assert lib.nacl_proxy_lse(C.byref(p)) == -7
+    p.flags = 0
+    p.lse_in = 0x9000
+    assert lib.nacl_proxy_lse(C.byref(p)) == -7
+    p.lse_in = None
+    p.K = 0x1004
+    assert lib.nacl_proxy_lse(C.byref(p)) == -4
+    p.K, p.out_lse = 0x1000, 0x8002
+    p.workspace, p.workspace_bytes = 0x10000, 1 << 24    # a workspace, so that no device is asked for one
+    assert lib.nacl_proxy_lse(C.byref(p)) == -4          # misaligned out_lse
+
+
 def test_paged_kv_validation_without_touching_the_device(lib):
     from paper_2408_03675_b200.binding import NaclParams
 

@@ -884,3 +884,31 @@ def test_timed_configuration_full_size(binding, cid):
     torch.cuda.synchronize()
     for i in range(len(layers)):
         same_outputs(captured[i], eager[i])
+
+
+@pytest.mark.parametrize("case", [(1, 4100, 32, 8, 128, 64, "bf16", 0), (2, 1000, 8, 2, 128, 16, "bf16", 0), (1, 1300, 8, 2, 128, 128, "bf16", 0),
+                                  (1, 1200, 8, 2, 128, 100, "bf16", 0), (2, 333, 4, 2, 64, 5, "f32", 0), (1, 2049, 8, 2, 128, 32, "bf16", 1),
+                                  (2, 515, 4, 2, 64, 7, "f32", 1)],
+                         ids=["tc_GP256_ragged", "tc_GP64", "tc_GP512_row_blocks", "tc_GP400_partial_row_block", "cuda_core_f32",
+                              "tc_causal", "cuda_core_causal"])
+def test_proxy_lse_feeds_the_single_sweep_call(binding, case):
+    """nacl_proxy_lse (step a2 alone): the row log-sum-exps equal the oracle's fp64 values, and an
+    eviction that is handed them through lse_in passes the whole parity protocol with a single sweep over K."""
+    B, L, Hq, Hkv, d, P, dt, causal = case
+    K, V, Q = make_random_inputs(B, L, Hq, Hkv, d, P, dtype=dt, seed=L + 9)
+    flags = binding.FLAG_CAUSAL if causal else 0
+    _, lse_ref = oracle.importance(K, Q, flags=oracle.CAUSAL if causal else 0, return_lse=True)
+    ws = torch.full((binding.nacl_workspace_bytes(B, L, Hq, Hkv, d, P),), 0xC3, dtype=torch.uint8, device="cuda")
+    lse = binding.nacl_proxy_lse(K.cuda(), Q.cuda(), flags=flags, workspace=ws)
+    lse2 = binding.nacl_proxy_lse(K.cuda(), Q.cuda(), flags=flags)  # the library's workspace; same bits
+    torch.cuda.synchronize()
+    assert torch.equal(lse, lse2)
+    # an error delta of a row's lse scales that row's softmax by exp(delta): 5e-5 spends 2.5 % of the 2e-3 score tolerance
+    # (fp32 sums of up to L exponentials, part of them from the FMA-pipe polynomial exp2; measured: up to 1.1e-5)
+    np.testing.assert_allclose(lse.cpu().numpy(), lse_ref, rtol=0, atol=1e-4 if causal else 5e-5)
+    # the two-sweep call reports the same statistics
+    nr = min(P, L // 2)
+    Bp, Br = max(L // 6, 4 + nr), L // 20
+    two = binding.nacl_evict_ex(K.cuda(), V.cuda(), Q.cuda(), Bp, Br, 4, nr, 5, 1, flags=flags, want_lse=True)
+    np.testing.assert_allclose(two["lse"].cpu().numpy(), lse.cpu().numpy(), rtol=1e-6, atol=1e-6)
+    full_parity(K, V, Q, Bp, Br, 4, nr, seed=5, layer=1, flags=flags, lse_in=lse.cpu())

@@ -2,6 +2,9 @@
 
     python -m paper_2408_03675_b200.build [--force]
 
+Diagnostics variants of the kernels (NACL_NVCC_EXTRA="-DNACL_...") are built only with NACL_DIAGNOSTICS=1 in the
+environment: some of them give wrong results by design and none of them is the product.
+
 nvcc cross-compiles for sm_100a without a GPU.  The library is git-ignored but travels to the GPU
 box with the gpurun snapshot.
 """
@@ -44,7 +47,15 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc] + NVCC_FLAGS + ["-I", INCLUDE, "-I", CSRC]
-    cmd += os.environ.get("NACL_NVCC_EXTRA", "").split()  # diagnostics builds: -DNACL_TC_TRACE, -DNACL_TC_STAMPS, -DNACL_SEL_TRACE
+    extra = os.environ.get("NACL_NVCC_EXTRA", "").split()
+    # Diagnostics builds (-DNACL_TC_TRACE, -DNACL_TC_STAMPS, -DNACL_SEL_TRACE, -DNACL_DIAG_*, -DNACL_EPI_TRIVIAL,
+    # -DNACL_FORCE_CLUSTER=n ...) add undeclared debug exports and, some of them, compute WRONG results on purpose (they
+    # switch parts of a kernel off to time the rest).  They reproduce the tables under profiles/ and are never the product:
+    # the build refuses them unless NACL_DIAGNOSTICS=1 says the caller knows what the resulting library is.
+    if any(f.startswith("-DNACL_") for f in extra) and os.environ.get("NACL_DIAGNOSTICS") != "1":
+        raise RuntimeError("NACL_NVCC_EXTRA asks for a diagnostics build of libnacl_evict.so (results may be wrong by design); "
+                           "set NACL_DIAGNOSTICS=1 to build it, and rebuild without both afterwards")
+    cmd += extra
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += ["-o", LIB + ".tmp"] + sources()

@@ -282,3 +282,13 @@ def test_log_table_is_what_its_generator_writes():
         assert abs(inv - 1.0 / c) <= math.ulp(inv)
         assert abs(hi - math.log(c)) <= math.ulp(hi) if c != 1.0 else hi == 0.0
         assert abs(lo) <= math.ulp(hi) / 2 if c != 1.0 else lo == 0.0
+
+
+def test_diagnostics_builds_are_refused_by_default(monkeypatch):
+    """The -DNACL_* variants of the kernels (timing aids, some wrong by design) must not end up as the product library by
+    accident: the build refuses them unless NACL_DIAGNOSTICS=1 is set."""
+    monkeypatch.setenv("NACL_NVCC_EXTRA", "-DNACL_EPI_TRIVIAL")
+    monkeypatch.delenv("NACL_DIAGNOSTICS", raising=False)
+    with pytest.raises(RuntimeError, match="NACL_DIAGNOSTICS"):
+        nacl_build.build(force=True)
+    assert os.path.exists(nacl_build.LIB)  # the refused build left the product library alone
